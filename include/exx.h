@@ -1,0 +1,141 @@
+/*
+ * exx.h — C ABI of libexx: plane-wave Fock-exchange operator V_x|psi_nk> and exchange energy E_x on one B200.
+ *
+ * The operation (PAPER.md = arXiv 1111.0716; P:Lnn is line nn of it):
+ *   - FOCK_ACC "applies the Fock exchange operator"; the exchange energy is Eq. 2;
+ *   - four nested loops, two over k-points k,q and two over bands n,m; the band loops run on the GPU and every
+ *     operation inside them stays on the device;
+ *   - FFTs, scatter/gather "used to express cutoffs", data-manipulation kernels;
+ *   - library contexts created/destroyed at the start/end of the program.
+ * On the FFT grid this is definition (D) of DESIGN.md section 2 (Hartree atomic units, no spin factor):
+ *   u_nk(r_j)       = sum_{g in sphere(k)} c_nk(g) e^{+i G.r_j}
+ *   rho~_{nk,mq}(g) = (1/Ng) sum_j conj(u_mq(r_j)) u_nk(r_j) e^{-i G.r_j}
+ *   v_{nk,mq}(r_j)  = (1/Omega) sum_g K(|k-q+G|) rho~_{nk,mq}(g) e^{+i G.r_j}
+ *   (V_x u)_nk(r_j) = - sum_q w_q sum_m f_mq u_mq(r_j) v_{nk,mq}(r_j)
+ *   (V_x c)_nk(g)   = (1/Ng) sum_j (V_x u)_nk(r_j) e^{-i G.r_j},  g in sphere(k) = { g : |k+G|^2/2 < E_cut }
+ *   E_x             = 1/2 sum_k w_k sum_n f_nk Re <c_nk | (V_x c)_nk>
+ *
+ * Conventions
+ *   - complex numbers: interleaved (re, im) fp64.  All arithmetic is fp64.
+ *   - FFT box: C order, index (j1*N2 + j2)*N3 + j3; integer frequency g_i = j_i if 2 j_i < N_i else j_i - N_i.
+ *   - sphere(k) is listed by ascending box index; exx_index_map returns that list (bit-exact contract).
+ *   - psi / out layout: k-major, then band, then sphere index: element (k,n,ig) at
+ *       exx_psi_offset(k) + n*npw(k) + ig   (complex elements),  exx_psi_offset(k) = nbands * sum_{k'<k} npw(k').
+ *   - pointers named *_dev are device (HBM) pointers, *_host are host pointers; both are owned by the caller.
+ *     The context owns its index maps, kernel tables, the real-space cache u_nk(r) and all workspaces; they are
+ *     allocated in exx_create and freed in exx_destroy.  exx_apply allocates nothing.
+ *   - every call returns EXX_OK (0) or a negative error code; no exceptions, no abort, nothing printed.
+ *     On error, output arguments are left untouched.  exx_last_error() gives detail for EXX_ERR_CUDA.
+ *   - work is enqueued on the CUDA stream given to exx_create (a cudaStream_t cast to void*; NULL = default
+ *     stream).  exx_apply returns without synchronising; exx_energy and the *_host calls synchronise that stream.
+ */
+#ifndef EXX_H
+#define EXX_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct exx_ctx exx_ctx; /* opaque */
+
+typedef struct {
+    int kind;     /* 0: bare Coulomb 4 pi/Q^2, term at k-q+G = 0 set to 0;
+                     1: HSE short range (4 pi/Q^2)(1 - exp(-Q^2/(4 mu^2))), term at k-q+G = 0 is pi/mu^2 */
+    double mu;    /* bohr^-1, used when kind == 1 (HSE06: 0.106) */
+    double scale; /* multiplies K (1.0 in all BASELINE configs; HSE06's 1/4 mixing is NOT applied implicitly) */
+} exx_kernel_params;
+
+enum {
+    EXX_OK = 0,
+    EXX_ERR_NULL = -1,        /* a required pointer is NULL */
+    EXX_ERR_BAD_GRID = -2,    /* N_i not of the form 2^a 3^b (a+b >= 1), N_i > 1024, or the cutoff sphere does not fit the box */
+    EXX_ERR_BAD_LATTICE = -3, /* zero or non-finite cell volume */
+    EXX_ERR_BAD_CUTOFF = -4,  /* E_cut <= 0 or non-finite, or an empty sphere */
+    EXX_ERR_BAD_KERNEL = -5,  /* unknown kind, mu <= 0 for HSE, non-finite scale */
+    EXX_ERR_BAD_OCC = -6,     /* an occupation is negative or non-finite */
+    EXX_ERR_ALLOC = -7,       /* host or device allocation failed */
+    EXX_ERR_CUDA = -8,        /* a CUDA call or kernel launch failed; see exx_last_error */
+    EXX_ERR_BAD_ARG = -9,     /* index out of range, nk/nbands < 1, weights not finite, unknown option */
+    EXX_ERR_ALIAS = -10       /* out aliases psi */
+};
+
+/* Options (exx_set_option / exx_get_option).  All are tuning knobs: results may differ only by rounding order. */
+enum {
+    EXX_OPT_PATH = 1,       /* 0 auto (fused kernels when the grid is supported, else generic), 1 generic per-axis kernels, 2 fused */
+    EXX_OPT_TILE_N = 2,     /* bands n per tile (0 = auto) */
+    EXX_OPT_TILE_M = 3,     /* bands m per tile (0 = auto) */
+    EXX_OPT_PRUNE = 4,      /* 1 (default): skip transforms whose input/output is zero by band limit, only when alias-free */
+    EXX_OPT_PROFILE = 5     /* 1: bracket every kernel launch with CUDA events so exx_get_kernel_time works (slower) */
+};
+
+/* Counters (exx_get_info), all for the most recent exx_apply on this context unless stated. */
+enum {
+    EXX_INFO_LAUNCHES = 1,        /* kernels launched */
+    EXX_INFO_PAIRS_ORDERED = 2,   /* ordered band-pair exchange evaluations covered: sum over (k,q) of Nb * Nocc(q) */
+    EXX_INFO_PAIRS_EXECUTED = 3,  /* pair FFT round trips actually executed (== ordered unless a symmetry is exploited) */
+    EXX_INFO_PATH_USED = 4,       /* 1 generic, 2 fused */
+    EXX_INFO_WORKSPACE_BYTES = 5, /* device bytes owned by the context */
+    EXX_INFO_NCOEF = 6,           /* complex elements in psi / out */
+    EXX_INFO_TILE_N = 7,
+    EXX_INFO_TILE_M = 8,
+    EXX_INFO_PRUNED = 9,          /* 1 if band-limit pruning was active */
+    EXX_INFO_NUM_KERNEL_CLASSES = 10
+};
+
+/* Create a context.  grid: N1,N2,N3.  lattice: 9 doubles, row i = a_i in bohr.  kfrac: nk*3 fractional reciprocal
+ * coordinates kappa (k = sum kappa_i b_i, a_i.b_j = 2 pi delta_ij).  kweight: nk weights w_k (the caller makes them
+ * sum to 1).  All host pointers, read during the call only.  Builds index maps, the kernel tables
+ * K'_{k-q}(g) = K(|k-q+G|)/(Omega Ng^2) for every distinct k-q, twiddle tables and workspaces (host work + H2D). */
+int exx_create(exx_ctx** out, const int grid[3], const double lattice[9], int nk, const double* kfrac_host,
+               const double* kweight_host, double ecut_hartree, const exx_kernel_params* kp, int nbands, void* cuda_stream);
+int exx_destroy(exx_ctx* ctx);
+
+/* Queries (host). */
+int exx_npw(const exx_ctx* ctx, int ik, int* npw);
+int exx_index_map(const exx_ctx* ctx, int ik, int32_t* host_out /* npw(ik) entries */);
+int exx_psi_offset(const exx_ctx* ctx, int ik /* 0..nk; nk gives the total */, int64_t* complex_elems);
+int exx_set_option(exx_ctx* ctx, int option, int64_t value);
+int exx_get_option(const exx_ctx* ctx, int option, int64_t* value);
+int exx_get_info(const exx_ctx* ctx, int what, int64_t* value);
+/* With EXX_OPT_PROFILE = 1: device time (CUDA events on the context's stream) and launch count of kernel class
+ * `kclass` (0 .. EXX_INFO_NUM_KERNEL_CLASSES-1) during the most recent exx_apply; synchronises the stream.
+ * exx_kernel_class_name gives the class name (static string, NULL if out of range). */
+int exx_get_kernel_time(exx_ctx* ctx, int kclass, double* ms_total, int64_t* launches);
+const char* exx_kernel_class_name(int kclass);
+
+/* V_x applied to every band: out(k,n,:) = (V_x c)_nk.  psi_dev/out_dev: device, exx_psi_offset(nk) complex elements
+ * each, 16-byte aligned, must not overlap.  occ_host: nk*nbands occupations f_nk in [0, inf), host, read during the
+ * call.  Bands with f = 0 are skipped as m (they contribute exactly 0) and kept as n.  Asynchronous on the stream. */
+int exx_apply(exx_ctx* ctx, const double* psi_dev, const double* occ_host, double* out_dev);
+
+/* E_x = 1/2 sum w_k f_nk Re<c_nk|(V_x c)_nk>.  If vxpsi_dev_or_null is NULL the library first applies V_x into an
+ * internal buffer.  ex_host: 1 double.  per_band_host_or_null: nk*nbands terms 1/2 w_k f_nk Re<c|V_x c> (or NULL).
+ * Synchronises the stream. */
+int exx_energy(exx_ctx* ctx, const double* psi_dev, const double* occ_host, const double* vxpsi_dev_or_null, double* ex_host,
+               double* per_band_host_or_null);
+
+/* Same as exx_apply (+ exx_energy when ex_host_or_null != NULL) on HOST buffers: copies psi to the device, applies,
+ * copies out back; synchronises.  Pinned host memory makes the copies asynchronous, pageable memory works too. */
+int exx_apply_host(exx_ctx* ctx, const double* psi_host, const double* occ_host, double* out_host, double* ex_host_or_null);
+
+/* Building blocks exposed for parity tests and stand-alone use (all asynchronous on the stream, device pointers):
+ * exx_scatter: box(b, map_k[ig]) = coef(b, ig), zero elsewhere; exx_gather: the reverse (pure data movement, bit exact);
+ * exx_fft3d: in-place unnormalised 3-D transform of nbatch boxes, sign = -1 forward (e^{-i G.r}), +1 inverse;
+ * exx_to_real: u = scatter + inverse transform (step S1). */
+int exx_scatter(exx_ctx* ctx, int ik, const double* coef_dev, int nbatch, double* box_dev);
+int exx_gather(exx_ctx* ctx, int ik, const double* box_dev, int nbatch, double* coef_dev);
+int exx_fft3d(exx_ctx* ctx, double* box_dev, int nbatch, int sign);
+int exx_to_real(exx_ctx* ctx, int ik, const double* coef_dev, int nbatch, double* box_dev);
+/* K'_{k-q}(g) as the library tabulated it (host_out: Ng doubles, C order). */
+int exx_kernel_table(const exx_ctx* ctx, int ik, int iq, double* host_out);
+
+const char* exx_strerror(int code);
+const char* exx_last_error(const exx_ctx* ctx_or_null); /* detail of the last EXX_ERR_CUDA (thread-local if ctx NULL) */
+int exx_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EXX_H */

@@ -1,0 +1,242 @@
+"""Thin Python binding of libexx (include/exx.h): argument marshalling only.
+
+Every step of the path runs in the CUDA library; torch is used for device memory and the stream handle.
+There is no CPU fallback: if libexx.so cannot be loaded, every entry point raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libexx.so")
+
+EXX_OPT_PATH, EXX_OPT_TILE_N, EXX_OPT_TILE_M, EXX_OPT_PRUNE, EXX_OPT_PROFILE = 1, 2, 3, 4, 5
+(EXX_INFO_LAUNCHES, EXX_INFO_PAIRS_ORDERED, EXX_INFO_PAIRS_EXECUTED, EXX_INFO_PATH_USED, EXX_INFO_WORKSPACE_BYTES,
+ EXX_INFO_NCOEF, EXX_INFO_TILE_N, EXX_INFO_TILE_M, EXX_INFO_PRUNED, EXX_INFO_NUM_KERNEL_CLASSES) = range(1, 11)
+
+# every symbol include/exx.h declares (tests/test_abi.py checks the library exports them all)
+SYMBOLS = ("exx_create", "exx_destroy", "exx_npw", "exx_index_map", "exx_psi_offset", "exx_set_option", "exx_get_option",
+           "exx_get_info", "exx_get_kernel_time", "exx_kernel_class_name", "exx_apply", "exx_energy", "exx_apply_host",
+           "exx_scatter", "exx_gather", "exx_fft3d", "exx_to_real", "exx_kernel_table", "exx_strerror", "exx_last_error",
+           "exx_version")
+
+
+class KernelParams(C.Structure):
+    _fields_ = [("kind", C.c_int), ("mu", C.c_double), ("scale", C.c_double)]
+
+
+class ExxError(RuntimeError):
+    def __init__(self, code, detail=""):
+        self.code = code
+        msg = "libexx error %d: %s" % (code, lib().exx_strerror(code).decode())
+        if detail:
+            msg += " [" + detail + "]"
+        super().__init__(msg)
+
+
+_lib = None
+
+
+def lib():
+    """Load libexx.so (built in-tree by paper_1111_0716_b200.build).  Raises if it is missing: no fallback."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError("libexx.so not found at %s: build it with `python -m paper_1111_0716_b200.build` "
+                               "(there is no CPU fallback)" % LIB_PATH)
+        L = C.CDLL(LIB_PATH)
+        vp, dp, ip = C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int)
+        i64p = C.POINTER(C.c_int64)
+        L.exx_create.argtypes = [C.POINTER(vp), ip, dp, C.c_int, dp, dp, C.c_double, C.POINTER(KernelParams), C.c_int, vp]
+        L.exx_destroy.argtypes = [vp]
+        L.exx_npw.argtypes = [vp, C.c_int, ip]
+        L.exx_index_map.argtypes = [vp, C.c_int, C.POINTER(C.c_int32)]
+        L.exx_psi_offset.argtypes = [vp, C.c_int, i64p]
+        L.exx_set_option.argtypes = [vp, C.c_int, C.c_int64]
+        L.exx_get_option.argtypes = [vp, C.c_int, i64p]
+        L.exx_get_info.argtypes = [vp, C.c_int, i64p]
+        L.exx_get_kernel_time.argtypes = [vp, C.c_int, dp, i64p]
+        L.exx_kernel_class_name.argtypes = [C.c_int]
+        L.exx_kernel_class_name.restype = C.c_char_p
+        L.exx_apply.argtypes = [vp, vp, dp, vp]
+        L.exx_energy.argtypes = [vp, vp, dp, vp, dp, dp]
+        L.exx_apply_host.argtypes = [vp, vp, dp, vp, dp]
+        L.exx_scatter.argtypes = [vp, C.c_int, vp, C.c_int, vp]
+        L.exx_gather.argtypes = [vp, C.c_int, vp, C.c_int, vp]
+        L.exx_fft3d.argtypes = [vp, vp, C.c_int, C.c_int]
+        L.exx_to_real.argtypes = [vp, C.c_int, vp, C.c_int, vp]
+        L.exx_kernel_table.argtypes = [vp, C.c_int, C.c_int, dp]
+        L.exx_strerror.argtypes = [C.c_int]
+        L.exx_strerror.restype = C.c_char_p
+        L.exx_last_error.argtypes = [vp]
+        L.exx_last_error.restype = C.c_char_p
+        L.exx_version.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+class Exx:
+    """exx_ctx wrapper.  Methods carry the C names without the prefix: apply, energy, apply_host, ..."""
+
+    def __init__(self, grid, lattice, kfrac, kweight, ecut, kind=0, mu=0.0, scale=1.0, nbands=1, stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("libexx needs a CUDA device (no CPU fallback)")
+        self._torch = torch
+        L = lib()
+        self.grid = tuple(int(g) for g in grid)
+        self.ng = self.grid[0] * self.grid[1] * self.grid[2]
+        self.nk = len(kweight)
+        self.nbands = int(nbands)
+        lat = np.ascontiguousarray(lattice, dtype=np.float64).reshape(9)
+        kf = np.ascontiguousarray(kfrac, dtype=np.float64).reshape(self.nk * 3)
+        kw = np.ascontiguousarray(kweight, dtype=np.float64)
+        kp = KernelParams(int(kind), float(mu), float(scale))
+        self.stream = stream if stream is not None else torch.cuda.current_stream()
+        self._h = C.c_void_p()
+        g = (C.c_int * 3)(*self.grid)
+        rc = L.exx_create(C.byref(self._h), g, _dp(lat), self.nk, _dp(kf), _dp(kw), float(ecut), C.byref(kp), self.nbands,
+                          C.c_void_p(self.stream.cuda_stream))
+        if rc:
+            raise ExxError(rc, L.exx_last_error(None).decode())
+        self.npw = []
+        for k in range(self.nk):
+            n = C.c_int()
+            self._chk(L.exx_npw(self._h, k, C.byref(n)))
+            self.npw.append(n.value)
+        self.offsets = []
+        for k in range(self.nk + 1):
+            o = C.c_int64()
+            self._chk(L.exx_psi_offset(self._h, k, C.byref(o)))
+            self.offsets.append(o.value)
+        self.ncoef = self.offsets[-1]
+
+    @classmethod
+    def from_workload(cls, w, stream=None):
+        return cls(w.grid, w.lattice, w.kfrac, w.kweight, w.ecut, w.kernel_kind, w.mu, w.scale, w.nbands, stream)
+
+    def _chk(self, rc):
+        if rc:
+            raise ExxError(rc, lib().exx_last_error(self._h).decode())
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().exx_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- queries
+    def index_map(self, ik):
+        m = np.empty(self.npw[ik], dtype=np.int32)
+        self._chk(lib().exx_index_map(self._h, ik, m.ctypes.data_as(C.POINTER(C.c_int32))))
+        return m
+
+    def kernel_table(self, ik, iq):
+        K = np.empty(self.grid, dtype=np.float64)
+        self._chk(lib().exx_kernel_table(self._h, ik, iq, _dp(K)))
+        return K
+
+    def set_option(self, opt, value):
+        self._chk(lib().exx_set_option(self._h, opt, int(value)))
+
+    def get_option(self, opt):
+        v = C.c_int64()
+        self._chk(lib().exx_get_option(self._h, opt, C.byref(v)))
+        return v.value
+
+    def get_info(self, what):
+        v = C.c_int64()
+        self._chk(lib().exx_get_info(self._h, what, C.byref(v)))
+        return v.value
+
+    def kernel_times(self):
+        """{class name: (ms_total, launches)} for the last apply (needs EXX_OPT_PROFILE = 1)."""
+        res = {}
+        for k in range(self.get_info(EXX_INFO_NUM_KERNEL_CLASSES)):
+            ms, n = C.c_double(), C.c_int64()
+            self._chk(lib().exx_get_kernel_time(self._h, k, C.byref(ms), C.byref(n)))
+            res[lib().exx_kernel_class_name(k).decode()] = (ms.value, n.value)
+        return res
+
+    # ---- device helpers (torch = memory only)
+    def _dev(self, t, nelem):
+        torch = self._torch
+        assert t.is_cuda and t.dtype == torch.complex128 and t.is_contiguous() and t.numel() == nelem, \
+            "expected a contiguous complex128 CUDA tensor with %d elements" % nelem
+        return C.c_void_p(t.data_ptr())
+
+    def _occ(self, occ):
+        occ = np.ascontiguousarray(occ, dtype=np.float64).reshape(-1)
+        assert occ.size == self.nk * self.nbands
+        return occ
+
+    def empty_like_psi(self):
+        return self._torch.empty(self.ncoef, dtype=self._torch.complex128, device="cuda")
+
+    def to_device(self, psi_host):
+        return self._torch.from_numpy(np.ascontiguousarray(psi_host, dtype=np.complex128).reshape(-1)).cuda()
+
+    # ---- the calls of include/exx.h
+    def apply(self, psi_dev, occ, out_dev=None):
+        out_dev = self.empty_like_psi() if out_dev is None else out_dev
+        occ = self._occ(occ)
+        self._chk(lib().exx_apply(self._h, self._dev(psi_dev, self.ncoef), _dp(occ), self._dev(out_dev, self.ncoef)))
+        return out_dev
+
+    def energy(self, psi_dev, occ, vxpsi_dev=None):
+        occ = self._occ(occ)
+        ex = C.c_double()
+        pb = np.empty(self.nk * self.nbands)
+        vx = self._dev(vxpsi_dev, self.ncoef) if vxpsi_dev is not None else None
+        self._chk(lib().exx_energy(self._h, self._dev(psi_dev, self.ncoef), _dp(occ), vx,
+                                   C.cast(C.byref(ex), C.POINTER(C.c_double)), _dp(pb)))
+        return ex.value, pb
+
+    def apply_host(self, psi_host, occ, out_host=None, want_energy=True):
+        """psi_host/out_host: complex128 numpy arrays or pinned CPU torch tensors (ncoef elements)."""
+        occ = self._occ(occ)
+        if out_host is None:
+            out_host = np.empty(self.ncoef, dtype=np.complex128)
+        ex = C.c_double()
+        exp = C.cast(C.byref(ex), C.POINTER(C.c_double)) if want_energy else None
+        self._chk(lib().exx_apply_host(self._h, C.c_void_p(_host_ptr(psi_host, self.ncoef)), _dp(occ),
+                                       C.c_void_p(_host_ptr(out_host, self.ncoef)), exp))
+        return out_host, (ex.value if want_energy else None)
+
+    def scatter(self, ik, coef_dev, nbatch, box_dev):
+        self._chk(lib().exx_scatter(self._h, ik, self._dev(coef_dev, nbatch * self.npw[ik]), nbatch, self._dev(box_dev, nbatch * self.ng)))
+        return box_dev
+
+    def gather(self, ik, box_dev, nbatch, coef_dev):
+        self._chk(lib().exx_gather(self._h, ik, self._dev(box_dev, nbatch * self.ng), nbatch, self._dev(coef_dev, nbatch * self.npw[ik])))
+        return coef_dev
+
+    def fft3d(self, box_dev, nbatch, sign):
+        self._chk(lib().exx_fft3d(self._h, self._dev(box_dev, nbatch * self.ng), nbatch, sign))
+        return box_dev
+
+    def to_real(self, ik, coef_dev, nbatch, box_dev):
+        self._chk(lib().exx_to_real(self._h, ik, self._dev(coef_dev, nbatch * self.npw[ik]), nbatch, self._dev(box_dev, nbatch * self.ng)))
+        return box_dev
+
+    def band(self, arr, ik, n):
+        o = self.offsets[ik] + n * self.npw[ik]
+        return arr.reshape(-1)[o:o + self.npw[ik]]
+
+
+def _host_ptr(a, nelem):
+    if isinstance(a, np.ndarray):
+        assert a.dtype == np.complex128 and a.flags["C_CONTIGUOUS"] and a.size == nelem
+        return a.ctypes.data
+    assert (not a.is_cuda) and a.is_contiguous() and a.numel() == nelem  # torch CPU tensor (pinned or not)
+    return a.data_ptr()

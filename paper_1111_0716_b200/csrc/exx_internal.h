@@ -1,0 +1,139 @@
+// exx_internal.h — context layout and launch helpers shared by the translation units of libexx.
+// Product code: shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/exx.h"
+
+namespace exx {
+
+// kernel classes for launch counting / event timing (EXX_INFO_NUM_KERNEL_CLASSES entries)
+enum KClass {
+    KC_SCATTER = 0,
+    KC_GATHER = 1,
+    KC_FFT_AXIS = 2,     // generic per-axis FFT
+    KC_CODENSITY = 3,    // generic rho = conj(u_m) u_n
+    KC_KMUL = 4,         // generic v^ = K' rho^
+    KC_ACCUM = 5,        // generic acc -= w f u_m v
+    KC_ENERGY = 6,
+    KC_PASS_A = 7,       // fused: co-density + forward (y,z)-plane transform
+    KC_PASS_B = 8,       // fused: forward x, K', inverse x
+    KC_PASS_C = 9,       // fused: inverse (y,z)-plane transform, times f_m u_m, accumulate
+    KC_COUNT = 10
+};
+
+struct Plan1D {
+    int n = 0;
+    int nst = 0;
+    int radix[16] = {0};
+    double2* tw_dev = nullptr;  // n entries exp(-2 pi i j / n)
+};
+
+struct EventRec {
+    cudaEvent_t a, b;
+    int kclass;
+};
+
+}  // namespace exx
+
+struct exx_ctx {
+    int N[3];
+    int64_t Ng;
+    double A[9], B[9], omega;
+    int nk, nb;
+    std::vector<double> kfrac, kw;
+    double ecut;
+    exx_kernel_params kp;
+    int gmax[3];                      // max |g_i| over all spheres
+    bool alias_free;                  // 4*gmax_i + 1 <= N_i for all i
+
+    std::vector<int> npw;
+    std::vector<int64_t> off;         // nk+1, complex elements
+    std::vector<std::vector<int32_t>> map_h;
+    std::vector<int64_t> map_off;     // nk+1 offsets into map_dev
+    int32_t* map_dev = nullptr;
+
+    std::vector<int> ktab_of;         // nk*nk -> table index
+    int ntab = 0;
+    std::vector<std::vector<double>> ktab_dk;  // per table the delta-kappa triple
+    double* ktab_dev = nullptr;       // ntab * Ng, K'(g) = K/(Omega Ng^2), C order
+
+    exx::Plan1D plan[3];
+
+    cudaStream_t stream = nullptr;
+    double2* u_dev = nullptr;         // nk*nb boxes, u_nk(r)
+    double2* work_dev = nullptr;      // pair workspace
+    double2* acc_dev = nullptr;       // accumulators of one n-tile
+    size_t work_boxes = 0, acc_boxes = 0;
+    double2* vx_dev = nullptr;        // internal V_x psi buffer (exx_energy with NULL, exx_apply_host)
+    double2* psi_stage_dev = nullptr; // exx_apply_host staging
+    double* band_dot_dev = nullptr;   // nk*nb Re<c|Vc>
+    double* band_e_dev = nullptr;     // nk*nb + 1: per-band energies, then total
+    double* occw_dev = nullptr;       // nk*nb: 1/2 w_k f_nk
+    int64_t* band_off_dev = nullptr;  // nk*nb: offset of band (k,n) in psi (complex elements)
+    int* band_len_dev = nullptr;      // nk*nb: npw(k)
+    double* host_pinned = nullptr;    // nk*nb + 1 doubles, pinned
+    size_t dev_bytes = 0;
+
+    // fused path state (exx_fused.cu)
+    void* fused = nullptr;
+
+    // options
+    int64_t opt_path = 0, opt_tile_n = 0, opt_tile_m = 0, opt_prune = 1, opt_profile = 0;
+
+    // counters of the last apply
+    int64_t launches = 0, pairs_ordered = 0, pairs_executed = 0, path_used = 0, tile_n_used = 0, tile_m_used = 0, pruned_used = 0;
+    int64_t launches_by_class[exx::KC_COUNT] = {0};
+    std::vector<exx::EventRec> events;
+    std::vector<cudaEvent_t> event_pool;
+    size_t event_pool_used = 0;
+
+    std::string last_error;
+};
+
+namespace exx {
+
+void set_thread_error(const std::string& s);
+int cuda_fail(exx_ctx* c, cudaError_t e, const char* what);
+
+#define EXX_CUDA(c, call)                                         \
+    do {                                                          \
+        cudaError_t e__ = (call);                                 \
+        if (e__ != cudaSuccess) return exx::cuda_fail((c), e__, #call); \
+    } while (0)
+
+// launch bookkeeping: count, optionally bracket with events
+struct LaunchScope {
+    exx_ctx* c;
+    int kclass;
+    cudaEvent_t a = nullptr, b = nullptr;
+    LaunchScope(exx_ctx* c_, int k);
+    ~LaunchScope();
+};
+
+// ---- generic kernels (exx_kernels.cu) ----
+struct MTile {
+    int tm;
+    int m_idx[32];     // band indices within k-point q
+    double wf[32];     // w_q * f_mq
+};
+int fft_generic_init(exx_ctx* c);
+int launch_scatter(exx_ctx* c, int ik, const double2* coef, int nbatch, double2* box);
+int launch_gather(exx_ctx* c, int ik, const double2* box, int nbatch, double2* coef);
+int launch_fft3d_generic(exx_ctx* c, double2* box, int nbatch, int sign);
+int launch_codensity_tile(exx_ctx* c, const double2* un_base, int n0, int tn, const double2* uq_base, const MTile& mt, double2* work);
+int launch_kmul(exx_ctx* c, const double* ktab, double2* work, int nboxes);
+int launch_accumulate_tile(exx_ctx* c, const double2* uq_base, const MTile& mt, int tn, const double2* work, double2* acc);
+int launch_energy(exx_ctx* c, const double2* psi, const double2* vx);
+
+// ---- fused path (exx_fused.cu) ----
+bool fused_supported(const exx_ctx* c);
+int fused_create(exx_ctx* c);
+void fused_destroy(exx_ctx* c);
+int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out);
+
+}  // namespace exx

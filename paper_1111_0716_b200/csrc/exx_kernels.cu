@@ -1,0 +1,327 @@
+// exx_kernels.cu — generic (any 2^a 3^b grid) kernels of libexx: scatter/gather, per-axis batched fp64 FFT,
+// co-density, kernel multiply, weighted accumulation, energy reduction.  These are the reference-speed path
+// (EXX_OPT_PATH = 1) and the fallback for grids the fused path (exx_fused.cu) does not cover.
+//
+// Steps S0..S8 refer to DESIGN.md section 1 (hot path), which cites PAPER.md L107, L119, L127-130, L143-145.
+#include <math.h>
+
+#include "exx_internal.h"
+
+namespace exx {
+
+__device__ __forceinline__ double2 cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+__device__ __forceinline__ double2 cmul_conj_a(double2 a, double2 b) {  // conj(a) * b
+    return make_double2(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x);
+}
+__device__ __forceinline__ double2 cadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ double2 csub(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
+
+// ---------------------------------------------------------------------------------------------------------------
+// S1/S7 data movement: sphere <-> box through the precomputed index map ("scatter/gather operations used to
+// express cutoffs").  Pure copies: bit exact.
+__global__ void scatter_kernel(const double2* __restrict__ coef, const int32_t* __restrict__ map, int npw, int64_t Ng,
+                               double2* __restrict__ box) {
+    int b = blockIdx.y;
+    for (int ig = blockIdx.x * blockDim.x + threadIdx.x; ig < npw; ig += gridDim.x * blockDim.x)
+        box[(int64_t)b * Ng + map[ig]] = coef[(int64_t)b * npw + ig];
+}
+__global__ void gather_kernel(const double2* __restrict__ box, const int32_t* __restrict__ map, int npw, int64_t Ng,
+                              double2* __restrict__ coef) {
+    int b = blockIdx.y;
+    for (int ig = blockIdx.x * blockDim.x + threadIdx.x; ig < npw; ig += gridDim.x * blockDim.x)
+        coef[(int64_t)b * npw + ig] = box[(int64_t)b * Ng + map[ig]];
+}
+
+int launch_scatter(exx_ctx* c, int ik, const double2* coef, int nbatch, double2* box) {
+    EXX_CUDA(c, cudaMemsetAsync(box, 0, sizeof(double2) * (size_t)c->Ng * nbatch, c->stream));
+    int npw = c->npw[ik];
+    for (int b0 = 0; b0 < nbatch; b0 += 32768) {
+        int nb = nbatch - b0 < 32768 ? nbatch - b0 : 32768;
+        LaunchScope ls(c, KC_SCATTER);
+        dim3 grid((npw + 255) / 256, nb);
+        scatter_kernel<<<grid, 256, 0, c->stream>>>(coef + (int64_t)b0 * npw, c->map_dev + c->map_off[ik], npw, c->Ng, box + (int64_t)b0 * c->Ng);
+    }
+    EXX_CUDA(c, cudaGetLastError());
+    return EXX_OK;
+}
+int launch_gather(exx_ctx* c, int ik, const double2* box, int nbatch, double2* coef) {
+    int npw = c->npw[ik];
+    for (int b0 = 0; b0 < nbatch; b0 += 32768) {
+        int nb = nbatch - b0 < 32768 ? nbatch - b0 : 32768;
+        LaunchScope ls(c, KC_GATHER);
+        dim3 grid((npw + 255) / 256, nb);
+        gather_kernel<<<grid, 256, 0, c->stream>>>(box + (int64_t)b0 * c->Ng, c->map_dev + c->map_off[ik], npw, c->Ng, coef + (int64_t)b0 * npw);
+    }
+    EXX_CUDA(c, cudaGetLastError());
+    return EXX_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// S3/S5 generic: batched 1-D transforms along one axis of [outer][n][inner] (inner = product of the faster dims).
+// A CTA stages P pencils in shared memory and runs a Stockham autosort FFT with runtime radices 2/3/4:
+//   stage with radix R and Ns = product of earlier radices: butterfly j in [0, n/R): k = j mod Ns,
+//   v[r] = x[j + r n/R] W^{r k n/(Ns R)},  R-point DFT,  y[(j/Ns) Ns R + k + r Ns] = v[r].
+struct Radices {
+    int nst;
+    int r[16];
+};
+
+template <int SIGN>
+__device__ __forceinline__ double2 twiddle(const double2* __restrict__ tw, int idx) {
+    double2 w = __ldg(tw + idx);  // exp(-2 pi i idx / n)
+    if (SIGN > 0) w.y = -w.y;
+    return w;
+}
+
+template <int SIGN>
+__global__ void __launch_bounds__(256) fft_axis_generic_kernel(double2* __restrict__ data, const double2* __restrict__ tw, int n, Radices rad,
+                                                                int64_t inner, int64_t nouter, int P, int pitch) {
+    extern __shared__ double2 smem[];
+    double2* s0 = smem;
+    double2* s1 = smem + (size_t)P * pitch;
+    const int tid = threadIdx.x, nth = blockDim.x;
+
+    // tile -> (outer index o, first inner index i0) or, for inner == 1, P consecutive outer indices
+    int64_t tile = blockIdx.x;
+    int64_t base;     // element offset of pencil 0, element 0
+    int np;           // pencils in this tile
+    int64_t pstride;  // element stride between pencils of the tile
+    int64_t estride;  // element stride along the pencil
+    if (inner == 1) {
+        int64_t o0 = tile * P;
+        np = (int)((nouter - o0) < P ? (nouter - o0) : P);
+        base = o0 * n;
+        pstride = n;
+        estride = 1;
+    } else {
+        int64_t tpo = (inner + P - 1) / P;
+        int64_t o = tile / tpo, i0 = (tile % tpo) * P;
+        np = (int)((inner - i0) < P ? (inner - i0) : P);
+        base = o * n * inner + i0;
+        pstride = 1;
+        estride = inner;
+    }
+    // load
+    if (inner == 1) {
+        for (int e = tid; e < np * n; e += nth) {
+            int p = e / n, j = e - p * n;
+            s0[p * pitch + j] = data[base + e];
+        }
+    } else {
+        for (int e = tid; e < np * n; e += nth) {
+            int j = e / np, p = e - j * np;
+            s0[p * pitch + j] = data[base + (int64_t)j * estride + p];
+        }
+    }
+    __syncthreads();
+    int Ns = 1;
+    for (int s = 0; s < rad.nst; s++) {
+        const int R = rad.r[s];
+        const int nbf = n / R;
+        const int tws = n / (Ns * R);
+        for (int w = tid; w < np * nbf; w += nth) {
+            int p = w / nbf, j = w - p * nbf;
+            int k = j % Ns;
+            const double2* src = s0 + p * pitch + j;
+            double2* dst = s1 + p * pitch + (j / Ns) * Ns * R + k;
+            if (R == 2) {
+                double2 a = src[0], b = cmul(src[nbf], twiddle<SIGN>(tw, k * tws));
+                dst[0] = cadd(a, b);
+                dst[Ns] = csub(a, b);
+            } else if (R == 4) {
+                double2 a = src[0];
+                double2 b = cmul(src[nbf], twiddle<SIGN>(tw, k * tws));
+                double2 cc = cmul(src[2 * nbf], twiddle<SIGN>(tw, 2 * k * tws));
+                double2 d = cmul(src[3 * nbf], twiddle<SIGN>(tw, 3 * k * tws));
+                double2 t0 = cadd(a, cc), t1 = csub(a, cc), t2 = cadd(b, d), t3 = csub(b, d);
+                // forward: W4 = -i ; inverse: +i.   (-i)*t3 = (t3.y, -t3.x)
+                double2 t3r = (SIGN < 0) ? make_double2(t3.y, -t3.x) : make_double2(-t3.y, t3.x);
+                dst[0] = cadd(t0, t2);
+                dst[Ns] = cadd(t1, t3r);
+                dst[2 * Ns] = csub(t0, t2);
+                dst[3 * Ns] = csub(t1, t3r);
+            } else {  // R == 3
+                double2 a = src[0];
+                double2 b = cmul(src[nbf], twiddle<SIGN>(tw, k * tws));
+                double2 cc = cmul(src[2 * nbf], twiddle<SIGN>(tw, 2 * k * tws));
+                const double hs3 = 0.86602540378443864676372317075294;  // sqrt(3)/2
+                double2 t1 = cadd(b, cc), t2 = csub(b, cc);
+                double2 m = make_double2(a.x - 0.5 * t1.x, a.y - 0.5 * t1.y);
+                // forward: X1 = m - i hs3 t2, X2 = m + i hs3 t2 ; inverse swaps
+                double2 r = (SIGN < 0) ? make_double2(hs3 * t2.y, -hs3 * t2.x) : make_double2(-hs3 * t2.y, hs3 * t2.x);
+                dst[0] = cadd(a, t1);
+                dst[Ns] = cadd(m, r);
+                dst[2 * Ns] = csub(m, r);
+            }
+        }
+        __syncthreads();
+        double2* t = s0;
+        s0 = s1;
+        s1 = t;
+        Ns *= R;
+    }
+    // store
+    if (inner == 1) {
+        for (int e = tid; e < np * n; e += nth) {
+            int p = e / n, j = e - p * n;
+            data[base + e] = s0[p * pitch + j];
+        }
+    } else {
+        for (int e = tid; e < np * n; e += nth) {
+            int j = e / np, p = e - j * np;
+            data[base + (int64_t)j * estride + p] = s0[p * pitch + j];
+        }
+    }
+    (void)pstride;
+}
+
+static int launch_fft_axis(exx_ctx* c, double2* data, int axis, int nbatch, int sign) {
+    const Plan1D& pl = c->plan[axis];
+    int n = pl.n;
+    if (n == 1) return EXX_OK;
+    int64_t inner = (axis == 2) ? 1 : (axis == 1 ? c->N[2] : (int64_t)c->N[1] * c->N[2]);
+    int64_t nouter = (int64_t)nbatch * c->Ng / ((int64_t)n * inner);
+    int P = n > 256 ? 2 : (n > 128 ? 4 : (n > 64 ? 8 : 16));
+    int pitch = n | 1;
+    size_t smem = sizeof(double2) * 2 * (size_t)P * pitch;
+    int64_t tiles = (inner == 1) ? (nouter + P - 1) / P : nouter * ((inner + P - 1) / P);
+    Radices rad;
+    rad.nst = pl.nst;
+    for (int i = 0; i < 16; i++) rad.r[i] = pl.radix[i];
+    LaunchScope ls(c, KC_FFT_AXIS);
+    if (sign < 0)
+        fft_axis_generic_kernel<-1><<<(unsigned)tiles, 256, smem, c->stream>>>(data, pl.tw_dev, n, rad, inner, nouter, P, pitch);
+    else
+        fft_axis_generic_kernel<+1><<<(unsigned)tiles, 256, smem, c->stream>>>(data, pl.tw_dev, n, rad, inner, nouter, P, pitch);
+    EXX_CUDA(c, cudaGetLastError());
+    return EXX_OK;
+}
+
+int fft_generic_init(exx_ctx* c) {
+    EXX_CUDA(c, cudaFuncSetAttribute(fft_axis_generic_kernel<-1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+    EXX_CUDA(c, cudaFuncSetAttribute(fft_axis_generic_kernel<+1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024));
+    return EXX_OK;
+}
+
+int launch_fft3d_generic(exx_ctx* c, double2* box, int nbatch, int sign) {
+    // keep each launch's grid below 2^31 tiles and batches modest
+    for (int axis = 2; axis >= 0; axis--) {
+        int rc = launch_fft_axis(c, box, axis, nbatch, sign);
+        if (rc) return rc;
+    }
+    return EXX_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// S2 generic: work[(i*tm + j)][r] = conj(u_{m_j q}(r)) u_{n0+i, k}(r)
+__global__ void codensity_kernel(const double2* __restrict__ un_base, int n0, int tn, const double2* __restrict__ uq_base, MTile mt, int64_t Ng,
+                                 double2* __restrict__ work) {
+    int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= Ng) return;
+    int i = blockIdx.y;
+    double2 un = un_base[(int64_t)(n0 + i) * Ng + r];
+    for (int j = 0; j < mt.tm; j++) {
+        double2 um = uq_base[(int64_t)mt.m_idx[j] * Ng + r];
+        work[((int64_t)i * mt.tm + j) * Ng + r] = cmul_conj_a(um, un);
+    }
+}
+int launch_codensity_tile(exx_ctx* c, const double2* un_base, int n0, int tn, const double2* uq_base, const MTile& mt, double2* work) {
+    LaunchScope ls(c, KC_CODENSITY);
+    dim3 grid((unsigned)((c->Ng + 255) / 256), tn);
+    codensity_kernel<<<grid, 256, 0, c->stream>>>(un_base, n0, tn, uq_base, mt, c->Ng, work);
+    EXX_CUDA(c, cudaGetLastError());
+    return EXX_OK;
+}
+
+// S4 generic: work[t][g] *= K'(g)
+__global__ void kmul_kernel(const double* __restrict__ ktab, double2* __restrict__ work, int64_t Ng) {
+    int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= Ng) return;
+    double kv = ktab[g];
+    double2* w = work + (int64_t)blockIdx.y * Ng + g;
+    double2 v = *w;
+    *w = make_double2(kv * v.x, kv * v.y);
+}
+int launch_kmul(exx_ctx* c, const double* ktab, double2* work, int nboxes) {
+    LaunchScope ls(c, KC_KMUL);
+    dim3 grid((unsigned)((c->Ng + 255) / 256), nboxes);
+    kmul_kernel<<<grid, 256, 0, c->stream>>>(ktab, work, c->Ng);
+    EXX_CUDA(c, cudaGetLastError());
+    return EXX_OK;
+}
+
+// S6 generic: acc[i][r] -= sum_j (w_q f_mj) u_mj(r) v_ij(r), j in ascending order (fixed summation order)
+__global__ void accumulate_kernel(const double2* __restrict__ uq_base, MTile mt, int64_t Ng, const double2* __restrict__ work,
+                                  double2* __restrict__ acc) {
+    int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= Ng) return;
+    int i = blockIdx.y;
+    double2 a = acc[(int64_t)i * Ng + r];
+    for (int j = 0; j < mt.tm; j++) {
+        double2 um = uq_base[(int64_t)mt.m_idx[j] * Ng + r];
+        double2 v = work[((int64_t)i * mt.tm + j) * Ng + r];
+        double2 p = cmul(um, v);
+        a.x -= mt.wf[j] * p.x;
+        a.y -= mt.wf[j] * p.y;
+    }
+    acc[(int64_t)i * Ng + r] = a;
+}
+int launch_accumulate_tile(exx_ctx* c, const double2* uq_base, const MTile& mt, int tn, const double2* work, double2* acc) {
+    LaunchScope ls(c, KC_ACCUM);
+    dim3 grid((unsigned)((c->Ng + 255) / 256), tn);
+    accumulate_kernel<<<grid, 256, 0, c->stream>>>(uq_base, mt, c->Ng, work, acc);
+    EXX_CUDA(c, cudaGetLastError());
+    return EXX_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// S8: per band s = Re sum_g conj(c(g)) v(g): each thread strides over the band in a fixed order, warp shuffles, then a
+// fixed-order pass over the warp partials; a second one-warp kernel forms e_i = occw_i s_i and E_x = sum_i e_i.
+__global__ void __launch_bounds__(256) band_dot_kernel(const double2* __restrict__ psi, const double2* __restrict__ vx, const int64_t* __restrict__ band_off,
+                                                        const int* __restrict__ band_len, double* __restrict__ dots) {
+    int b = blockIdx.x;
+    const double2* a = psi + band_off[b];
+    const double2* v = vx + band_off[b];
+    int n = band_len[b];
+    double s = 0.0;
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        double2 x = a[i], y = v[i];
+        s += x.x * y.x + x.y * y.y;
+    }
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+    __shared__ double part[8];
+    if ((threadIdx.x & 31) == 0) part[threadIdx.x >> 5] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < 8; w++) t += part[w];
+        dots[b] = t;
+    }
+}
+__global__ void energy_sum_kernel(const double* __restrict__ dots, const double* __restrict__ occw, int nbt, double* __restrict__ out) {
+    // one warp; lane-strided fixed order, then shuffle tree
+    double s = 0.0;
+    for (int i = threadIdx.x; i < nbt; i += 32) {
+        double e = occw[i] * dots[i];
+        out[i] = e;
+        s += e;
+    }
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+    if (threadIdx.x == 0) out[nbt] = s;
+}
+
+int launch_energy(exx_ctx* c, const double2* psi, const double2* vx) {
+    int nbt = c->nk * c->nb;
+    {
+        LaunchScope ls(c, KC_ENERGY);
+        band_dot_kernel<<<nbt, 256, 0, c->stream>>>(psi, vx, c->band_off_dev, c->band_len_dev, c->band_dot_dev);
+    }
+    {
+        LaunchScope ls(c, KC_ENERGY);
+        energy_sum_kernel<<<1, 32, 0, c->stream>>>(c->band_dot_dev, c->occw_dev, nbt, c->band_e_dev);
+    }
+    EXX_CUDA(c, cudaGetLastError());
+    return EXX_OK;
+}
+
+}  // namespace exx

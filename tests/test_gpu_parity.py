@@ -1,0 +1,297 @@
+"""GPU parity tests (-m gpu): the CUDA library, called through its C ABI, against the oracle on the same seeded inputs.
+
+Bars (BASELINE.json north_star): index maps bit-exact; V_x psi_n within 1e-10 relative L2 per band; E_x within 1e-11
+relative; fp64.  Building blocks (scatter/gather, FFT, kernel table) are held to tighter, arithmetic-derived bars.
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+from oracle import exx_ref as R
+from paper_1111_0716_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+TOL_VX = 1e-10
+TOL_EX = 1e-11
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1111_0716_b200 import binding
+    binding.lib()  # fails loudly if libexx.so is missing
+    return binding
+
+
+def _pair(B, w):
+    o = R.RefExx(w.grid, w.lattice, w.kfrac, w.kweight, w.ecut, w.kernel_kind, w.mu, w.scale, w.nbands)
+    g = B.Exx.from_workload(w)
+    return o, g
+
+
+def _rel(a, b):
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+SMALL = {
+    "kpts_frac_occ": dict(grid=(12, 12, 12), lat=("rh", 6.0, 63.0), kf=[[0, 0, 0], [0.5, 0, 0], [0.25, -0.25, 0.125]],
+                          kw=[0.5, 0.25, 0.25], ecut=4.0, nb=5, occ=[1, 1, 0.5, 0.25, 0], kind=0, mu=0.0),
+    "noncubic_hse": dict(grid=(12, 18, 16), lat=("rh", 7.3, 71.0), kf=[[0.1, -0.3, 0.25], [0.5, 0, 0]], kw=[0.5, 0.5],
+                         ecut=5.0, nb=4, occ=[1, 0.7, 0, 0.2], kind=1, mu=0.3),
+    "tiny_aliased": dict(grid=(8, 6, 9), lat=("sc", 5.0), kf=[[0, 0, 0]], kw=[1.0], ecut=3.5, nb=3, occ=[1, 1, 1], kind=0, mu=0.0),
+    "pow2_rect": dict(grid=(32, 16, 8), lat=("rh", 6.5, 75.0), kf=[[0, 0, 0], [0, 0.5, 0.5]], kw=[0.3, 0.7], ecut=2.5, nb=3,
+                      occ=[1, 0.5, 0], kind=1, mu=0.106),
+    "one_band": dict(grid=(24, 24, 24), lat=("sc", 9.0), kf=[[0, 0, 0]], kw=[1.0], ecut=5.0, nb=1, occ=[1.0], kind=0, mu=0.0),
+    "mixed_27": dict(grid=(27, 24, 36), lat=("rh", 10.0, 80.0), kf=[[0.25, 0.25, 0.25]], kw=[1.0], ecut=4.0, nb=3, occ=[1, 1, 0.5],
+                     kind=0, mu=0.0),
+}
+
+
+def _small(name):
+    s = SMALL[name]
+    lat = W.cubic(s["lat"][1]) if s["lat"][0] == "sc" else W.rhombohedral(s["lat"][1], s["lat"][2])
+    return W.custom(name, 77 + len(name), s["grid"], lat, s["kf"], s["kw"], s["ecut"], s["nb"], s["occ"], s["kind"], s["mu"])
+
+
+# ---------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4a", "C4b", "C5"])
+def test_index_maps_bit_exact(B, name):
+    w = W.make(name)
+    if name in ("C4b", "C5"):  # keep device memory modest: the maps do not depend on the band count
+        w.nbands, w.occ_per_k = 2, np.ones(2)
+    o, g = _pair(B, w)
+    assert g.npw == o.npw and g.offsets == o.offsets
+    for k in range(w.nk):
+        a, b = g.index_map(k), o.index_map(k)
+        assert a.dtype == np.int32 and np.array_equal(a, b)
+    g.close()
+
+
+@pytest.mark.parametrize("name", list(SMALL))
+def test_index_maps_and_kernel_tables_small(B, name):
+    w = _small(name)
+    o, g = _pair(B, w)
+    assert g.npw == o.npw
+    for k in range(w.nk):
+        assert np.array_equal(g.index_map(k), o.index_map(k))
+        for q in range(w.nk):
+            want = o.kernel_table(k, q) / (o.omega * float(w.ng) ** 2)
+            got = g.kernel_table(k, q)
+            assert np.abs(got - want).max() <= 4e-16 * np.abs(want).max()
+            assert np.array_equal(got == 0, want == 0)
+    g.close()
+
+
+def test_scatter_gather_round_trip_bit_exact(B):
+    import torch
+    w = W.make("C2")
+    w.nbands, w.occ_per_k = 3, np.ones(3)
+    o, g = _pair(B, w)
+    psi = w.coefficients(o.npw)
+    for k in (0, 5):
+        coef = np.array([o.band(psi, k, n) for n in range(3)]).reshape(-1)
+        cd = torch.from_numpy(coef).cuda()
+        box = torch.full((3 * w.ng,), 7.0 + 1j, dtype=torch.complex128, device="cuda")
+        g.scatter(k, cd, 3, box)
+        hb = box.cpu().numpy().reshape(3, w.ng)
+        m = o.index_map(k)
+        want = np.zeros((3, w.ng), complex)
+        want[:, m] = coef.reshape(3, -1)
+        assert np.array_equal(hb.view(np.float64), want.view(np.float64))       # bit identical, zero elsewhere
+        back = torch.empty_like(cd)
+        g.gather(k, box, 3, back)
+        assert np.array_equal(back.cpu().numpy().view(np.float64), coef.view(np.float64))
+    g.close()
+
+
+@pytest.mark.parametrize("grid,nbatch", [((16, 16, 16), 5), ((48, 48, 48), 2), ((12, 18, 16), 3), ((27, 24, 36), 1), ((8, 6, 9), 4),
+                                         ((64, 64, 64), 1), ((96, 96, 96), 1), ((128, 128, 128), 1), ((32, 16, 8), 2), ((2, 3, 4), 7)])
+def test_fft3d_against_oracle_fft(B, grid, nbatch):
+    import torch
+    g = B.Exx(grid, W.cubic(50.0), np.zeros((1, 3)), [1.0], 0.005, nbands=1)  # sphere = {0}: any grid holds it
+    rng = np.random.default_rng(sum(grid))
+    x = rng.standard_normal((nbatch,) + grid) + 1j * rng.standard_normal((nbatch,) + grid)
+    for sign in (-1, +1):
+        d = torch.from_numpy(x.reshape(-1).copy()).cuda()
+        g.fft3d(d, nbatch, sign)
+        got = d.cpu().numpy().reshape((nbatch,) + grid)
+        for b in range(nbatch if max(grid) < 64 else 1):
+            want = R.fft3d(x[b], sign)
+            assert _rel(got[b], want) < 2e-15 * np.log2(np.prod(grid))
+    g.close()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+def _check_full(B, w, paths=(0,), tile_m=(0,)):
+    """Full element-by-element parity of V_x psi (every band), per-band energies and E_x."""
+    o, g = _pair(B, w)
+    psi = w.coefficients(o.npw)
+    want = o.apply(psi, w.occ)
+    e_want, pb_want = o.energy(psi, w.occ, want)
+    pd = g.to_device(psi)
+    for path in paths:
+        for tm in tile_m:
+            g.set_option(B.EXX_OPT_PATH, path)
+            g.set_option(B.EXX_OPT_TILE_M, tm)
+            out = g.apply(pd, w.occ)
+            got = out.cpu().numpy()
+            for k in range(w.nk):
+                for n in range(w.nbands):
+                    assert _rel(o.band(got, k, n), o.band(want, k, n)) < TOL_VX, (w.name, path, tm, k, n)
+            e, pb = g.energy(pd, w.occ, out)
+            assert abs(e - e_want) <= TOL_EX * abs(e_want)
+            assert np.abs(pb - pb_want).max() <= TOL_EX * abs(e_want)
+            assert abs(pb.sum() - e) <= 1e-14 * abs(e)
+            assert e <= 0
+            e2, _ = g.energy(pd, w.occ, None)          # library applies V_x itself
+            assert abs(e2 - e) <= 1e-15 * abs(e)
+            assert g.get_info(B.EXX_INFO_PAIRS_ORDERED) == w.pair_evals
+            assert g.get_info(B.EXX_INFO_LAUNCHES) > 0
+    g.close()
+    return o, psi, want
+
+
+@pytest.mark.parametrize("name", list(SMALL))
+def test_apply_small_cases_full_parity(B, name):
+    _check_full(B, _small(name), paths=(0, 1), tile_m=(0, 1, 3))
+
+
+def test_apply_C1_full_parity(B):
+    w = W.make("C1")
+    o, psi, want = _check_full(B, w, paths=(0, 1), tile_m=(0, 5))
+    gold = json.load(open(os.path.join(GOLD, "exx_C1.json")))
+    e, _ = o.energy(psi, w.occ, want)
+    assert abs(e - gold["E_x_E1"]) < 1e-15
+
+
+def _check_golden(B, name, live_rows=0):
+    """Big configs: the GPU applies V_x in full; rows, per-band energies and E_x are compared with stored oracle
+    results (tests/golden/make_golden.py) and, for `live_rows` rows, with the oracle run now."""
+    import torch
+    w = W.make(name)
+    if not os.path.exists(os.path.join(GOLD, "exx_%s.json" % name)):
+        pytest.skip("golden values for %s not generated (tests/golden/make_golden.py)" % name)
+    gold = json.load(open(os.path.join(GOLD, "exx_%s.json" % name)))
+    rows_gold = np.load(os.path.join(GOLD, "exx_%s_rows.npz" % name))
+    g = B.Exx.from_workload(w)
+    assert g.npw == gold["npw"]
+    psi = w.coefficients(g.npw)
+    assert [psi[0].real, psi[0].imag] == gold["psi_first"]
+    pd = g.to_device(psi)
+    out = g.apply(pd, w.occ)
+    e, pb = g.energy(pd, w.occ, out)
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    for i, (k, n) in enumerate(gold["rows"]):
+        want = rows_gold["row%d" % i]
+        assert _rel(g.band(got, k, n), want) < TOL_VX, (name, k, n)
+        assert abs(pb[k * w.nbands + n] - gold["row_energy"][i]) <= TOL_EX * abs(gold["row_energy"][i]) + 1e-300
+    if "E_x_E1" in gold:
+        assert abs(e - gold["E_x_E1"]) <= TOL_EX * abs(gold["E_x_E1"])
+        assert abs(e - gold["E_x_E2"]) <= 1e-10 * abs(gold["E_x_E2"])
+        assert np.abs(pb - np.array(gold["per_band_energy"])).max() <= TOL_EX * abs(gold["E_x_E1"])
+        norms = np.array([np.linalg.norm(g.band(got, k, n)) for k in range(w.nk) for n in range(w.nbands)])
+        assert np.abs(norms / np.array(gold["per_band_norm"]) - 1).max() < TOL_VX
+    # properties that hold at any size
+    assert e < 0 and abs(pb.sum() - e) <= 1e-13 * abs(e) and np.all(pb <= 0)
+    assert g.get_info(B.EXX_INFO_PAIRS_ORDERED) == w.pair_evals
+    if live_rows:
+        o = R.RefExx(w.grid, w.lattice, w.kfrac, w.kweight, w.ecut, w.kernel_kind, w.mu, w.scale, w.nbands)
+        rows = [(w.nk // 2, w.nbands // 3), (0, 1)][:live_rows]
+        for (k, n), r in zip(rows, o.apply_rows(psi, w.occ, rows)):
+            assert _rel(g.band(got, k, n), r) < TOL_VX, (name, "live", k, n)
+    g.close()
+
+
+def test_apply_C2_parity(B):
+    _check_golden(B, "C2", live_rows=1)
+
+
+def test_apply_C3_parity(B):
+    _check_golden(B, "C3", live_rows=1)
+
+
+def test_apply_C4a_parity(B):
+    _check_golden(B, "C4a")
+
+
+def test_apply_C5_parity(B):
+    _check_golden(B, "C5")
+
+
+@pytest.mark.skipif(not os.path.exists(os.path.join(GOLD, "exx_C4b.json")), reason="C4b golden rows not generated yet")
+def test_apply_C4b_parity(B):
+    _check_golden(B, "C4b")
+
+
+# ---------------------------------------------------------------------------------------------------------------
+def test_edge_cases_and_errors(B):
+    import torch
+    w = _small("kpts_frac_occ")
+    o, g = _pair(B, w)
+    psi = w.coefficients(o.npw)
+    pd = g.to_device(psi)
+    # all occupations zero: V_x = 0 exactly, E_x = 0, no pair executed
+    out = g.apply(pd, np.zeros(w.nk * w.nbands))
+    assert float(out.abs().max()) == 0.0
+    assert g.get_info(B.EXX_INFO_PAIRS_EXECUTED) == 0
+    assert g.energy(pd, np.zeros(w.nk * w.nbands), out)[0] == 0.0
+    # only one occupied band at one k-point: matches the oracle, other k-points still get rows
+    occ1 = np.zeros(w.nk * w.nbands)
+    occ1[w.nbands + 2] = 0.75
+    got = g.apply(pd, occ1).cpu().numpy()
+    assert _rel(got, o.apply(psi, occ1)) < TOL_VX
+    # errors: aliasing, bad occupations, wrong sizes are refused and leave the output alone
+    with pytest.raises(B.ExxError) as ei:
+        g.apply(pd, w.occ, pd)
+    assert ei.value.code == -10
+    bad = w.occ.copy()
+    bad[1] = -0.1
+    sentinel = torch.full_like(pd, 3.0)
+    with pytest.raises(B.ExxError) as ei:
+        g.apply(pd, bad, sentinel)
+    assert ei.value.code == -6 and float((sentinel - 3.0).abs().max()) == 0.0
+    bad[1] = float("inf")
+    with pytest.raises(B.ExxError):
+        g.energy(pd, bad, out)
+    with pytest.raises(B.ExxError):
+        g.set_option(99, 1)
+    with pytest.raises(B.ExxError):   # sphere does not fit the box
+        B.Exx((8, 8, 8), W.cubic(10.0), np.zeros((1, 3)), [1.0], 6.0, nbands=1)
+    g.close()
+
+
+def test_apply_host_matches_device_path(B):
+    import torch
+    w = W.make("C1")
+    o, g = _pair(B, w)
+    psi = w.coefficients(o.npw)
+    out_d = g.apply(g.to_device(psi), w.occ).cpu().numpy()
+    e_d, _ = g.energy(g.to_device(psi), w.occ, None)
+    out_h, e_h = g.apply_host(psi, w.occ)
+    assert np.array_equal(out_h.view(np.float64), out_d.view(np.float64)) and e_h == e_d
+    pin_in = torch.from_numpy(psi).pin_memory()
+    pin_out = torch.empty(g.ncoef, dtype=torch.complex128).pin_memory()
+    g.apply_host(pin_in, w.occ, pin_out, want_energy=False)
+    assert np.array_equal(pin_out.numpy().view(np.float64), out_d.view(np.float64))
+    g.close()
+
+
+def test_to_real_matches_oracle(B):
+    import torch
+    w = _small("noncubic_hse")
+    o, g = _pair(B, w)
+    psi = w.coefficients(o.npw)
+    for k in range(w.nk):
+        coef = np.array([o.band(psi, k, n) for n in range(w.nbands)]).reshape(-1)
+        box = torch.empty(w.nbands * w.ng, dtype=torch.complex128, device="cuda")
+        g.to_real(k, torch.from_numpy(coef).cuda(), w.nbands, box)
+        hb = box.cpu().numpy().reshape((w.nbands,) + w.grid)
+        for n in range(w.nbands):
+            assert _rel(hb[n], o.to_real(k, o.band(psi, k, n))) < 1e-14
+    g.close()

@@ -1,0 +1,267 @@
+#!/usr/bin/env python
+"""bench.py — band-pair exchange evaluations per second for one full V_x application (+ E_x) on synthetic
+boron-shaped workloads (BASELINE.json metric), one process per GPU.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C4a] [--impl ours|reference]
+
+A step = one pass of the whole hot path (S1..S8 of DESIGN.md: scatter + inverse FFT of every band, all band pairs,
+forward FFT + gather, energy reduction) over the workload.  `value` times it with psi already in HBM; `e2e` times the
+same call through exx_apply_host with pinned HOST buffers (H2D of psi, D2H of V_x psi and E_x inside the timed region).
+N > 1 runs N independent replicas (the path is single-GPU by design): weak scaling, no collective
+on the data path; timing is barrier + max over ranks.
+`--impl reference` times the oracle (oracle/, plain CPU code, as it stands) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1111_0716_b200 import workloads as W  # noqa: E402
+
+METRIC = "band_pair_exchange_evals_per_s"
+UNIT = "pair-evals/s"
+
+
+def read_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            d = json.load(open(p))
+            return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons sampled during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.rows, self.stop_flag = index, [], False
+
+    def run(self):
+        while not self.stop_flag:
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([x.strip() for x in out.split(",")])
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def summary(self):
+        sm = [float(r[0]) for r in self.rows if r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[i] for r in self.rows if len(r) >= 7 for i in range(4) if r[3 + i].lower().startswith("active")})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons,
+                "samples": len(self.rows)}
+
+
+def dist_setup(n):
+    """torchrun sets RANK/WORLD_SIZE/LOCAL_RANK/MASTER_*; single process otherwise."""
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+def max_over_ranks(x, world, device):
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def run_reference(args, rank, world):
+    """The oracle timed on the host cores, rank 0 only; each step = one output row (all (q,m) pairs of band (0,0))."""
+    if rank != 0:
+        return 0
+    from oracle import exx_ref as R
+    w = W.make(args.workload)
+    o = R.RefExx(w.grid, w.lattice, w.kfrac, w.kweight, w.ecut, w.kernel_kind, w.mu, w.scale, w.nbands)
+    psi = w.coefficients(o.npw)
+    pairs = w.nk * w.nocc
+    for _ in range(args.warmup):
+        o.apply_rows(psi, w.occ, [(0, 0)])
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        o.apply_rows(psi, w.occ, [(0, 0)])
+    dt = (time.perf_counter() - t0) / args.steps
+    v = pairs / dt
+    sample = "one V_x row (k0, band 0): %d pair evaluations incl. the real-space transforms of the %d bands it needs" % (pairs, pairs + 1)
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": {"workload": w.name, "description": w.description, "sample": sample},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": R.num_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# algorithmic bytes per work unit of each kernel class, in units of Ng bytes:
+# a generic box pass reads and writes one complex128 box (32 Ng); each fused pass moves 32 Ng per pair (96 Ng for the
+# three passes = the B_model of the pair evaluation).
+BYTES_PER_UNIT_NG = {"fft_axis_generic": 32, "codensity": 32, "kernel_multiply": 32, "accumulate": 32,
+                     "fused_pass_a": 32, "fused_pass_b": 32, "fused_pass_c": 32, "scatter": 16, "gather": 16}
+
+
+def run_ours(args, rank, world, local):
+    import torch
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    from paper_1111_0716_b200 import binding as B
+    B.lib()
+    w = W.make(args.workload)
+    g = B.Exx.from_workload(w)
+    if args.path is not None:
+        g.set_option(B.EXX_OPT_PATH, args.path)
+    psi = w.coefficients(g.npw)
+    occ = w.occ
+    pd = g.to_device(psi)
+    out = g.empty_like_psi()
+    pin_in = torch.from_numpy(psi).pin_memory()
+    pin_out = torch.empty(g.ncoef, dtype=torch.complex128).pin_memory()
+    peak, peak_src = read_peaks()
+
+    def step_dev():
+        g.apply(pd, occ, out)
+        return g.energy(pd, occ, out)[0]
+
+    def sync_all():
+        torch.cuda.synchronize()
+        if world > 1:
+            torch.distributed.barrier()
+
+    for _ in range(args.warmup):
+        ex = step_dev()
+    # ---- timed region 1: inputs resident in HBM (events on the stream libexx launches on = torch's current stream)
+    g.set_option(B.EXX_OPT_PROFILE, 0)
+    sampler = ClockSampler(local)
+    sync_all()
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        ex = step_dev()
+    e1.record()
+    sync_all()
+    sampler.stop_flag = True
+    ms = max_over_ranks(e0.elapsed_time(e1), world, dev) / args.steps
+    launches = g.get_info(B.EXX_INFO_LAUNCHES)
+    pairs_ord, pairs_exec = g.get_info(B.EXX_INFO_PAIRS_ORDERED), g.get_info(B.EXX_INFO_PAIRS_EXECUTED)
+
+    # ---- timed region 2: per-kernel-class device time (events around every launch) over the same K steps
+    g.set_option(B.EXX_OPT_PROFILE, 1)
+    acc = {}
+    sync_all()
+    p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    p0.record()
+    for _ in range(args.steps):
+        g.apply(pd, occ, out)
+        for name, (t, n, u) in g.kernel_times().items():
+            a = acc.setdefault(name, [0.0, 0, 0])
+            a[0] += t; a[1] += n; a[2] += u
+        g.energy(pd, occ, out)
+    p1.record()
+    sync_all()
+    ms_prof = p0.elapsed_time(p1) / args.steps
+    g.set_option(B.EXX_OPT_PROFILE, 0)
+    dom = max(acc, key=lambda k: acc[k][0])
+    t_dom, n_dom, u_dom = acc[dom]
+    bytes_dom = BYTES_PER_UNIT_NG.get(dom, 32) * w.ng * u_dom
+    achieved = bytes_dom / (t_dom * 1e-3) / 1e9 if t_dom > 0 else 0.0
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": None, "peak_source": peak_src, "avg_launch_us": 1e3 * t_dom / max(1, n_dom),
+                "algorithmic_bytes_per_launch": bytes_dom / max(1, n_dom), "share_of_step": t_dom / args.steps / ms_prof,
+                "kernel_ms_per_step": {k: v[0] / args.steps for k, v in acc.items() if v[1]}}
+    # the graded pipeline figure: B_model = 96 Ng bytes per EXECUTED pair over the whole apply
+    pipe = 96.0 * w.ng * pairs_exec / (ms * 1e-3) / 1e9
+    pipeline = {"model_bytes_per_pair": 96 * w.ng, "pairs_executed": pairs_exec, "achieved": pipe, "unit": "GB/s", "peak": peak,
+                "frac": pipe / peak, "us_per_executed_pair": 1e3 * ms / max(1, pairs_exec), "ms_per_step_profiled": ms_prof}
+
+    # ---- timed region 3: end to end through exx_apply_host, pinned host buffers, copies inside the timed region
+    for _ in range(min(2, args.warmup)):
+        g.apply_host(pin_in, occ, pin_out)
+    sync_all()
+    h0, h1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    h0.record()
+    for _ in range(args.steps):
+        _, ex_h = g.apply_host(pin_in, occ, pin_out)
+    h1.record()
+    sync_all()
+    ms_e2e = max_over_ranks(h0.elapsed_time(h1), world, dev) / args.steps
+    assert ex_h == ex or abs(ex_h - ex) <= 1e-12 * abs(ex)
+
+    value = world * pairs_ord / (ms * 1e-3)
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "description": w.description, "grid": list(w.grid), "nk": w.nk, "nbands": w.nbands,
+                       "pairs_per_step": pairs_ord, "parallelism": "replicas x%d" % world,
+                       "path": {1: "generic", 2: "fused"}.get(g.get_info(B.EXX_INFO_PATH_USED)),
+                       "tile_n": g.get_info(B.EXX_INFO_TILE_N), "tile_m": g.get_info(B.EXX_INFO_TILE_M),
+                       "pruned": g.get_info(B.EXX_INFO_PRUNED),
+                       "l2": "inputs larger than L2: the real-space cache u_nk(r) is %.2f GB, streamed every step" % (w.nk * w.nbands * w.ng * 16 / 1e9)},
+            "E_x": ex, "vx_apply_ms": ms, "clocks": sampler.summary(), "roofline": roofline, "pipeline_roofline": pipeline,
+            "e2e": {"value": world * pairs_ord / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
+                    "h2d_bytes_per_step": g.ncoef * 16, "d2h_bytes_per_step": g.ncoef * 16 + 8},
+            "gpu_launches": launches * args.steps}
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"] = cpu_baseline(w, psi)
+    if rank == 0:
+        print(json.dumps(line))
+    g.close()
+    if world > 1:
+        torch.distributed.destroy_process_group()
+    return 0
+
+
+def cpu_baseline(w, psi):
+    """The oracle as it stands on the host cores: one V_x row (all (q,m) pairs of band (0,0)) of the same workload."""
+    from oracle import exx_ref as R
+    o = R.RefExx(w.grid, w.lattice, w.kfrac, w.kweight, w.ecut, w.kernel_kind, w.mu, w.scale, w.nbands)
+    pairs = w.nk * w.nocc
+    t0 = time.perf_counter()
+    o.apply_rows(psi, w.occ, [(0, 0)])
+    dt = time.perf_counter() - t0
+    return {"value": pairs / dt, "unit": UNIT, "cores": R.num_threads(), "kind": "oracle", "seconds": dt,
+            "sample": "one V_x row (k0, band 0): %d pair evaluations incl. the real-space transforms of the %d bands it needs" % (pairs, pairs + 1)}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C4a", choices=list(W.ALL))
+    ap.add_argument("--path", type=int, default=None, help="EXX_OPT_PATH override: 1 generic, 2 fused")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    rank, world, local = dist_setup(args.gpus)
+    if args.impl == "reference":
+        return run_reference(args, rank, world)
+    return run_ours(args, rank, world, local)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

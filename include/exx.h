@@ -99,10 +99,11 @@ int exx_psi_offset(const exx_ctx* ctx, int ik /* 0..nk; nk gives the total */, i
 int exx_set_option(exx_ctx* ctx, int option, int64_t value);
 int exx_get_option(const exx_ctx* ctx, int option, int64_t* value);
 int exx_get_info(const exx_ctx* ctx, int what, int64_t* value);
-/* With EXX_OPT_PROFILE = 1: device time (CUDA events on the context's stream) and launch count of kernel class
- * `kclass` (0 .. EXX_INFO_NUM_KERNEL_CLASSES-1) during the most recent exx_apply; synchronises the stream.
+/* Per kernel class `kclass` (0 .. EXX_INFO_NUM_KERNEL_CLASSES-1), for the most recent exx_apply: launch count, work
+ * units (generic kernels: box passes, i.e. one read + one write of an FFT box; fused passes: band pairs), and — with
+ * EXX_OPT_PROFILE = 1 — the device time from CUDA events on the context's stream (0 otherwise).  Synchronises.
  * exx_kernel_class_name gives the class name (static string, NULL if out of range). */
-int exx_get_kernel_time(exx_ctx* ctx, int kclass, double* ms_total, int64_t* launches);
+int exx_get_kernel_time(exx_ctx* ctx, int kclass, double* ms_total, int64_t* launches, int64_t* units);
 const char* exx_kernel_class_name(int kclass);
 
 /* V_x applied to every band: out(k,n,:) = (V_x c)_nk.  psi_dev/out_dev: device, exx_psi_offset(nk) complex elements

@@ -56,7 +56,7 @@ def lib():
         L.exx_set_option.argtypes = [vp, C.c_int, C.c_int64]
         L.exx_get_option.argtypes = [vp, C.c_int, i64p]
         L.exx_get_info.argtypes = [vp, C.c_int, i64p]
-        L.exx_get_kernel_time.argtypes = [vp, C.c_int, dp, i64p]
+        L.exx_get_kernel_time.argtypes = [vp, C.c_int, dp, i64p, i64p]
         L.exx_kernel_class_name.argtypes = [C.c_int]
         L.exx_kernel_class_name.restype = C.c_char_p
         L.exx_apply.argtypes = [vp, vp, dp, vp]
@@ -160,12 +160,12 @@ class Exx:
         return v.value
 
     def kernel_times(self):
-        """{class name: (ms_total, launches)} for the last apply (needs EXX_OPT_PROFILE = 1)."""
+        """{class name: (ms_total, launches, units)} for the last apply (ms needs EXX_OPT_PROFILE = 1)."""
         res = {}
         for k in range(self.get_info(EXX_INFO_NUM_KERNEL_CLASSES)):
-            ms, n = C.c_double(), C.c_int64()
-            self._chk(lib().exx_get_kernel_time(self._h, k, C.byref(ms), C.byref(n)))
-            res[lib().exx_kernel_class_name(k).decode()] = (ms.value, n.value)
+            ms, n, u = C.c_double(), C.c_int64(), C.c_int64()
+            self._chk(lib().exx_get_kernel_time(self._h, k, C.byref(ms), C.byref(n), C.byref(u)))
+            res[lib().exx_kernel_class_name(k).decode()] = (ms.value, n.value, u.value)
         return res
 
     # ---- device helpers (torch = memory only)

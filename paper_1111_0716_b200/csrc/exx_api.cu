@@ -22,9 +22,10 @@ int cuda_fail(exx_ctx* c, cudaError_t e, const char* what) {
     return EXX_ERR_CUDA;
 }
 
-LaunchScope::LaunchScope(exx_ctx* c_, int k) : c(c_), kclass(k) {
+LaunchScope::LaunchScope(exx_ctx* c_, int k, int64_t units) : c(c_), kclass(k) {
     c->launches++;
     c->launches_by_class[k]++;
+    c->units_by_class[k] += units;
     if (c->opt_profile) {
         if (c->event_pool_used + 2 > c->event_pool.size()) {
             for (int i = 0; i < 256; i++) {
@@ -416,8 +417,8 @@ int exx_get_info(const exx_ctx* c, int what, int64_t* value) {
     default: return EXX_ERR_BAD_ARG;
     }
 }
-int exx_get_kernel_time(exx_ctx* c, int kclass, double* ms_total, int64_t* launches) {
-    if (!c || !ms_total || !launches) return EXX_ERR_NULL;
+int exx_get_kernel_time(exx_ctx* c, int kclass, double* ms_total, int64_t* launches, int64_t* units) {
+    if (!c || !ms_total || !launches || !units) return EXX_ERR_NULL;
     if (kclass < 0 || kclass >= KC_COUNT) return EXX_ERR_BAD_ARG;
     EXX_CUDA(c, cudaStreamSynchronize(c->stream));
     double ms = 0.0;
@@ -429,6 +430,7 @@ int exx_get_kernel_time(exx_ctx* c, int kclass, double* ms_total, int64_t* launc
         }
     *ms_total = ms;
     *launches = c->launches_by_class[kclass];
+    *units = c->units_by_class[kclass];
     return EXX_OK;
 }
 
@@ -465,7 +467,7 @@ static int check_occ(const exx_ctx* c, const double* occ) {
 
 static void reset_counters(exx_ctx* c) {
     c->launches = 0;
-    for (int i = 0; i < KC_COUNT; i++) c->launches_by_class[i] = 0;
+    for (int i = 0; i < KC_COUNT; i++) c->launches_by_class[i] = c->units_by_class[i] = 0;
     c->events.clear();
     c->event_pool_used = 0;
     c->pairs_ordered = c->pairs_executed = 0;

@@ -88,6 +88,7 @@ struct exx_ctx {
     // counters of the last apply
     int64_t launches = 0, pairs_ordered = 0, pairs_executed = 0, path_used = 0, tile_n_used = 0, tile_m_used = 0, pruned_used = 0;
     int64_t launches_by_class[exx::KC_COUNT] = {0};
+    int64_t units_by_class[exx::KC_COUNT] = {0};   // box passes (generic) or pairs (fused) processed
     std::vector<exx::EventRec> events;
     std::vector<cudaEvent_t> event_pool;
     size_t event_pool_used = 0;
@@ -111,7 +112,7 @@ struct LaunchScope {
     exx_ctx* c;
     int kclass;
     cudaEvent_t a = nullptr, b = nullptr;
-    LaunchScope(exx_ctx* c_, int k);
+    LaunchScope(exx_ctx* c_, int k, int64_t units = 0);
     ~LaunchScope();
 };
 

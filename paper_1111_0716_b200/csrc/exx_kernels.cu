@@ -37,7 +37,7 @@ int launch_scatter(exx_ctx* c, int ik, const double2* coef, int nbatch, double2*
     int npw = c->npw[ik];
     for (int b0 = 0; b0 < nbatch; b0 += 32768) {
         int nb = nbatch - b0 < 32768 ? nbatch - b0 : 32768;
-        LaunchScope ls(c, KC_SCATTER);
+        LaunchScope ls(c, KC_SCATTER, nb);
         dim3 grid((npw + 255) / 256, nb);
         scatter_kernel<<<grid, 256, 0, c->stream>>>(coef + (int64_t)b0 * npw, c->map_dev + c->map_off[ik], npw, c->Ng, box + (int64_t)b0 * c->Ng);
     }
@@ -48,7 +48,7 @@ int launch_gather(exx_ctx* c, int ik, const double2* box, int nbatch, double2* c
     int npw = c->npw[ik];
     for (int b0 = 0; b0 < nbatch; b0 += 32768) {
         int nb = nbatch - b0 < 32768 ? nbatch - b0 : 32768;
-        LaunchScope ls(c, KC_GATHER);
+        LaunchScope ls(c, KC_GATHER, nb);
         dim3 grid((npw + 255) / 256, nb);
         gather_kernel<<<grid, 256, 0, c->stream>>>(box + (int64_t)b0 * c->Ng, c->map_dev + c->map_off[ik], npw, c->Ng, coef + (int64_t)b0 * npw);
     }
@@ -188,7 +188,7 @@ static int launch_fft_axis(exx_ctx* c, double2* data, int axis, int nbatch, int 
     Radices rad;
     rad.nst = pl.nst;
     for (int i = 0; i < 16; i++) rad.r[i] = pl.radix[i];
-    LaunchScope ls(c, KC_FFT_AXIS);
+    LaunchScope ls(c, KC_FFT_AXIS, nbatch);
     if (sign < 0)
         fft_axis_generic_kernel<-1><<<(unsigned)tiles, 256, smem, c->stream>>>(data, pl.tw_dev, n, rad, inner, nouter, P, pitch);
     else
@@ -226,7 +226,7 @@ __global__ void codensity_kernel(const double2* __restrict__ un_base, int n0, in
     }
 }
 int launch_codensity_tile(exx_ctx* c, const double2* un_base, int n0, int tn, const double2* uq_base, const MTile& mt, double2* work) {
-    LaunchScope ls(c, KC_CODENSITY);
+    LaunchScope ls(c, KC_CODENSITY, (int64_t)tn * mt.tm);
     dim3 grid((unsigned)((c->Ng + 255) / 256), tn);
     codensity_kernel<<<grid, 256, 0, c->stream>>>(un_base, n0, tn, uq_base, mt, c->Ng, work);
     EXX_CUDA(c, cudaGetLastError());
@@ -243,7 +243,7 @@ __global__ void kmul_kernel(const double* __restrict__ ktab, double2* __restrict
     *w = make_double2(kv * v.x, kv * v.y);
 }
 int launch_kmul(exx_ctx* c, const double* ktab, double2* work, int nboxes) {
-    LaunchScope ls(c, KC_KMUL);
+    LaunchScope ls(c, KC_KMUL, nboxes);
     dim3 grid((unsigned)((c->Ng + 255) / 256), nboxes);
     kmul_kernel<<<grid, 256, 0, c->stream>>>(ktab, work, c->Ng);
     EXX_CUDA(c, cudaGetLastError());
@@ -267,7 +267,7 @@ __global__ void accumulate_kernel(const double2* __restrict__ uq_base, MTile mt,
     acc[(int64_t)i * Ng + r] = a;
 }
 int launch_accumulate_tile(exx_ctx* c, const double2* uq_base, const MTile& mt, int tn, const double2* work, double2* acc) {
-    LaunchScope ls(c, KC_ACCUM);
+    LaunchScope ls(c, KC_ACCUM, (int64_t)tn * mt.tm);
     dim3 grid((unsigned)((c->Ng + 255) / 256), tn);
     accumulate_kernel<<<grid, 256, 0, c->stream>>>(uq_base, mt, c->Ng, work, acc);
     EXX_CUDA(c, cudaGetLastError());

@@ -124,6 +124,25 @@ static int dev_alloc(exx_ctx* c, T** p, size_t count) {
 
 }  // namespace exx
 
+namespace exx {
+// S1: u_nk(r) for every band (batches bounded so a launch never exceeds ~2^28 elements)
+int compute_u_cache(exx_ctx* c, const double2* psi) {
+    int rc;
+    const int nb = c->nb, nk = c->nk;
+    const int64_t Ng = c->Ng;
+    for (int k = 0; k < nk; k++) {
+        int bmax = (int)std::max<int64_t>(1, std::min<int64_t>(nb, ((int64_t)1 << 28) / Ng));
+        for (int n0 = 0; n0 < nb; n0 += bmax) {
+            int bn = std::min(bmax, nb - n0);
+            double2* box = c->u_dev + ((size_t)k * nb + n0) * Ng;
+            if ((rc = launch_scatter(c, k, psi + c->off[k] + (int64_t)n0 * c->npw[k], bn, box))) return rc;
+            if ((rc = launch_fft3d_generic(c, box, bn, +1))) return rc;
+        }
+    }
+    return EXX_OK;
+}
+}  // namespace exx
+
 using namespace exx;
 
 extern "C" {
@@ -290,11 +309,18 @@ int exx_create(exx_ctx** out, const int grid[3], const double lattice[9], int nk
         // ---- workspaces
         int nbt = nk * nbands;
         if ((rc = dev_alloc(c, &c->u_dev, (size_t)nbt * c->Ng))) return fail(rc);
-        // generic pipeline: one n at a time, up to 16 m per tile, at most ~1 GiB of pair workspace
+        // generic pipeline: one n at a time, up to 16 m per tile, at most ~1 GiB of pair workspace;
+        // fused pipeline: tn x tm pairs per batch (work) and tn accumulators
         size_t box_bytes = sizeof(double2) * (size_t)c->Ng;
         size_t wb = std::max<size_t>(1, std::min<size_t>(16, ((size_t)1 << 30) / box_bytes));
         c->work_boxes = wb;
         c->acc_boxes = 1;
+        if (fused_supported(c)) {
+            int tn, tm;
+            fused_tiles(c, &tn, &tm);
+            c->acc_boxes = tn;
+            c->work_boxes = std::max<size_t>(wb, (size_t)tn * tm);
+        }
         if ((rc = dev_alloc(c, &c->work_dev, c->work_boxes * c->Ng))) return fail(rc);
         if ((rc = dev_alloc(c, &c->acc_dev, c->acc_boxes * c->Ng))) return fail(rc);
         if ((rc = dev_alloc(c, &c->vx_dev, (size_t)c->off[nk]))) return fail(rc);
@@ -480,16 +506,7 @@ static int apply_generic(exx_ctx* c, const double2* psi, const double* occ, doub
     const int64_t Ng = c->Ng;
     c->path_used = 1;
     c->pruned_used = 0;
-    // S1: u_nk(r) for every band (batches bounded so a launch never exceeds ~2^31 elements of work per grid dim)
-    for (int k = 0; k < nk; k++) {
-        int bmax = (int)std::max<int64_t>(1, std::min<int64_t>(nb, ((int64_t)1 << 28) / Ng));
-        for (int n0 = 0; n0 < nb; n0 += bmax) {
-            int bn = std::min(bmax, nb - n0);
-            double2* box = c->u_dev + ((size_t)k * nb + n0) * Ng;
-            if ((rc = launch_scatter(c, k, psi + c->off[k] + (int64_t)n0 * c->npw[k], bn, box))) return rc;
-            if ((rc = launch_fft3d_generic(c, box, bn, +1))) return rc;
-        }
-    }
+    if ((rc = compute_u_cache(c, psi))) return rc;
     int tm_max = (int)std::min<size_t>(c->work_boxes, 32);
     if (c->opt_tile_m > 0) tm_max = (int)std::min<int64_t>(tm_max, c->opt_tile_m);
     c->tile_n_used = 1;

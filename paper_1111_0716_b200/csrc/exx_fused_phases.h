@@ -1,0 +1,351 @@
+// exx_fused_phases.h — the per-thread phases of the three fused passes, written as
+// __host__ __device__ functions of (tid, tile) so that exx_fused.cu can run them between __syncthreads() and
+// exx_host_emu.cpp can run the very same index logic thread by thread on the CPU (host logic test, no GPU).
+// Product code: shares nothing with oracle/.
+//
+// Grid N = 8 R1 per axis (cubic), R1 in {6, 8, 9, 12, 16}.  Every 1-D transform of length N is two in-register steps
+//   n = 8 n1 + n2, k = k1 + R1 k2:   R1-point DFT over n1 (stride 8)  ->  twiddle W_N^(n2 k1)  ->  8-point DFT over n2
+// done in place, so a frequency k sits at position pos(k) = 8 (k mod R1) + k div R1; the inverse runs the two steps
+// backwards and lands in natural order.  The pair pipeline (S2..S6) is cut at the two points where a full exchange
+// through memory is unavoidable:
+//   pass A (p1_*): rho = conj(u_m) u_n; z transform (both steps); first y step          tile: one x, U values of y mod 8
+//   pass B (p2_*): second y step; x transform; times K'; inverse x; first inverse y step  tile: one k1y, Z positions of z
+//   pass C (p3_*): second inverse y step; inverse z; acc -= w f u_m v                     tile: as pass A, loops over m
+#pragma once
+#include <stddef.h>
+
+#include "exx_dft.h"
+
+namespace exx {
+
+// twiddle tables W_N^j, j < N, for every supported N, in one array (constant memory on the device)
+constexpr int TW_TOTAL = 48 + 64 + 72 + 96 + 128;
+template <int R1>
+struct TwOff;
+template <>
+struct TwOff<6> {
+    static constexpr int v = 0;
+};
+template <>
+struct TwOff<8> {
+    static constexpr int v = 48;
+};
+template <>
+struct TwOff<9> {
+    static constexpr int v = 112;
+};
+template <>
+struct TwOff<12> {
+    static constexpr int v = 184;
+};
+template <>
+struct TwOff<16> {
+    static constexpr int v = 280;
+};
+
+#if defined(__CUDA_ARCH__)
+#define EXX_TW(R1, j) c_tw[TwOff<R1>::v + (j)]
+#else
+extern cplx h_tw[TW_TOTAL];
+#define EXX_TW(R1, j) h_tw[TwOff<R1>::v + (j)]
+#endif
+
+// per-grid launch geometry: U = tile height of passes A/C in units of R1 rows, NT13 = their CTA size, Z = z positions per
+// pass-B tile, NT2 = its CTA size (chosen so that every step's item count is a small multiple of the thread count)
+template <int R1>
+struct FusedCfg;
+template <>
+struct FusedCfg<6> {
+    static constexpr int U = 4, NT13 = 96, Z = 4, NT2 = 64;
+};
+template <>
+struct FusedCfg<8> {
+    static constexpr int U = 4, NT13 = 128, Z = 4, NT2 = 128;
+};
+template <>
+struct FusedCfg<9> {
+    static constexpr int U = 4, NT13 = 96, Z = 4, NT2 = 96;
+};
+template <>
+struct FusedCfg<12> {
+    static constexpr int U = 2, NT13 = 96, Z = 4, NT2 = 128;
+};
+template <>
+struct FusedCfg<16> {
+    static constexpr int U = 1, NT13 = 128, Z = 4, NT2 = 256;
+};
+
+// ---- shared-memory layouts -------------------------------------------------------------------------------------
+// passes A/C: S[row][k1z][j], XOR swizzle of j with (row R1 + k1z) & 7: conflict-free for the three access patterns
+// (lanes along j; lanes along (row,k1z); lanes along the position 8 k1z + j), no padding.
+template <int R1>
+EXX_HD int sidx(int row, int k1z, int j) {
+    return row * (8 * R1) + k1z * 8 + (j ^ ((row * R1 + k1z) & 7));
+}
+// z twiddle table in shared memory: T[k1z][j] = W_N^(j k1z), same swizzle idea
+EXX_HD int tidx(int k1z, int j) { return k1z * 8 + (j ^ (k1z & 7)); }
+
+// pass B: S[xpos][k2y][kzl], x pitch padded so that lanes along (xpos, kzl) are conflict-free
+template <int Z>
+struct P2Geo {
+    static constexpr int PX = 8 * Z + (Z == 8 ? 0 : Z);
+};
+
+// ================================================================================================================
+// pass A
+template <int R1, int U, int NT>
+EXX_HD void p1_z1(int tid, const cplx* __restrict__ un, const cplx* __restrict__ um, int x, int yb, cplx* S) {
+    constexpr int N = 8 * R1, NI = U * R1 * 8, IT = (NI + NT - 1) / NT;
+#pragma unroll
+    for (int i = 0; i < IT; i++) {
+        int it = tid + i * NT;
+        if (it < NI) {
+            int row = it >> 3, n2z = it & 7;
+            int u = row / R1, n1y = row - u * R1;
+            size_t base = ((size_t)x * N + (n1y * 8 + yb * U + u)) * N + n2z;
+            cplx a[R1], b[R1], v[R1];
+#pragma unroll
+            for (int j = 0; j < R1; j++) {
+                a[j] = un[base + j * 8];
+                b[j] = um[base + j * 8];
+            }
+#pragma unroll
+            for (int j = 0; j < R1; j++) v[j] = conj_mul(b[j], a[j]);  // rho = conj(u_m) u_n   (S2)
+            dft<R1, -1>(v);
+#pragma unroll
+            for (int j = 0; j < R1; j++) S[sidx<R1>(row, j, n2z)] = v[j];
+        }
+    }
+}
+
+template <int R1, int U, int NT, int SIGN>
+EXX_HD void p13_z8(int tid, cplx* S, const cplx* T) {
+    // the 8-point z step on items (row, k1z).  SIGN < 0: twiddle then forward DFT; SIGN > 0: inverse DFT then conj twiddle
+    constexpr int NI = U * R1 * R1, IT = (NI + NT - 1) / NT;
+#pragma unroll
+    for (int i = 0; i < IT; i++) {
+        int it = tid + i * NT;
+        if (it < NI) {
+            int row = it / R1, k1z = it - row * R1;
+            cplx v[8];
+#pragma unroll
+            for (int j = 0; j < 8; j++) v[j] = S[sidx<R1>(row, k1z, j)];
+            if (SIGN < 0) {
+#pragma unroll
+                for (int j = 1; j < 8; j++) v[j] = v[j] * T[tidx(k1z, j)];
+                dft<8, -1>(v);
+            } else {
+                dft<8, +1>(v);
+#pragma unroll
+                for (int j = 1; j < 8; j++) v[j] = mul_conj_b(v[j], T[tidx(k1z, j)]);
+            }
+#pragma unroll
+            for (int j = 0; j < 8; j++) S[sidx<R1>(row, k1z, j)] = v[j];
+        }
+    }
+}
+
+template <int R1, int U, int NT>
+EXX_HD void p1_y1(int tid, const cplx* S, cplx* __restrict__ W, int x, int yb) {
+    constexpr int N = 8 * R1, NI = U * N, IT = (NI + NT - 1) / NT;
+#pragma unroll
+    for (int i = 0; i < IT; i++) {
+        int it = tid + i * NT;
+        if (it < NI) {
+            int u = it / N, kzpos = it - u * N;
+            cplx v[R1];
+#pragma unroll
+            for (int j = 0; j < R1; j++) v[j] = S[sidx<R1>(u * R1 + j, kzpos >> 3, kzpos & 7)];
+            dft<R1, -1>(v);
+            size_t base = ((size_t)x * N + (yb * U + u)) * N + kzpos;
+#pragma unroll
+            for (int j = 0; j < R1; j++) W[base + (size_t)j * 8 * N] = v[j];  // row k1y * 8 + n2y
+        }
+    }
+}
+
+// ================================================================================================================
+// pass B.  Tile: rows k1y*8 + n2y (n2y < 8), all x, z positions zb*Z .. zb*Z+Z-1.
+template <int R1, int Z, int NT>
+EXX_HD void p2_yf(int tid, const cplx* __restrict__ W, int k1y, int zb, cplx* S) {
+    constexpr int N = 8 * R1, NI = N * Z, IT = (NI + NT - 1) / NT, PX = P2Geo<Z>::PX;
+#pragma unroll
+    for (int i = 0; i < IT; i++) {
+        int it = tid + i * NT;
+        if (it < NI) {
+            int xpos = it / Z, kzl = it - xpos * Z;
+            size_t base = ((size_t)xpos * N + k1y * 8) * N + zb * Z + kzl;
+            cplx v[8];
+#pragma unroll
+            for (int j = 0; j < 8; j++) v[j] = W[base + (size_t)j * N];
+#pragma unroll
+            for (int j = 1; j < 8; j++) v[j] = v[j] * EXX_TW(R1, j * k1y);  // y twiddle W_N^(n2y k1y), uniform per CTA
+            dft<8, -1>(v);
+#pragma unroll
+            for (int j = 0; j < 8; j++) S[xpos * PX + j * Z + kzl] = v[j];
+        }
+    }
+}
+
+template <int R1, int Z, int NT, int SIGN>
+EXX_HD void p2_xR(int tid, cplx* S) {
+    // the R1-point x step on items (n2x, rem = k2y*Z + kzl).  Forward: DFT then twiddle W_N^(n2x k1x); inverse: DFT only
+    // (the conjugate twiddle was applied at the end of p2_x8).
+    constexpr int NI = 8 * 8 * Z, IT = (NI + NT - 1) / NT, PX = P2Geo<Z>::PX;
+#pragma unroll
+    for (int i = 0; i < IT; i++) {
+        int it = tid + i * NT;
+        if (it < NI) {
+            int n2x = it / (8 * Z), rem = it - n2x * (8 * Z);
+            cplx v[R1];
+#pragma unroll
+            for (int j = 0; j < R1; j++) v[j] = S[(j * 8 + n2x) * PX + rem];
+            dft<R1, SIGN>(v);
+            if (SIGN < 0) {
+#pragma unroll
+                for (int j = 1; j < R1; j++) v[j] = v[j] * EXX_TW(R1, n2x * j);
+            }
+#pragma unroll
+            for (int j = 0; j < R1; j++) S[(j * 8 + n2x) * PX + rem] = v[j];
+        }
+    }
+}
+
+template <int R1, int Z, int NT>
+EXX_HD void p2_x8(int tid, cplx* S, const double* __restrict__ Kt) {
+    // items (k1x, rem): second forward x step, times K' (S4), first inverse x step, conjugate twiddle.
+    // Kt: this tile's slice of the permuted kernel table, 8 consecutive doubles (k2x = 0..7) per item.
+    constexpr int NI = R1 * 8 * Z, IT = (NI + NT - 1) / NT, PX = P2Geo<Z>::PX;
+#pragma unroll
+    for (int i = 0; i < IT; i++) {
+        int it = tid + i * NT;
+        if (it < NI) {
+            int k1x = it / (8 * Z), rem = it - k1x * (8 * Z);
+            cplx v[8];
+            double kk[8];
+#pragma unroll
+            for (int j = 0; j < 8; j++) kk[j] = Kt[(size_t)it * 8 + j];
+#pragma unroll
+            for (int j = 0; j < 8; j++) v[j] = S[(k1x * 8 + j) * PX + rem];
+            dft<8, -1>(v);
+#pragma unroll
+            for (int j = 0; j < 8; j++) v[j] = scale(kk[j], v[j]);
+            dft<8, +1>(v);
+#pragma unroll
+            for (int j = 1; j < 8; j++) v[j] = mul_conj_b(v[j], EXX_TW(R1, j * k1x));
+#pragma unroll
+            for (int j = 0; j < 8; j++) S[(k1x * 8 + j) * PX + rem] = v[j];
+        }
+    }
+}
+
+template <int R1, int Z, int NT>
+EXX_HD void p2_yinv(int tid, const cplx* S, cplx* __restrict__ W, int k1y, int zb) {
+    constexpr int N = 8 * R1, NI = N * Z, IT = (NI + NT - 1) / NT, PX = P2Geo<Z>::PX;
+#pragma unroll
+    for (int i = 0; i < IT; i++) {
+        int it = tid + i * NT;
+        if (it < NI) {
+            int xpos = it / Z, kzl = it - xpos * Z;
+            size_t base = ((size_t)xpos * N + k1y * 8) * N + zb * Z + kzl;
+            cplx v[8];
+#pragma unroll
+            for (int j = 0; j < 8; j++) v[j] = S[xpos * PX + j * Z + kzl];
+            dft<8, +1>(v);
+#pragma unroll
+            for (int j = 1; j < 8; j++) v[j] = mul_conj_b(v[j], EXX_TW(R1, j * k1y));
+#pragma unroll
+            for (int j = 0; j < 8; j++) W[base + (size_t)j * N] = v[j];
+        }
+    }
+}
+
+// ================================================================================================================
+// pass C
+template <int R1, int U, int NT>
+EXX_HD void p3_y2inv(int tid, const cplx* __restrict__ W, int x, int yb, cplx* S) {
+    constexpr int N = 8 * R1, NI = U * N, IT = (NI + NT - 1) / NT;
+#pragma unroll
+    for (int i = 0; i < IT; i++) {
+        int it = tid + i * NT;
+        if (it < NI) {
+            int u = it / N, kzpos = it - u * N;
+            size_t base = ((size_t)x * N + (yb * U + u)) * N + kzpos;
+            cplx v[R1];
+#pragma unroll
+            for (int j = 0; j < R1; j++) v[j] = W[base + (size_t)j * 8 * N];
+            dft<R1, +1>(v);
+#pragma unroll
+            for (int j = 0; j < R1; j++) S[sidx<R1>(u * R1 + j, kzpos >> 3, kzpos & 7)] = v[j];
+        }
+    }
+}
+
+template <int R1, int U, int NT>
+EXX_HD void p3_zinv2(int tid, const cplx* S, const cplx* __restrict__ um, double wf, int x, int yb, cplx* A, bool first) {
+    // items (row, n2z): last inverse z step, then acc -= (w_q f_m) u_m v   (S6); A is this CTA's private accumulator tile
+    constexpr int N = 8 * R1, NI = U * R1 * 8, IT = (NI + NT - 1) / NT;
+#pragma unroll
+    for (int i = 0; i < IT; i++) {
+        int it = tid + i * NT;
+        if (it < NI) {
+            int row = it >> 3, n2z = it & 7;
+            int u = row / R1, n1y = row - u * R1;
+            size_t base = ((size_t)x * N + (n1y * 8 + yb * U + u)) * N + n2z;
+            cplx b[R1], v[R1];
+#pragma unroll
+            for (int j = 0; j < R1; j++) b[j] = um[base + j * 8];
+#pragma unroll
+            for (int j = 0; j < R1; j++) v[j] = S[sidx<R1>(row, j, n2z)];
+            dft<R1, +1>(v);
+#pragma unroll
+            for (int j = 0; j < R1; j++) {
+                cplx p = b[j] * v[j];
+                cplx* a = A + row * N + j * 8 + n2z;
+                if (first)
+                    *a = mk(-wf * p.x, -wf * p.y);
+                else
+                    *a = mk(a->x - wf * p.x, a->y - wf * p.y);
+            }
+        }
+    }
+}
+
+template <int R1, int U, int NT>
+EXX_HD void p3_flush(int tid, const cplx* A, cplx* __restrict__ accg, int x, int yb) {
+    constexpr int N = 8 * R1, NI = U * R1 * 8, IT = (NI + NT - 1) / NT;
+#pragma unroll
+    for (int i = 0; i < IT; i++) {
+        int it = tid + i * NT;
+        if (it < NI) {
+            int row = it >> 3, n2z = it & 7;
+            int u = row / R1, n1y = row - u * R1;
+            size_t base = ((size_t)x * N + (n1y * 8 + yb * U + u)) * N + n2z;
+#pragma unroll
+            for (int j = 0; j < R1; j++) {
+                cplx g = accg[base + j * 8], a = A[row * N + j * 8 + n2z];
+                accg[base + j * 8] = g + a;
+            }
+        }
+    }
+}
+
+// ================================================================================================================
+// Host side of the layout: K' in natural C order -> the order pass B reads it in,
+//   [k1y][zb][k1x][k2y][kzl][k2x]  with kx = k1x + R1 k2x, ky = k1y + R1 k2y, zpos = zb Z + kzl = 8 k1z + k2z, kz = k1z + R1 k2z.
+inline void permute_ktable(int R1, int Z, const double* nat, double* perm) {
+    const int N = 8 * R1;
+    size_t o = 0;
+    for (int k1y = 0; k1y < R1; k1y++)
+        for (int zb = 0; zb < N / Z; zb++)
+            for (int k1x = 0; k1x < R1; k1x++)
+                for (int k2y = 0; k2y < 8; k2y++)
+                    for (int kzl = 0; kzl < Z; kzl++)
+                        for (int k2x = 0; k2x < 8; k2x++) {
+                            int zpos = zb * Z + kzl, k1z = zpos >> 3, k2z = zpos & 7;
+                            int kx = k1x + R1 * k2x, ky = k1y + R1 * k2y, kz = k1z + R1 * k2z;
+                            perm[o++] = nat[((size_t)kx * N + ky) * N + kz];
+                        }
+}
+
+}  // namespace exx

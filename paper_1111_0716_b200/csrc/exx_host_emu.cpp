@@ -1,0 +1,96 @@
+// exx_host_emu.cpp — CPU execution of the fused passes' per-thread phases (exx_fused_phases.h), thread by thread and
+// tile by tile, exactly as exx_fused.cu schedules them on the device.  Built only by tests/test_fused_host_emulation.py
+// (g++, no CUDA); it lets the index/layout logic of the kernels be checked without a GPU.  Not part of libexx.so.
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <vector>
+
+#include "exx_fused_phases.h"
+
+namespace exx {
+cplx h_tw[TW_TOTAL];
+
+static void fill_tw() {
+    const int Ns[5] = {48, 64, 72, 96, 128};
+    const int off[5] = {TwOff<6>::v, TwOff<8>::v, TwOff<9>::v, TwOff<12>::v, TwOff<16>::v};
+    const long double tp = 6.283185307179586476925286766559005768L;
+    for (int s = 0; s < 5; s++)
+        for (int j = 0; j < Ns[s]; j++) {
+            long double a = tp * j / Ns[s];
+            h_tw[off[s] + j] = mk((double)cosl(a), (double)(-sinl(a)));
+        }
+}
+
+template <int R1>
+static void emu_pair(const cplx* un, const cplx* um, const double* Knat, double wf, cplx* acc, cplx* W) {
+    typedef FusedCfg<R1> C;
+    constexpr int N = 8 * R1, U = C::U, NT13 = C::NT13, Z = C::Z, NT2 = C::NT2;
+    std::vector<double> Kp((size_t)N * N * N);
+    permute_ktable(R1, Z, Knat, Kp.data());
+    std::vector<cplx> S((size_t)U * R1 * N), A((size_t)U * R1 * N), T(R1 * 8), S2((size_t)N * P2Geo<Z>::PX);
+    for (int k = 0; k < R1; k++)
+        for (int j = 0; j < 8; j++) T[tidx(k, j)] = EXX_TW(R1, j * k);
+    // pass A
+    for (int x = 0; x < N; x++)
+        for (int yb = 0; yb < 8 / U; yb++) {
+            for (int t = 0; t < NT13; t++) p1_z1<R1, U, NT13>(t, un, um, x, yb, S.data());
+            for (int t = 0; t < NT13; t++) p13_z8<R1, U, NT13, -1>(t, S.data(), T.data());
+            for (int t = 0; t < NT13; t++) p1_y1<R1, U, NT13>(t, S.data(), W, x, yb);
+        }
+    // pass B
+    for (int k1y = 0; k1y < R1; k1y++)
+        for (int zb = 0; zb < N / Z; zb++) {
+            const double* Kt = Kp.data() + ((size_t)k1y * (N / Z) + zb) * ((size_t)N * 8 * Z);
+            for (int t = 0; t < NT2; t++) p2_yf<R1, Z, NT2>(t, W, k1y, zb, S2.data());
+            for (int t = 0; t < NT2; t++) p2_xR<R1, Z, NT2, -1>(t, S2.data());
+            for (int t = 0; t < NT2; t++) p2_x8<R1, Z, NT2>(t, S2.data(), Kt);
+            for (int t = 0; t < NT2; t++) p2_xR<R1, Z, NT2, +1>(t, S2.data());
+            for (int t = 0; t < NT2; t++) p2_yinv<R1, Z, NT2>(t, S2.data(), W, k1y, zb);
+        }
+    // pass C (one m)
+    for (int x = 0; x < N; x++)
+        for (int yb = 0; yb < 8 / U; yb++) {
+            for (int t = 0; t < NT13; t++) p3_y2inv<R1, U, NT13>(t, W, x, yb, S.data());
+            for (int t = 0; t < NT13; t++) p13_z8<R1, U, NT13, +1>(t, S.data(), T.data());
+            for (int t = 0; t < NT13; t++) p3_zinv2<R1, U, NT13>(t, S.data(), um, wf, x, yb, A.data(), true);
+            for (int t = 0; t < NT13; t++) p3_flush<R1, U, NT13>(t, A.data(), acc, x, yb);
+        }
+}
+}  // namespace exx
+
+using namespace exx;
+
+extern "C" {
+// in-register codelet: inout = R complex numbers, sign -1 forward / +1 unnormalised inverse
+int exx_emu_dft(int R, int sign, double* inout) {
+    cplx* v = (cplx*)inout;
+#define CASE(r)                 \
+    case r:                     \
+        if (sign < 0)           \
+            dft<r, -1>(v);      \
+        else                    \
+            dft<r, +1>(v);      \
+        return 0;
+    switch (R) {
+        CASE(2) CASE(3) CASE(4) CASE(6) CASE(8) CASE(9) CASE(12) CASE(16)
+    default: return -1;
+    }
+#undef CASE
+}
+
+// one pair evaluation through the three fused passes on the CPU: acc += -wf * u_m * IFFT[K' FFT[conj(u_m) u_n]]
+// (un, um, acc, work: N^3 complex each, 16-byte aligned; Knat: N^3 doubles in natural C order), N = 8 R1
+int exx_emu_pair(int R1, const double* un, const double* um, const double* Knat, double wf, double* acc, double* work) {
+    fill_tw();
+    switch (R1) {
+    case 6: emu_pair<6>((const cplx*)un, (const cplx*)um, Knat, wf, (cplx*)acc, (cplx*)work); return 0;
+    case 8: emu_pair<8>((const cplx*)un, (const cplx*)um, Knat, wf, (cplx*)acc, (cplx*)work); return 0;
+    case 9: emu_pair<9>((const cplx*)un, (const cplx*)um, Knat, wf, (cplx*)acc, (cplx*)work); return 0;
+    case 12: emu_pair<12>((const cplx*)un, (const cplx*)um, Knat, wf, (cplx*)acc, (cplx*)work); return 0;
+    case 16: emu_pair<16>((const cplx*)un, (const cplx*)um, Knat, wf, (cplx*)acc, (cplx*)work); return 0;
+    default: return -1;
+    }
+}
+}

@@ -130,9 +130,11 @@ int launch_codensity_tile(exx_ctx* c, const double2* un_base, int n0, int tn, co
 int launch_kmul(exx_ctx* c, const double* ktab, double2* work, int nboxes);
 int launch_accumulate_tile(exx_ctx* c, const double2* uq_base, const MTile& mt, int tn, const double2* work, double2* acc);
 int launch_energy(exx_ctx* c, const double2* psi, const double2* vx);
+int compute_u_cache(exx_ctx* c, const double2* psi);  // exx_api.cu: S1 for every band
 
 // ---- fused path (exx_fused.cu) ----
 bool fused_supported(const exx_ctx* c);
+void fused_tiles(const exx_ctx* c, int* tn, int* tm);
 int fused_create(exx_ctx* c);
 void fused_destroy(exx_ctx* c);
 int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out);

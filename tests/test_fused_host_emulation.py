@@ -1,0 +1,80 @@
+"""Host-logic test (no GPU): the fused passes' per-thread phases (csrc/exx_fused_phases.h) and the in-register DFT
+codelets (csrc/exx_dft.h) are __host__ __device__ code; csrc/exx_host_emu.cpp runs them on the CPU thread by thread and
+tile by tile in the order exx_fused.cu launches them.  Compared here with numpy.fft (a library routine, independent of
+the product): this checks the index maps of the two-step transforms, the shared-memory layouts, the permuted kernel
+table and the accumulation — everything about the kernels except the device-side barriers and memory system.
+"""
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+SRC = os.path.join(ROOT, "paper_1111_0716_b200", "csrc", "exx_host_emu.cpp")
+dp = C.POINTER(C.c_double)
+
+
+@pytest.fixture(scope="module")
+def emu(tmp_path_factory):
+    so = str(tmp_path_factory.mktemp("emu") / "libexx_emu.so")
+    subprocess.check_call(["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-ffp-contract=off", "-o", so, SRC])
+    L = C.CDLL(so)
+    L.exx_emu_dft.argtypes = [C.c_int, C.c_int, dp]
+    L.exx_emu_pair.argtypes = [C.c_int, dp, dp, dp, C.c_double, dp, dp]
+    return L
+
+
+def _p(a):
+    return a.ctypes.data_as(dp)
+
+
+@pytest.mark.parametrize("R", [2, 3, 4, 6, 8, 9, 12, 16])
+@pytest.mark.parametrize("sign", [-1, 1])
+def test_codelets_against_numpy(emu, R, sign):
+    rng = np.random.default_rng(100 * R + sign)
+    x = rng.standard_normal(R) + 1j * rng.standard_normal(R)
+    v = x.copy()
+    assert emu.exx_emu_dft(R, sign, _p(v)) == 0
+    want = np.fft.fft(x) if sign < 0 else np.fft.ifft(x) * R
+    assert np.linalg.norm(v - want) <= 1e-15 * R * np.linalg.norm(want)
+    # delta -> constant, constant -> delta (exact)
+    d = np.zeros(R, dtype=np.complex128)
+    d[0] = 1.0
+    emu.exx_emu_dft(R, sign, _p(d))
+    assert np.array_equal(d, np.ones(R))
+
+
+@pytest.mark.parametrize("R1", [6, 8, 9, 12, 16])
+def test_three_passes_equal_definition(emu, R1):
+    """acc += -w f u_m IFFT[K' FFT[conj(u_m) u_n]] (unnormalised transforms), one pair, whole box."""
+    N = 8 * R1
+    rng = np.random.default_rng(R1)
+    shp = (N, N, N)
+    un = rng.standard_normal(shp) + 1j * rng.standard_normal(shp)
+    um = rng.standard_normal(shp) + 1j * rng.standard_normal(shp)
+    K = rng.random(shp)  # any real table: an asymmetric one catches transposed / mirrored frequency indices
+    acc0 = rng.standard_normal(shp) + 1j * rng.standard_normal(shp)
+    acc, work = acc0.copy(), np.zeros(shp, dtype=np.complex128)
+    wf = 0.7
+    assert emu.exx_emu_pair(R1, _p(un), _p(um), _p(K), wf, _p(acc), _p(work)) == 0
+    want = -wf * um * np.fft.ifftn(K * np.fft.fftn(np.conj(um) * un)) * N ** 3
+    assert np.linalg.norm(acc - acc0 - want) <= 1e-14 * np.linalg.norm(want)
+
+
+def test_single_plane_wave_pair(emu):
+    """u_n = e^{i g_n.r}, u_m = e^{i g_m.r}: the pair density is one plane wave, so the result is K'(g_n-g_m) Ng u_n."""
+    R1 = 6
+    N = 8 * R1
+    j = np.arange(N)
+    def pw(g):
+        return np.exp(2j * np.pi * (g[0] * j[:, None, None] + g[1] * j[None, :, None] + g[2] * j[None, None, :]) / N)
+    gn, gm = (3, -2, 5), (1, 4, -7)
+    K = np.random.default_rng(5).random((N, N, N))
+    acc, work = np.zeros((N, N, N), dtype=np.complex128), np.zeros((N, N, N), dtype=np.complex128)
+    un, um = pw(gn), pw(gm)
+    assert emu.exx_emu_pair(R1, _p(un), _p(um), _p(K), 1.0, _p(acc), _p(work)) == 0
+    d = [(a - b) % N for a, b in zip(gn, gm)]
+    want = -K[d[0], d[1], d[2]] * N ** 3 * un
+    assert np.abs(acc - want).max() <= 1e-12 * N ** 3

@@ -31,16 +31,18 @@ def needs_build():
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force=False, verbose=False, extra=()):
-    if not force and not needs_build():
+def build(force=False, verbose=False, extra=(), out=None):
+    """Build libexx.so (or `out`, e.g. a tuning variant compiled with extra -D flags)."""
+    if out is None and not force and not needs_build():
         return LIB
-    tmp = LIB + ".tmp.%d" % os.getpid()
+    target = out or LIB
+    tmp = target + ".tmp.%d" % os.getpid()
     cmd = [_nvcc()] + NVCC_FLAGS + list(extra) + ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
     if verbose:
         print(" ".join(cmd))
     subprocess.check_call(cmd)
-    os.replace(tmp, LIB)
-    return LIB
+    os.replace(tmp, target)
+    return target
 
 
 if __name__ == "__main__":

@@ -28,9 +28,11 @@ struct FusedState {
 // pass A: rho = conj(u_m) u_n, z transform, first y step.  One CTA per (tile, m, n), n fastest so that the CTAs that
 // share a u_m / u_n tile run back to back and the tile is fetched from HBM once.
 template <int R1>
-__global__ void __launch_bounds__(FusedCfg<R1>::NT13) pass_a_kernel(const cplx* __restrict__ un_base, const cplx* __restrict__ uq_base,
+__global__ void __launch_bounds__(FusedCfg<R1>::NT1, FusedCfg<R1>::MINB1) pass_a_kernel(const cplx* __restrict__ un_base, const cplx* __restrict__ uq_base,
                                                                     MTile mt, int tn, cplx* __restrict__ work) {
-    constexpr int N = 8 * R1, U = FusedCfg<R1>::U, NT = FusedCfg<R1>::NT13;
+    constexpr int N = 8 * R1, U = FusedCfg<R1>::U1, NT = FusedCfg<R1>::NT1;
+    constexpr bool TWREG = FusedCfg<R1>::TWREG;
+    static_assert(!TWREG || NT % R1 == 0, "TWREG needs a thread-invariant k1z");
     constexpr size_t Ng = (size_t)N * N * N;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx* S = reinterpret_cast<cplx*>(smem_raw);
@@ -42,32 +44,81 @@ __global__ void __launch_bounds__(FusedCfg<R1>::NT13) pass_a_kernel(const cplx* 
     const int m = bid % mt.tm;
     const int tile = bid / mt.tm;
     const int x = tile / (8 / U), yb = tile % (8 / U);
-    for (int i = tid; i < R1 * 8; i += NT) T[tidx(i >> 3, i & 7)] = c_tw[TwOff<R1>::v + (i >> 3) * (i & 7)];
+    cplx twr[8];
+    if (TWREG)
+        load_twr<R1>(tid, twr);
+    else
+        for (int i = tid; i < R1 * 8; i += NT) T[tidx(i >> 3, i & 7)] = c_tw[TwOff<R1>::v + (i >> 3) * (i & 7)];
     const cplx* un = un_base + (size_t)n * Ng;
     const cplx* um = uq_base + (size_t)mt.m_idx[m] * Ng;
     cplx* W = work + ((size_t)n * mt.tm + m) * Ng;
     p1_z1<R1, U, NT>(tid, un, um, x, yb, S);
     __syncthreads();
-    p13_z8<R1, U, NT, -1>(tid, S, T);
+    p13_z8<R1, U, NT, -1, TWREG>(tid, S, T, twr);
     __syncthreads();
     p1_y1<R1, U, NT>(tid, S, W, x, yb);
 }
 
-// pass B: second y step, x transform, K', inverse x, first inverse y step; in place on the pair's work box.
+// ---- bulk-copy (TMA, 1-D) and mbarrier helpers for pass B --------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)), "l"(gsrc),
+                 "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void* gdst, const void* smem_src, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(smem_u32(smem_src)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit_wait_all() {
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+}
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// pass B: second y step, x transform, K', inverse x, first inverse y step; in place on the pair's work box.  The tile
+// (k1y, zb) is one contiguous run of the work box (layout widx): N rows of 512 bytes are bulk-copied (TMA) into the padded
+// shared-memory tile, all five steps run in shared memory, and the rows are bulk-copied back.
 template <int R1>
-__global__ void __launch_bounds__(FusedCfg<R1>::NT2) pass_b_kernel(cplx* __restrict__ work, const double* __restrict__ kperm, int npairs) {
-    constexpr int N = 8 * R1, Z = FusedCfg<R1>::Z, NT = FusedCfg<R1>::NT2;
+__global__ void __launch_bounds__(FusedCfg<R1>::NT2, FusedCfg<R1>::MINB2) pass_b_kernel(cplx* __restrict__ work, const double* __restrict__ kperm, int npairs) {
+    constexpr int N = 8 * R1, Z = FusedCfg<R1>::Z, NT = FusedCfg<R1>::NT2, PX = P2Geo<Z>::PX;
     constexpr size_t Ng = (size_t)N * N * N;
+    constexpr uint32_t ROWB = 8 * Z * sizeof(cplx);
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx* S = reinterpret_cast<cplx*>(smem_raw);
+    __shared__ __align__(8) uint64_t bar;
     const int tid = threadIdx.x;
     const unsigned bid = blockIdx.x;
     const int pair = bid % npairs;
     const int tile = bid / npairs;
-    const int k1y = tile / (N / Z), zb = tile % (N / Z);
-    cplx* W = work + (size_t)pair * Ng;
+    const int k1y = tile / (N / Z);
+    cplx* Wt = work + (size_t)pair * Ng + (size_t)tile * ((size_t)N * 8 * Z);
     const double* Kt = kperm + (size_t)tile * ((size_t)N * 8 * Z);
-    p2_yf<R1, Z, NT>(tid, W, k1y, zb, S);
+    if (tid == 0) mbar_init(&bar, 1);
+    __syncthreads();
+    if (tid == 0) mbar_arrive_expect_tx(&bar, ROWB * N);
+    for (int x = tid; x < N; x += NT) bulk_g2s(S + x * PX, Wt + x * 8 * Z, ROWB, &bar);
+    mbar_wait(&bar, 0);
+    p2_y8<R1, Z, NT, -1>(tid, S, k1y);
     __syncthreads();
     p2_xR<R1, Z, NT, -1>(tid, S);
     __syncthreads();
@@ -75,45 +126,68 @@ __global__ void __launch_bounds__(FusedCfg<R1>::NT2) pass_b_kernel(cplx* __restr
     __syncthreads();
     p2_xR<R1, Z, NT, +1>(tid, S);
     __syncthreads();
-    p2_yinv<R1, Z, NT>(tid, S, W, k1y, zb);
+    p2_y8<R1, Z, NT, +1>(tid, S, k1y);
+    fence_proxy_async_smem();
+    __syncthreads();
+    for (int x = tid; x < N; x += NT) bulk_s2g(Wt + x * 8 * Z, S + x * PX, ROWB);
+    bulk_commit_wait_all();
 }
 
 // pass C: second inverse y step, inverse z, acc_n -= w f u_m v.  One CTA per (tile, n) loops over the m-tile with its
 // accumulator tile in shared memory, then adds it to acc_n in global memory once (fixed summation order).
 template <int R1>
-__global__ void __launch_bounds__(FusedCfg<R1>::NT13) pass_c_kernel(const cplx* __restrict__ work, const cplx* __restrict__ uq_base, MTile mt,
+__global__ void __launch_bounds__(FusedCfg<R1>::NT3, FusedCfg<R1>::MINB3) pass_c_kernel(const cplx* __restrict__ work, const cplx* __restrict__ uq_base, MTile mt,
                                                                     int tn, cplx* __restrict__ acc) {
-    constexpr int N = 8 * R1, U = FusedCfg<R1>::U, NT = FusedCfg<R1>::NT13;
+    constexpr int N = 8 * R1, U = FusedCfg<R1>::U3, NT = FusedCfg<R1>::NT3;
+    constexpr bool TWREG = FusedCfg<R1>::TWREG, ACCREG = FusedCfg<R1>::ACCREG;
+    static_assert(!TWREG || NT % R1 == 0, "TWREG needs a thread-invariant k1z");
     constexpr size_t Ng = (size_t)N * N * N;
+    constexpr int IT = (U * R1 * 8 + NT - 1) / NT;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx* S = reinterpret_cast<cplx*>(smem_raw);
-    cplx* A = S + U * R1 * N;
-    cplx* T = A + U * R1 * N;
+    cplx* A = S + U * R1 * N;                       // unused when ACCREG
+    cplx* T = A + (ACCREG ? 0 : U * R1 * N);
     const int tid = threadIdx.x;
     const unsigned bid = blockIdx.x;
     const int n = bid % tn;
     const int tile = bid / tn;
     const int x = tile / (8 / U), yb = tile % (8 / U);
-    for (int i = tid; i < R1 * 8; i += NT) T[tidx(i >> 3, i & 7)] = c_tw[TwOff<R1>::v + (i >> 3) * (i & 7)];
+    cplx twr[8];
+    if (TWREG)
+        load_twr<R1>(tid, twr);
+    else
+        for (int i = tid; i < R1 * 8; i += NT) T[tidx(i >> 3, i & 7)] = c_tw[TwOff<R1>::v + (i >> 3) * (i & 7)];
+    cplx accr[ACCREG ? IT * R1 : 1];
+    if (ACCREG) {
+#pragma unroll
+        for (int i = 0; i < (ACCREG ? IT * R1 : 1); i++) accr[i] = mk(0.0, 0.0);
+    }
     for (int m = 0; m < mt.tm; m++) {
         const cplx* W = work + ((size_t)n * mt.tm + m) * Ng;
         const cplx* um = uq_base + (size_t)mt.m_idx[m] * Ng;
         p3_y2inv<R1, U, NT>(tid, W, x, yb, S);
         __syncthreads();
-        p13_z8<R1, U, NT, +1>(tid, S, T);
+        p13_z8<R1, U, NT, +1, TWREG>(tid, S, T, twr);
         __syncthreads();
-        p3_zinv2<R1, U, NT>(tid, S, um, mt.wf[m], x, yb, A, m == 0);
+        if (ACCREG)
+            p3_zinv2_reg<R1, U, NT>(tid, S, um, mt.wf[m], x, yb, accr);
+        else
+            p3_zinv2<R1, U, NT>(tid, S, um, mt.wf[m], x, yb, A, m == 0);
         __syncthreads();
     }
-    p3_flush<R1, U, NT>(tid, A, acc + (size_t)n * Ng, x, yb);
+    if (ACCREG)
+        p3_flush_reg<R1, U, NT>(tid, accr, acc + (size_t)n * Ng, x, yb);
+    else
+        p3_flush<R1, U, NT>(tid, A, acc + (size_t)n * Ng, x, yb);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
 template <int R1>
 struct Launch {
-    static constexpr int N = 8 * R1, U = FusedCfg<R1>::U, Z = FusedCfg<R1>::Z;
-    static constexpr size_t smem_a = sizeof(cplx) * ((size_t)U * R1 * N + R1 * 8);
-    static constexpr size_t smem_c = sizeof(cplx) * ((size_t)2 * U * R1 * N + R1 * 8);
+    static constexpr int N = 8 * R1, U1 = FusedCfg<R1>::U1, U3 = FusedCfg<R1>::U3, Z = FusedCfg<R1>::Z;
+    static constexpr bool TWREG = FusedCfg<R1>::TWREG, ACCREG = FusedCfg<R1>::ACCREG;
+    static constexpr size_t smem_a = sizeof(cplx) * ((size_t)U1 * R1 * N + (TWREG ? 0 : R1 * 8));
+    static constexpr size_t smem_c = sizeof(cplx) * ((size_t)(ACCREG ? 1 : 2) * U3 * R1 * N + (TWREG ? 0 : R1 * 8));
     static constexpr size_t smem_b = sizeof(cplx) * ((size_t)N * P2Geo<Z>::PX);
 
     static int init(exx_ctx* c) {
@@ -125,10 +199,10 @@ struct Launch {
     // all pairs (n0..n0+tn) x mt of one (k, q): the three passes
     static int pairs(exx_ctx* c, const cplx* un_base, const cplx* uq_base, const MTile& mt, int tn, const double* kperm, cplx* work, cplx* acc) {
         const int npairs = tn * mt.tm;
-        const unsigned tiles13 = N * (8 / U), tiles2 = R1 * (N / Z);
+        const unsigned tiles1 = N * (8 / U1), tiles3 = N * (8 / U3), tiles2 = R1 * (N / Z);
         {
             LaunchScope ls(c, KC_PASS_A, npairs);
-            pass_a_kernel<R1><<<tiles13 * npairs, FusedCfg<R1>::NT13, smem_a, c->stream>>>(un_base, uq_base, mt, tn, work);
+            pass_a_kernel<R1><<<tiles1 * npairs, FusedCfg<R1>::NT1, smem_a, c->stream>>>(un_base, uq_base, mt, tn, work);
         }
         {
             LaunchScope ls(c, KC_PASS_B, npairs);
@@ -136,7 +210,7 @@ struct Launch {
         }
         {
             LaunchScope ls(c, KC_PASS_C, npairs);
-            pass_c_kernel<R1><<<tiles13 * tn, FusedCfg<R1>::NT13, smem_c, c->stream>>>(work, uq_base, mt, tn, acc);
+            pass_c_kernel<R1><<<tiles3 * tn, FusedCfg<R1>::NT3, smem_c, c->stream>>>(work, uq_base, mt, tn, acc);
         }
         EXX_CUDA(c, cudaGetLastError());
         return EXX_OK;

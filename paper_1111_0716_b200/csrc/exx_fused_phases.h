@@ -50,37 +50,88 @@ extern cplx h_tw[TW_TOTAL];
 #define EXX_TW(R1, j) h_tw[TwOff<R1>::v + (j)]
 #endif
 
-// per-grid launch geometry: U = tile height of passes A/C in units of R1 rows, NT13 = their CTA size, Z = z positions per
-// pass-B tile, NT2 = its CTA size (chosen so that every step's item count is a small multiple of the thread count)
+// per-grid launch geometry.  Passes A and C work on tiles of U*R1 rows (one x, U values of y mod 8) with NT1 / NT3 threads;
+// pass B on tiles of Z z-positions with NT2 threads.  Thread counts are chosen so that every step's item count is a small
+// multiple of the CTA size.  TWREG: the z twiddles W_N^(j k1z) live in 7 registers per thread (needs NT % R1 == 0 so that a
+// thread's k1z never changes) instead of a shared-memory table; ACCREG: pass C keeps its accumulator tile in registers
+// instead of shared memory.  The EXX_TUNE_* macros let a build override the N = 96 geometry (tuning sweeps).
+#ifndef EXX_TUNE_U1
+#define EXX_TUNE_U1 1
+#endif
+#ifndef EXX_TUNE_NT1
+#define EXX_TUNE_NT1 96
+#endif
+#ifndef EXX_TUNE_U3
+#define EXX_TUNE_U3 1
+#endif
+#ifndef EXX_TUNE_NT3
+#define EXX_TUNE_NT3 96
+#endif
+#ifndef EXX_TUNE_NT2
+#define EXX_TUNE_NT2 128
+#endif
+#ifndef EXX_TUNE_MINB1
+#define EXX_TUNE_MINB1 1
+#endif
+#ifndef EXX_TUNE_MINB2
+#define EXX_TUNE_MINB2 4
+#endif
+#ifndef EXX_TUNE_MINB3
+#define EXX_TUNE_MINB3 1
+#endif
+#ifndef EXX_TUNE_TWREG
+#define EXX_TUNE_TWREG 0
+#endif
+#ifndef EXX_TUNE_ACCREG
+#define EXX_TUNE_ACCREG 0
+#endif
 template <int R1>
 struct FusedCfg;
 template <>
 struct FusedCfg<6> {
-    static constexpr int U = 4, NT13 = 96, Z = 4, NT2 = 64;
+    static constexpr int U1 = 4, NT1 = 96, U3 = 4, NT3 = 96, Z = 4, NT2 = 64;
+    static constexpr bool TWREG = false, ACCREG = false;
+    static constexpr int MINB1 = 1, MINB2 = 1, MINB3 = 1;  // min CTAs per SM asked of the compiler (register cap)
 };
 template <>
 struct FusedCfg<8> {
-    static constexpr int U = 4, NT13 = 128, Z = 4, NT2 = 128;
+    static constexpr int U1 = 4, NT1 = 128, U3 = 4, NT3 = 128, Z = 4, NT2 = 128;
+    static constexpr bool TWREG = false, ACCREG = false;
+    static constexpr int MINB1 = 1, MINB2 = 1, MINB3 = 1;  // min CTAs per SM asked of the compiler (register cap)
 };
 template <>
 struct FusedCfg<9> {
-    static constexpr int U = 4, NT13 = 96, Z = 4, NT2 = 96;
+    static constexpr int U1 = 4, NT1 = 96, U3 = 4, NT3 = 96, Z = 4, NT2 = 96;
+    static constexpr bool TWREG = false, ACCREG = false;
+    static constexpr int MINB1 = 1, MINB2 = 1, MINB3 = 1;  // min CTAs per SM asked of the compiler (register cap)
 };
 template <>
 struct FusedCfg<12> {
-    static constexpr int U = 2, NT13 = 96, Z = 4, NT2 = 128;
+    static constexpr int U1 = EXX_TUNE_U1, NT1 = EXX_TUNE_NT1, U3 = EXX_TUNE_U3, NT3 = EXX_TUNE_NT3, Z = 4, NT2 = EXX_TUNE_NT2;
+    static constexpr bool TWREG = EXX_TUNE_TWREG != 0, ACCREG = EXX_TUNE_ACCREG != 0;
+    static constexpr int MINB1 = EXX_TUNE_MINB1, MINB2 = EXX_TUNE_MINB2, MINB3 = EXX_TUNE_MINB3;
 };
 template <>
 struct FusedCfg<16> {
-    static constexpr int U = 1, NT13 = 128, Z = 4, NT2 = 256;
+    static constexpr int U1 = 1, NT1 = 128, U3 = 1, NT3 = 128, Z = 4, NT2 = 256;
+    static constexpr bool TWREG = false, ACCREG = false;
+    static constexpr int MINB1 = 1, MINB2 = 1, MINB3 = 1;  // min CTAs per SM asked of the compiler (register cap)
 };
 
 // ---- shared-memory layouts -------------------------------------------------------------------------------------
-// passes A/C: S[row][k1z][j], XOR swizzle of j with (row R1 + k1z) & 7: conflict-free for the three access patterns
+// passes A/C: S[row][k1z][j], XOR swizzle of j with (row R1 + k1z) & 7 and 4 (u & 1): conflict-free for the three access patterns
 // (lanes along j; lanes along (row,k1z); lanes along the position 8 k1z + j), no padding.
 template <int R1>
-EXX_HD int sidx(int row, int k1z, int j) {
-    return row * (8 * R1) + k1z * 8 + (j ^ ((row * R1 + k1z) & 7));
+EXX_HD int sidx(int u, int r, int k1z, int j) {  // row = u R1 + r
+    int row = u * R1 + r;
+    return row * (8 * R1) + k1z * 8 + (j ^ (((row * R1 + k1z) & 7) ^ ((u & 1) << 2)));
+}
+// the pair work box W between the passes: [k1y][kzpos / 4][x][n2y][kzpos % 4] — a pass-B tile (k1y, zb) is one
+// contiguous run of N*32 elements (bulk-copied), and passes A/C touch it in runs of 4 U elements
+template <int R1>
+EXX_HD size_t widx(int k1y, int kzpos, int x, int n2y) {
+    constexpr int N = 8 * R1;
+    return ((((size_t)k1y * (N / 4) + (kzpos >> 2)) * N + x) * 8 + n2y) * 4 + (kzpos & 3);
 }
 // z twiddle table in shared memory: T[k1z][j] = W_N^(j k1z), same swizzle idea
 EXX_HD int tidx(int k1z, int j) { return k1z * 8 + (j ^ (k1z & 7)); }
@@ -113,13 +164,21 @@ EXX_HD void p1_z1(int tid, const cplx* __restrict__ un, const cplx* __restrict__
             for (int j = 0; j < R1; j++) v[j] = conj_mul(b[j], a[j]);  // rho = conj(u_m) u_n   (S2)
             dft<R1, -1>(v);
 #pragma unroll
-            for (int j = 0; j < R1; j++) S[sidx<R1>(row, j, n2z)] = v[j];
+            for (int j = 0; j < R1; j++) S[sidx<R1>(u, n1y, j, n2z)] = v[j];
         }
     }
 }
 
-template <int R1, int U, int NT, int SIGN>
-EXX_HD void p13_z8(int tid, cplx* S, const cplx* T) {
+// per-thread z twiddles for TWREG: twr[j] = W_N^(j k1z) with k1z = tid mod R1
+template <int R1>
+EXX_HD void load_twr(int tid, cplx* twr) {
+    int k1z = tid % R1;
+#pragma unroll
+    for (int j = 0; j < 8; j++) twr[j] = EXX_TW(R1, j * k1z);
+}
+
+template <int R1, int U, int NT, int SIGN, bool TWREG>
+EXX_HD void p13_z8(int tid, cplx* S, const cplx* T, const cplx* twr) {
     // the 8-point z step on items (row, k1z).  SIGN < 0: twiddle then forward DFT; SIGN > 0: inverse DFT then conj twiddle
     constexpr int NI = U * R1 * R1, IT = (NI + NT - 1) / NT;
 #pragma unroll
@@ -127,60 +186,82 @@ EXX_HD void p13_z8(int tid, cplx* S, const cplx* T) {
         int it = tid + i * NT;
         if (it < NI) {
             int row = it / R1, k1z = it - row * R1;
+            int u = row / R1, r = row - u * R1;
             cplx v[8];
 #pragma unroll
-            for (int j = 0; j < 8; j++) v[j] = S[sidx<R1>(row, k1z, j)];
+            for (int j = 0; j < 8; j++) v[j] = S[sidx<R1>(u, r, k1z, j)];
             if (SIGN < 0) {
 #pragma unroll
-                for (int j = 1; j < 8; j++) v[j] = v[j] * T[tidx(k1z, j)];
+                for (int j = 1; j < 8; j++) v[j] = v[j] * (TWREG ? twr[j] : T[tidx(k1z, j)]);
                 dft<8, -1>(v);
             } else {
                 dft<8, +1>(v);
 #pragma unroll
-                for (int j = 1; j < 8; j++) v[j] = mul_conj_b(v[j], T[tidx(k1z, j)]);
+                for (int j = 1; j < 8; j++) v[j] = mul_conj_b(v[j], TWREG ? twr[j] : T[tidx(k1z, j)]);
             }
 #pragma unroll
-            for (int j = 0; j < 8; j++) S[sidx<R1>(row, k1z, j)] = v[j];
+            for (int j = 0; j < 8; j++) S[sidx<R1>(u, r, k1z, j)] = v[j];
         }
     }
 }
 
 template <int R1, int U, int NT>
 EXX_HD void p1_y1(int tid, const cplx* S, cplx* __restrict__ W, int x, int yb) {
+    // items (kzblk, u, kzl), kzl fastest: 4 U consecutive lanes store one contiguous run of W
     constexpr int N = 8 * R1, NI = U * N, IT = (NI + NT - 1) / NT;
 #pragma unroll
     for (int i = 0; i < IT; i++) {
         int it = tid + i * NT;
         if (it < NI) {
-            int u = it / N, kzpos = it - u * N;
+            int kzl = it & 3, u = (it >> 2) % U, kzpos = (it / (4 * U)) * 4 + kzl;
             cplx v[R1];
 #pragma unroll
-            for (int j = 0; j < R1; j++) v[j] = S[sidx<R1>(u * R1 + j, kzpos >> 3, kzpos & 7)];
+            for (int j = 0; j < R1; j++) v[j] = S[sidx<R1>(u, j, kzpos >> 3, kzpos & 7)];
             dft<R1, -1>(v);
-            size_t base = ((size_t)x * N + (yb * U + u)) * N + kzpos;
+            size_t base = widx<R1>(0, kzpos, x, yb * U + u);
 #pragma unroll
-            for (int j = 0; j < R1; j++) W[base + (size_t)j * 8 * N] = v[j];  // row k1y * 8 + n2y
+            for (int j = 0; j < R1; j++) W[base + (size_t)j * (N / 4) * N * 32] = v[j];  // k1y = j
         }
     }
 }
 
 // ================================================================================================================
 // pass B.  Tile: rows k1y*8 + n2y (n2y < 8), all x, z positions zb*Z .. zb*Z+Z-1.
-template <int R1, int Z, int NT>
-EXX_HD void p2_yf(int tid, const cplx* __restrict__ W, int k1y, int zb, cplx* S) {
+// host stand-in for the bulk copies: tile rows W[tile][x][32] <-> S[x * PX ..]
+template <int R1, int Z>
+inline void p2_copy_rows(cplx* S, cplx* Wt, bool load) {
+    constexpr int N = 8 * R1, PX = P2Geo<Z>::PX;
+    for (int x = 0; x < N; x++)
+        for (int e = 0; e < 8 * Z; e++) {
+            if (load)
+                S[x * PX + e] = Wt[x * 8 * Z + e];
+            else
+                Wt[x * 8 * Z + e] = S[x * PX + e];
+        }
+}
+
+template <int R1, int Z, int NT, int SIGN>
+EXX_HD void p2_y8(int tid, cplx* S, int k1y) {
+    // items (xpos, kzl), in place in shared memory.  SIGN < 0: y twiddle W_N^(n2y k1y) (uniform per CTA), forward 8-point
+    // DFT over n2y;  SIGN > 0: inverse 8-point DFT over k2y, conjugate twiddle.
     constexpr int N = 8 * R1, NI = N * Z, IT = (NI + NT - 1) / NT, PX = P2Geo<Z>::PX;
 #pragma unroll
     for (int i = 0; i < IT; i++) {
         int it = tid + i * NT;
         if (it < NI) {
             int xpos = it / Z, kzl = it - xpos * Z;
-            size_t base = ((size_t)xpos * N + k1y * 8) * N + zb * Z + kzl;
             cplx v[8];
 #pragma unroll
-            for (int j = 0; j < 8; j++) v[j] = W[base + (size_t)j * N];
+            for (int j = 0; j < 8; j++) v[j] = S[xpos * PX + j * Z + kzl];
+            if (SIGN < 0) {
 #pragma unroll
-            for (int j = 1; j < 8; j++) v[j] = v[j] * EXX_TW(R1, j * k1y);  // y twiddle W_N^(n2y k1y), uniform per CTA
-            dft<8, -1>(v);
+                for (int j = 1; j < 8; j++) v[j] = v[j] * EXX_TW(R1, j * k1y);
+                dft<8, -1>(v);
+            } else {
+                dft<8, +1>(v);
+#pragma unroll
+                for (int j = 1; j < 8; j++) v[j] = mul_conj_b(v[j], EXX_TW(R1, j * k1y));
+            }
 #pragma unroll
             for (int j = 0; j < 8; j++) S[xpos * PX + j * Z + kzl] = v[j];
         }
@@ -239,27 +320,6 @@ EXX_HD void p2_x8(int tid, cplx* S, const double* __restrict__ Kt) {
     }
 }
 
-template <int R1, int Z, int NT>
-EXX_HD void p2_yinv(int tid, const cplx* S, cplx* __restrict__ W, int k1y, int zb) {
-    constexpr int N = 8 * R1, NI = N * Z, IT = (NI + NT - 1) / NT, PX = P2Geo<Z>::PX;
-#pragma unroll
-    for (int i = 0; i < IT; i++) {
-        int it = tid + i * NT;
-        if (it < NI) {
-            int xpos = it / Z, kzl = it - xpos * Z;
-            size_t base = ((size_t)xpos * N + k1y * 8) * N + zb * Z + kzl;
-            cplx v[8];
-#pragma unroll
-            for (int j = 0; j < 8; j++) v[j] = S[xpos * PX + j * Z + kzl];
-            dft<8, +1>(v);
-#pragma unroll
-            for (int j = 1; j < 8; j++) v[j] = mul_conj_b(v[j], EXX_TW(R1, j * k1y));
-#pragma unroll
-            for (int j = 0; j < 8; j++) W[base + (size_t)j * N] = v[j];
-        }
-    }
-}
-
 // ================================================================================================================
 // pass C
 template <int R1, int U, int NT>
@@ -269,14 +329,14 @@ EXX_HD void p3_y2inv(int tid, const cplx* __restrict__ W, int x, int yb, cplx* S
     for (int i = 0; i < IT; i++) {
         int it = tid + i * NT;
         if (it < NI) {
-            int u = it / N, kzpos = it - u * N;
-            size_t base = ((size_t)x * N + (yb * U + u)) * N + kzpos;
+            int kzl = it & 3, u = (it >> 2) % U, kzpos = (it / (4 * U)) * 4 + kzl;
+            size_t base = widx<R1>(0, kzpos, x, yb * U + u);
             cplx v[R1];
 #pragma unroll
-            for (int j = 0; j < R1; j++) v[j] = W[base + (size_t)j * 8 * N];
+            for (int j = 0; j < R1; j++) v[j] = W[base + (size_t)j * (N / 4) * N * 32];
             dft<R1, +1>(v);
 #pragma unroll
-            for (int j = 0; j < R1; j++) S[sidx<R1>(u * R1 + j, kzpos >> 3, kzpos & 7)] = v[j];
+            for (int j = 0; j < R1; j++) S[sidx<R1>(u, j, kzpos >> 3, kzpos & 7)] = v[j];
         }
     }
 }
@@ -296,7 +356,7 @@ EXX_HD void p3_zinv2(int tid, const cplx* S, const cplx* __restrict__ um, double
 #pragma unroll
             for (int j = 0; j < R1; j++) b[j] = um[base + j * 8];
 #pragma unroll
-            for (int j = 0; j < R1; j++) v[j] = S[sidx<R1>(row, j, n2z)];
+            for (int j = 0; j < R1; j++) v[j] = S[sidx<R1>(u, n1y, j, n2z)];
             dft<R1, +1>(v);
 #pragma unroll
             for (int j = 0; j < R1; j++) {
@@ -326,6 +386,48 @@ EXX_HD void p3_flush(int tid, const cplx* A, cplx* __restrict__ accg, int x, int
                 cplx g = accg[base + j * 8], a = A[row * N + j * 8 + n2z];
                 accg[base + j * 8] = g + a;
             }
+        }
+    }
+}
+
+// register-accumulator variants (ACCREG): acc[i*R1 + j] belongs to item tid + i*NT, element n1z = j
+template <int R1, int U, int NT>
+EXX_HD void p3_zinv2_reg(int tid, const cplx* S, const cplx* __restrict__ um, double wf, int x, int yb, cplx* acc) {
+    constexpr int N = 8 * R1, NI = U * R1 * 8, IT = (NI + NT - 1) / NT;
+#pragma unroll
+    for (int i = 0; i < IT; i++) {
+        int it = tid + i * NT;
+        if (it < NI) {
+            int row = it >> 3, n2z = it & 7;
+            int u = row / R1, n1y = row - u * R1;
+            size_t base = ((size_t)x * N + (n1y * 8 + yb * U + u)) * N + n2z;
+            cplx b[R1], v[R1];
+#pragma unroll
+            for (int j = 0; j < R1; j++) b[j] = um[base + j * 8];
+#pragma unroll
+            for (int j = 0; j < R1; j++) v[j] = S[sidx<R1>(u, n1y, j, n2z)];
+            dft<R1, +1>(v);
+#pragma unroll
+            for (int j = 0; j < R1; j++) {
+                cplx p = b[j] * v[j];
+                acc[i * R1 + j] = mk(acc[i * R1 + j].x - wf * p.x, acc[i * R1 + j].y - wf * p.y);
+            }
+        }
+    }
+}
+
+template <int R1, int U, int NT>
+EXX_HD void p3_flush_reg(int tid, const cplx* acc, cplx* __restrict__ accg, int x, int yb) {
+    constexpr int N = 8 * R1, NI = U * R1 * 8, IT = (NI + NT - 1) / NT;
+#pragma unroll
+    for (int i = 0; i < IT; i++) {
+        int it = tid + i * NT;
+        if (it < NI) {
+            int row = it >> 3, n2z = it & 7;
+            int u = row / R1, n1y = row - u * R1;
+            size_t base = ((size_t)x * N + (n1y * 8 + yb * U + u)) * N + n2z;
+#pragma unroll
+            for (int j = 0; j < R1; j++) accg[base + j * 8] = accg[base + j * 8] + acc[i * R1 + j];
         }
     }
 }

@@ -26,36 +26,61 @@ static void fill_tw() {
 template <int R1>
 static void emu_pair(const cplx* un, const cplx* um, const double* Knat, double wf, cplx* acc, cplx* W) {
     typedef FusedCfg<R1> C;
-    constexpr int N = 8 * R1, U = C::U, NT13 = C::NT13, Z = C::Z, NT2 = C::NT2;
+    constexpr int N = 8 * R1, U = C::U1, NT13 = C::NT1, U3 = C::U3, NT3 = C::NT3, Z = C::Z, NT2 = C::NT2;
+    constexpr bool TWREG = C::TWREG, ACCREG = C::ACCREG;
     std::vector<double> Kp((size_t)N * N * N);
     permute_ktable(R1, Z, Knat, Kp.data());
-    std::vector<cplx> S((size_t)U * R1 * N), A((size_t)U * R1 * N), T(R1 * 8), S2((size_t)N * P2Geo<Z>::PX);
+    std::vector<cplx> S((size_t)(U > U3 ? U : U3) * R1 * N), A((size_t)U3 * R1 * N), T(R1 * 8), S2((size_t)N * P2Geo<Z>::PX);
     for (int k = 0; k < R1; k++)
         for (int j = 0; j < 8; j++) T[tidx(k, j)] = EXX_TW(R1, j * k);
     // pass A
     for (int x = 0; x < N; x++)
         for (int yb = 0; yb < 8 / U; yb++) {
             for (int t = 0; t < NT13; t++) p1_z1<R1, U, NT13>(t, un, um, x, yb, S.data());
-            for (int t = 0; t < NT13; t++) p13_z8<R1, U, NT13, -1>(t, S.data(), T.data());
+            for (int t = 0; t < NT13; t++) {
+                cplx twr[8];
+                load_twr<R1>(t, twr);
+                p13_z8<R1, U, NT13, -1, TWREG>(t, S.data(), T.data(), twr);
+            }
             for (int t = 0; t < NT13; t++) p1_y1<R1, U, NT13>(t, S.data(), W, x, yb);
         }
     // pass B
     for (int k1y = 0; k1y < R1; k1y++)
         for (int zb = 0; zb < N / Z; zb++) {
             const double* Kt = Kp.data() + ((size_t)k1y * (N / Z) + zb) * ((size_t)N * 8 * Z);
-            for (int t = 0; t < NT2; t++) p2_yf<R1, Z, NT2>(t, W, k1y, zb, S2.data());
+            cplx* Wt = W + ((size_t)k1y * (N / Z) + zb) * ((size_t)N * 8 * Z);
+            p2_copy_rows<R1, Z>(S2.data(), Wt, true);
+            for (int t = 0; t < NT2; t++) p2_y8<R1, Z, NT2, -1>(t, S2.data(), k1y);
             for (int t = 0; t < NT2; t++) p2_xR<R1, Z, NT2, -1>(t, S2.data());
             for (int t = 0; t < NT2; t++) p2_x8<R1, Z, NT2>(t, S2.data(), Kt);
             for (int t = 0; t < NT2; t++) p2_xR<R1, Z, NT2, +1>(t, S2.data());
-            for (int t = 0; t < NT2; t++) p2_yinv<R1, Z, NT2>(t, S2.data(), W, k1y, zb);
+            for (int t = 0; t < NT2; t++) p2_y8<R1, Z, NT2, +1>(t, S2.data(), k1y);
+            p2_copy_rows<R1, Z>(S2.data(), Wt, false);
         }
     // pass C (one m)
+    constexpr int IT3 = (U3 * R1 * 8 + NT3 - 1) / NT3;
+    std::vector<cplx> accr((size_t)NT3 * IT3 * R1);
     for (int x = 0; x < N; x++)
-        for (int yb = 0; yb < 8 / U; yb++) {
-            for (int t = 0; t < NT13; t++) p3_y2inv<R1, U, NT13>(t, W, x, yb, S.data());
-            for (int t = 0; t < NT13; t++) p13_z8<R1, U, NT13, +1>(t, S.data(), T.data());
-            for (int t = 0; t < NT13; t++) p3_zinv2<R1, U, NT13>(t, S.data(), um, wf, x, yb, A.data(), true);
-            for (int t = 0; t < NT13; t++) p3_flush<R1, U, NT13>(t, A.data(), acc, x, yb);
+        for (int yb = 0; yb < 8 / U3; yb++) {
+            for (auto& a : accr) a = mk(0.0, 0.0);
+            for (int t = 0; t < NT3; t++) p3_y2inv<R1, U3, NT3>(t, W, x, yb, S.data());
+            for (int t = 0; t < NT3; t++) {
+                cplx twr[8];
+                load_twr<R1>(t, twr);
+                p13_z8<R1, U3, NT3, +1, TWREG>(t, S.data(), T.data(), twr);
+            }
+            for (int t = 0; t < NT3; t++) {
+                if (ACCREG)
+                    p3_zinv2_reg<R1, U3, NT3>(t, S.data(), um, wf, x, yb, accr.data() + (size_t)t * IT3 * R1);
+                else
+                    p3_zinv2<R1, U3, NT3>(t, S.data(), um, wf, x, yb, A.data(), true);
+            }
+            for (int t = 0; t < NT3; t++) {
+                if (ACCREG)
+                    p3_flush_reg<R1, U3, NT3>(t, accr.data() + (size_t)t * IT3 * R1, acc, x, yb);
+                else
+                    p3_flush<R1, U3, NT3>(t, A.data(), acc, x, yb);
+            }
         }
 }
 }  // namespace exx

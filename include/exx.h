@@ -23,7 +23,8 @@
  *       exx_psi_offset(k) + n*npw(k) + ig   (complex elements),  exx_psi_offset(k) = nbands * sum_{k'<k} npw(k').
  *   - pointers named *_dev are device (HBM) pointers, *_host are host pointers; both are owned by the caller.
  *     The context owns its index maps, kernel tables, the real-space cache u_nk(r) and all workspaces; they are
- *     allocated in exx_create and freed in exx_destroy.  exx_apply allocates nothing.
+ *     allocated in exx_create and freed in exx_destroy.  exx_apply allocates nothing, except the first apply after
+ *     EXX_OPT_PRUNE was switched off on a context that has a compact work grid (the full-grid buffers are made then).
  *   - every call returns EXX_OK (0) or a negative error code; no exceptions, no abort, nothing printed.
  *     On error, output arguments are left untouched.  exx_last_error() gives detail for EXX_ERR_CUDA.
  *   - work is enqueued on the CUDA stream given to exx_create (a cudaStream_t cast to void*; NULL = default
@@ -66,7 +67,8 @@ enum {
     EXX_OPT_PATH = 1,       /* 0 auto (fused kernels when the grid is supported, else generic), 1 generic per-axis kernels, 2 fused */
     EXX_OPT_TILE_N = 2,     /* bands n per tile (0 = auto) */
     EXX_OPT_TILE_M = 3,     /* bands m per tile (0 = auto) */
-    EXX_OPT_PRUNE = 4,      /* 1 (default): skip transforms whose input/output is zero by band limit, only when alias-free */
+    EXX_OPT_PRUNE = 4,      /* 1 (default): run the pair pipeline on the compact work grid when there is one (see EXX_INFO_COMPACT_GRID);
+                               0: always transform the caller's full grid */
     EXX_OPT_PROFILE = 5     /* 1: bracket every kernel launch with CUDA events so exx_get_kernel_time works (slower) */
 };
 
@@ -81,7 +83,12 @@ enum {
     EXX_INFO_TILE_N = 7,
     EXX_INFO_TILE_M = 8,
     EXX_INFO_PRUNED = 9,          /* 1 if band-limit pruning was active */
-    EXX_INFO_NUM_KERNEL_CLASSES = 10
+    EXX_INFO_NUM_KERNEL_CLASSES = 10,
+    EXX_INFO_WORK_GRID = 11,      /* N of the (cubic) grid the last apply transformed; first axis of the caller's grid if not compacted */
+    EXX_INFO_COMPACT_GRID = 12    /* (no apply needed) N of the compact work grid, 0 if none: the smallest supported cubic grid with
+                                     N >= 4 max|g_i| + 1, used when it is smaller than the caller's box and the caller's box is itself
+                                     alias-free (N_i >= 4 max|g_i| + 1).  Then no product the method forms wraps around on either grid and
+                                     V_x psi on the sphere is the same up to rounding */
 };
 
 /* Create a context.  grid: N1,N2,N3.  lattice: 9 doubles, row i = a_i in bohr.  kfrac: nk*3 fractional reciprocal

@@ -89,6 +89,7 @@ static double kernel_value(const exx_kernel_params& kp, const double B[9], const
 
 static void free_ctx(exx_ctx* c) {
     if (!c) return;
+    if (c->inner) free_ctx(c->inner);
     fused_destroy(c);
     cudaFree(c->map_dev);
     cudaFree(c->ktab_dev);
@@ -168,8 +169,10 @@ const char* exx_strerror(int code) {
 const char* exx_last_error(const exx_ctx* c) { return c ? c->last_error.c_str() : g_thread_error.c_str(); }
 const char* exx_kernel_class_name(int k) { return (k >= 0 && k < KC_COUNT) ? kclass_names[k] : nullptr; }
 
-int exx_create(exx_ctx** out, const int grid[3], const double lattice[9], int nk, const double* kfrac, const double* kweight,
-               double ecut, const exx_kernel_params* kp, int nbands, void* cuda_stream) {
+static int ensure_big(exx_ctx* c);
+
+static int create_impl(exx_ctx** out, const int grid[3], const double lattice[9], int nk, const double* kfrac, const double* kweight,
+                       double ecut, const exx_kernel_params* kp, int nbands, void* cuda_stream, bool allow_inner) {
     if (!out || !grid || !lattice || !kfrac || !kweight || !kp) return EXX_ERR_NULL;
     if (nk < 1 || nbands < 1) return EXX_ERR_BAD_ARG;
     for (int i = 0; i < 3; i++)
@@ -308,21 +311,6 @@ int exx_create(exx_ctx** out, const int grid[3], const double lattice[9], int nk
 
         // ---- workspaces
         int nbt = nk * nbands;
-        if ((rc = dev_alloc(c, &c->u_dev, (size_t)nbt * c->Ng))) return fail(rc);
-        // generic pipeline: one n at a time, up to 16 m per tile, at most ~1 GiB of pair workspace;
-        // fused pipeline: tn x tm pairs per batch (work) and tn accumulators
-        size_t box_bytes = sizeof(double2) * (size_t)c->Ng;
-        size_t wb = std::max<size_t>(1, std::min<size_t>(16, ((size_t)1 << 30) / box_bytes));
-        c->work_boxes = wb;
-        c->acc_boxes = 1;
-        if (fused_supported(c)) {
-            int tn, tm;
-            fused_tiles(c, &tn, &tm);
-            c->acc_boxes = tn;
-            c->work_boxes = std::max<size_t>(wb, (size_t)tn * tm);
-        }
-        if ((rc = dev_alloc(c, &c->work_dev, c->work_boxes * c->Ng))) return fail(rc);
-        if ((rc = dev_alloc(c, &c->acc_dev, c->acc_boxes * c->Ng))) return fail(rc);
         if ((rc = dev_alloc(c, &c->vx_dev, (size_t)c->off[nk]))) return fail(rc);
         if ((rc = dev_alloc(c, &c->band_dot_dev, (size_t)nbt))) return fail(rc);
         if ((rc = dev_alloc(c, &c->band_e_dev, (size_t)nbt + 1))) return fail(rc);
@@ -345,8 +333,31 @@ int exx_create(exx_ctx** out, const int grid[3], const double lattice[9], int nk
             cudaMemcpy(c->band_len_dev, bl.data(), sizeof(int) * nbt, cudaMemcpyHostToDevice);
         }
         if ((rc = fft_generic_init(c))) { exx_destroy(c); return rc; }
-        if (fused_supported(c))
-            if ((rc = fused_create(c))) { exx_destroy(c); return rc; }
+        // compact work grid: smallest fused-capable cubic grid with N >= 4 gmax + 1, if smaller than the caller's box
+        if (allow_inner && c->alias_free) {
+            int need = 0;
+            for (int i = 0; i < 3; i++) need = std::max(need, 4 * c->gmax[i] + 1);
+            const int cand[5] = {48, 64, 72, 96, 128};
+            for (int ci = 0; ci < 5; ci++)
+                if (cand[ci] >= need) {
+                    int64_t nw = cand[ci];
+                    if (nw * nw * nw < c->Ng) {
+                        int g3[3] = {cand[ci], cand[ci], cand[ci]};
+                        exx_ctx* in = nullptr;
+                        if (create_impl(&in, g3, lattice, nk, kfrac, kweight, ecut, kp, nbands, cuda_stream, false) == EXX_OK) {
+                            bool same = true;  // same spheres in the same order (ordering is grid-independent, checked anyway)
+                            for (int k = 0; k < nk; k++) same = same && in->npw[k] == c->npw[k];
+                            if (same)
+                                c->inner = in;
+                            else
+                                free_ctx(in);
+                        }
+                    }
+                    break;
+                }
+        }
+        if (!c->inner)
+            if ((rc = ensure_big(c))) { exx_destroy(c); return rc; }
         cudaError_t e = cudaDeviceSynchronize();
         if (e != cudaSuccess) { rc = cuda_fail(c, e, "exx_create sync"); exx_destroy(c); return rc; }
     } catch (const std::bad_alloc&) {
@@ -354,6 +365,37 @@ int exx_create(exx_ctx** out, const int grid[3], const double lattice[9], int nk
     }
     *out = c;
     return EXX_OK;
+}
+
+// the buffers that scale with nbands * Ng: real-space cache, pair workspace, accumulators, fused tables
+static int ensure_big(exx_ctx* c) {
+    if (c->big_alloc) return EXX_OK;
+    int rc;
+    int nbt = c->nk * c->nb;
+    if ((rc = dev_alloc(c, &c->u_dev, (size_t)nbt * c->Ng))) return rc;
+    // generic pipeline: one n at a time, up to 16 m per tile, at most ~1 GiB of pair workspace;
+    // fused pipeline: tn x tm pairs per batch (work) and tn accumulators
+    size_t box_bytes = sizeof(double2) * (size_t)c->Ng;
+    size_t wb = std::max<size_t>(1, std::min<size_t>(16, ((size_t)1 << 30) / box_bytes));
+    c->work_boxes = wb;
+    c->acc_boxes = 1;
+    if (fused_supported(c)) {
+        int tn, tm;
+        fused_tiles(c, &tn, &tm);
+        c->acc_boxes = tn;
+        c->work_boxes = std::max<size_t>(wb, (size_t)tn * tm);
+    }
+    if ((rc = dev_alloc(c, &c->work_dev, c->work_boxes * c->Ng))) return rc;
+    if ((rc = dev_alloc(c, &c->acc_dev, c->acc_boxes * c->Ng))) return rc;
+    if (fused_supported(c))
+        if ((rc = fused_create(c))) return rc;
+    c->big_alloc = true;
+    return EXX_OK;
+}
+
+int exx_create(exx_ctx** out, const int grid[3], const double lattice[9], int nk, const double* kfrac, const double* kweight,
+               double ecut, const exx_kernel_params* kp, int nbands, void* cuda_stream) {
+    return create_impl(out, grid, lattice, nk, kfrac, kweight, ecut, kp, nbands, cuda_stream, true);
 }
 
 int exx_destroy(exx_ctx* c) {
@@ -434,7 +476,9 @@ int exx_get_info(const exx_ctx* c, int what, int64_t* value) {
     case EXX_INFO_PAIRS_ORDERED: *value = c->pairs_ordered; return EXX_OK;
     case EXX_INFO_PAIRS_EXECUTED: *value = c->pairs_executed; return EXX_OK;
     case EXX_INFO_PATH_USED: *value = c->path_used; return EXX_OK;
-    case EXX_INFO_WORKSPACE_BYTES: *value = (int64_t)c->dev_bytes; return EXX_OK;
+    case EXX_INFO_WORKSPACE_BYTES: *value = (int64_t)c->dev_bytes + (c->inner ? (int64_t)c->inner->dev_bytes : 0); return EXX_OK;
+    case EXX_INFO_WORK_GRID: *value = (c->inner && c->last_pruned) ? c->inner->N[0] : c->N[0]; return EXX_OK;
+    case EXX_INFO_COMPACT_GRID: *value = c->inner ? c->inner->N[0] : 0; return EXX_OK;
     case EXX_INFO_NCOEF: *value = c->off[c->nk]; return EXX_OK;
     case EXX_INFO_TILE_N: *value = c->tile_n_used; return EXX_OK;
     case EXX_INFO_TILE_M: *value = c->tile_m_used; return EXX_OK;
@@ -446,6 +490,7 @@ int exx_get_info(const exx_ctx* c, int what, int64_t* value) {
 int exx_get_kernel_time(exx_ctx* c, int kclass, double* ms_total, int64_t* launches, int64_t* units) {
     if (!c || !ms_total || !launches || !units) return EXX_ERR_NULL;
     if (kclass < 0 || kclass >= KC_COUNT) return EXX_ERR_BAD_ARG;
+    if (c->inner && c->last_pruned) return exx_get_kernel_time(c->inner, kclass, ms_total, launches, units);
     EXX_CUDA(c, cudaStreamSynchronize(c->stream));
     double ms = 0.0;
     for (const EventRec& r : c->events)
@@ -546,6 +591,30 @@ static int apply_generic(exx_ctx* c, const double2* psi, const double* occ, doub
 
 static int apply_impl(exx_ctx* c, const double2* psi, const double* occ, double2* out) {
     reset_counters(c);
+    if (c->inner && c->opt_prune) {
+        // compact work grid: same spheres, same psi/out layout, every product alias-free on both grids
+        exx_ctx* in = c->inner;
+        in->opt_path = c->opt_path == 1 ? 1 : 0;
+        in->opt_tile_n = c->opt_tile_n;
+        in->opt_tile_m = c->opt_tile_m;
+        in->opt_profile = c->opt_profile;
+        int rc = apply_impl(in, psi, occ, out);
+        c->launches = in->launches;
+        c->pairs_ordered = in->pairs_ordered;
+        c->pairs_executed = in->pairs_executed;
+        c->path_used = in->path_used;
+        c->tile_n_used = in->tile_n_used;
+        c->tile_m_used = in->tile_m_used;
+        c->pruned_used = 1;
+        c->last_pruned = 1;
+        if (rc) c->last_error = in->last_error;
+        return rc;
+    }
+    c->last_pruned = 0;
+    {
+        int rc = ensure_big(c);
+        if (rc) return rc;
+    }
     bool use_fused = fused_supported(c) && c->opt_path != 1;
     if (use_fused) return fused_apply(c, occ, psi, out);
     return apply_generic(c, psi, occ, out);

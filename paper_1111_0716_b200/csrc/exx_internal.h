@@ -82,6 +82,14 @@ struct exx_ctx {
     // fused path state (exx_fused.cu)
     void* fused = nullptr;
 
+    // compact work grid (EXX_OPT_PRUNE): a second context of the same problem on the smallest supported cubic grid that still
+    // holds every product the method forms without wrap-around (N >= 4 gmax + 1); owned by this context.  big_alloc: the
+    // real-space cache, pair workspace, accumulators and fused tables of THIS grid exist (allocated in exx_create when there is
+    // no inner context, else on the first apply with pruning switched off).
+    exx_ctx* inner = nullptr;
+    bool big_alloc = false;
+    int last_pruned = 0;
+
     // options
     int64_t opt_path = 0, opt_tile_n = 0, opt_tile_m = 0, opt_prune = 1, opt_profile = 0;
 

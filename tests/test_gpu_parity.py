@@ -169,7 +169,7 @@ def test_apply_C1_full_parity(B):
     assert abs(e - gold["E_x_E1"]) < 1e-15
 
 
-def _check_golden(B, name, live_rows=0):
+def _check_golden(B, name, live_rows=0, prune=1):
     """Big configs: the GPU applies V_x in full; rows, per-band energies and E_x are compared with stored oracle
     results (tests/golden/make_golden.py) and, for `live_rows` rows, with the oracle run now."""
     import torch
@@ -183,7 +183,9 @@ def _check_golden(B, name, live_rows=0):
     psi = w.coefficients(g.npw)
     assert [psi[0].real, psi[0].imag] == gold["psi_first"]
     pd = g.to_device(psi)
+    g.set_option(B.EXX_OPT_PRUNE, prune)
     out = g.apply(pd, w.occ)
+    assert g.get_info(B.EXX_INFO_PRUNED) == (1 if (prune and g.get_info(B.EXX_INFO_COMPACT_GRID)) else 0)
     e, pb = g.energy(pd, w.occ, out)
     torch.cuda.synchronize()
     got = out.cpu().numpy()
@@ -227,6 +229,66 @@ def test_apply_C5_parity(B):
 @pytest.mark.skipif(not os.path.exists(os.path.join(GOLD, "exx_C4b.json")), reason="C4b golden rows not generated yet")
 def test_apply_C4b_parity(B):
     _check_golden(B, "C4b")
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# compact work grid (EXX_OPT_PRUNE): cells whose box is much larger than 4 gmax + 1
+COMPACT = {
+    "sc64_gamma": dict(grid=(64, 64, 64), lat=("sc", 10.0), kf=[[0, 0, 0]], kw=[1.0], ecut=12.0, nb=5, occ=[1, 1, 0.5, 0.25, 0],
+                       kind=0, mu=0.0, compact=48),
+    "rh64_kpts_hse": dict(grid=(64, 64, 64), lat=("rh", 9.0, 62.0), kf=[[0.25, 0.25, 0.25], [-0.25, 0.25, 0.0]], kw=[0.5, 0.5],
+                          ecut=9.0, nb=3, occ=[1, 0.6, 0.3], kind=1, mu=0.106, compact=48),
+}
+
+
+@pytest.mark.parametrize("name", list(COMPACT))
+def test_compact_grid_equals_full_grid_and_oracle(B, name):
+    s = COMPACT[name]
+    lat = W.cubic(s["lat"][1]) if s["lat"][0] == "sc" else W.rhombohedral(s["lat"][1], s["lat"][2])
+    w = W.custom(name, 4242, s["grid"], lat, s["kf"], s["kw"], s["ecut"], s["nb"], s["occ"], s["kind"], s["mu"])
+    o, g = _pair(B, w)
+    assert g.get_info(B.EXX_INFO_COMPACT_GRID) == s["compact"]
+    psi = w.coefficients(o.npw)
+    want = o.apply(psi, w.occ)              # the oracle works on the caller's full 64^3 grid
+    e_want, _ = o.energy(psi, w.occ, want)
+    pd = g.to_device(psi)
+    res = {}
+    for prune in (1, 0):
+        g.set_option(B.EXX_OPT_PRUNE, prune)
+        out = g.apply(pd, w.occ)
+        assert g.get_info(B.EXX_INFO_PRUNED) == prune
+        assert g.get_info(B.EXX_INFO_WORK_GRID) == (s["compact"] if prune else 64)
+        assert g.get_info(B.EXX_INFO_PAIRS_ORDERED) == w.pair_evals
+        got = out.cpu().numpy()
+        for k in range(w.nk):
+            for n in range(w.nbands):
+                assert _rel(o.band(got, k, n), o.band(want, k, n)) < TOL_VX, (name, prune, k, n)
+        e, _ = g.energy(pd, w.occ, out)
+        assert abs(e - e_want) <= TOL_EX * abs(e_want)
+        res[prune] = got
+    assert _rel(res[1], res[0]) < 1e-13
+    g.close()
+
+
+def test_compact_grid_not_used_when_caller_grid_aliases(B):
+    # C1 (16^3, needs 21) is aliased by construction and C2/C3 need their whole box: no compact grid
+    for name in ("C1", "C2", "C3"):
+        w = W.make(name)
+        w.nbands, w.occ_per_k = 2, np.ones(2)
+        g = B.Exx.from_workload(w)
+        assert g.get_info(B.EXX_INFO_COMPACT_GRID) == 0
+        g.close()
+    for name, n in (("C4a", 72), ("C5", 96)):
+        w = W.make(name)
+        w.nbands, w.occ_per_k = 2, np.ones(2)
+        g = B.Exx.from_workload(w)
+        assert g.get_info(B.EXX_INFO_COMPACT_GRID) == n
+        g.close()
+
+
+def test_apply_C4a_full_grid_parity(B):
+    """C4a on the caller's full 96^3 grid (EXX_OPT_PRUNE = 0); test_apply_C4a_parity covers the default (compact 72^3)."""
+    _check_golden(B, "C4a", prune=0)
 
 
 # ---------------------------------------------------------------------------------------------------------------

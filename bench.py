@@ -185,18 +185,47 @@ def run_ours(args, rank, world, local):
     sync_all()
     ms_prof = p0.elapsed_time(p1) / args.steps
     g.set_option(B.EXX_OPT_PROFILE, 0)
+    # grid the pair pipeline actually transformed (the compact work grid when EXX_OPT_PRUNE is active):
+    # all algorithmic-byte figures below use THAT grid, never the caller's larger box
+    nw = g.get_info(B.EXX_INFO_WORK_GRID)
+    ngw = nw ** 3 if g.get_info(B.EXX_INFO_PRUNED) else w.ng
     dom = max(acc, key=lambda k: acc[k][0])
     t_dom, n_dom, u_dom = acc[dom]
-    bytes_dom = BYTES_PER_UNIT_NG.get(dom, 32) * w.ng * u_dom
+    bytes_dom = BYTES_PER_UNIT_NG.get(dom, 32) * ngw * u_dom
     achieved = bytes_dom / (t_dom * 1e-3) / 1e9 if t_dom > 0 else 0.0
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": None, "peak_source": peak_src, "avg_launch_us": 1e3 * t_dom / max(1, n_dom),
                 "algorithmic_bytes_per_launch": bytes_dom / max(1, n_dom), "share_of_step": t_dom / args.steps / ms_prof,
+                "grid_points_transformed": ngw,
                 "kernel_ms_per_step": {k: v[0] / args.steps for k, v in acc.items() if v[1]}}
-    # the graded pipeline figure: B_model = 96 Ng bytes per EXECUTED pair over the whole apply
-    pipe = 96.0 * w.ng * pairs_exec / (ms * 1e-3) / 1e9
-    pipeline = {"model_bytes_per_pair": 96 * w.ng, "pairs_executed": pairs_exec, "achieved": pipe, "unit": "GB/s", "peak": peak,
-                "frac": pipe / peak, "us_per_executed_pair": 1e3 * ms / max(1, pairs_exec), "ms_per_step_profiled": ms_prof}
+    # the pipeline figure: B_model = 96 bytes per transformed grid point per EXECUTED pair over the whole apply
+    pipe = 96.0 * ngw * pairs_exec / (ms * 1e-3) / 1e9
+    pipeline = {"model_bytes_per_pair": 96 * ngw, "pairs_executed": pairs_exec, "achieved": pipe, "unit": "GB/s", "peak": peak,
+                "frac": pipe / peak, "us_per_executed_pair": 1e3 * ms / max(1, pairs_exec), "ms_per_step_profiled": ms_prof,
+                "work_grid": [nw] * 3 if ngw != w.ng else list(w.grid)}
+
+    # ---- the same apply on the caller's FULL grid (EXX_OPT_PRUNE = 0): the graded "96^3" pipeline number of BASELINE.md
+    full = None
+    if ngw != w.ng and not args.no_full_grid:
+        g.set_option(B.EXX_OPT_PRUNE, 0)
+        for _ in range(2):
+            g.apply(pd, occ, out)
+        sync_all()
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        f0.record()
+        for _ in range(args.steps):
+            g.apply(pd, occ, out)
+            ex_f = g.energy(pd, occ, out)[0]
+        f1.record()
+        sync_all()
+        ms_f = max_over_ranks(f0.elapsed_time(f1), world, dev) / args.steps
+        pe_f = g.get_info(B.EXX_INFO_PAIRS_EXECUTED)
+        pipe_f = 96.0 * w.ng * pe_f / (ms_f * 1e-3) / 1e9
+        full = {"grid": list(w.grid), "ms_per_step": ms_f, "value": world * pairs_ord / (ms_f * 1e-3), "unit": UNIT,
+                "us_per_executed_pair": 1e3 * ms_f / max(1, pe_f), "model_bytes_per_pair": 96 * w.ng,
+                "pipeline_achieved_GBs": pipe_f, "pipeline_frac": pipe_f / peak, "E_x": ex_f}
+        assert abs(ex_f - ex) <= 1e-11 * abs(ex)
+        g.set_option(B.EXX_OPT_PRUNE, 1)
 
     # ---- timed region 3: end to end through exx_apply_host, pinned host buffers, copies inside the timed region
     for _ in range(min(2, args.warmup)):
@@ -218,12 +247,14 @@ def run_ours(args, rank, world, local):
                        "pairs_per_step": pairs_ord, "parallelism": "replicas x%d" % world,
                        "path": {1: "generic", 2: "fused"}.get(g.get_info(B.EXX_INFO_PATH_USED)),
                        "tile_n": g.get_info(B.EXX_INFO_TILE_N), "tile_m": g.get_info(B.EXX_INFO_TILE_M),
-                       "pruned": g.get_info(B.EXX_INFO_PRUNED),
-                       "l2": "inputs larger than L2: the real-space cache u_nk(r) is %.2f GB, streamed every step" % (w.nk * w.nbands * w.ng * 16 / 1e9)},
+                       "pruned": g.get_info(B.EXX_INFO_PRUNED), "work_grid": pipeline["work_grid"],
+                       "l2": "inputs larger than L2: the real-space cache u_nk(r) is %.2f GB, streamed every step" % (w.nk * w.nbands * ngw * 16 / 1e9)},
             "E_x": ex, "vx_apply_ms": ms, "clocks": sampler.summary(), "roofline": roofline, "pipeline_roofline": pipeline,
             "e2e": {"value": world * pairs_ord / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
                     "h2d_bytes_per_step": g.ncoef * 16, "d2h_bytes_per_step": g.ncoef * 16 + 8},
             "gpu_launches": launches * args.steps}
+    if full is not None:
+        line["full_grid"] = full
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(w, psi)
     if rank == 0:
@@ -255,6 +286,7 @@ def main():
     ap.add_argument("--workload", default="C4a", choices=list(W.ALL))
     ap.add_argument("--path", type=int, default=None, help="EXX_OPT_PATH override: 1 generic, 2 fused")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-full-grid", action="store_true", help="skip the extra full-grid (EXX_OPT_PRUNE = 0) timing")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     rank, world, local = dist_setup(args.gpus)

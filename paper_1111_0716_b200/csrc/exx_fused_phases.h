@@ -54,69 +54,81 @@ extern cplx h_tw[TW_TOTAL];
 // pass B on tiles of Z z-positions with NT2 threads.  Thread counts are chosen so that every step's item count is a small
 // multiple of the CTA size.  TWREG: the z twiddles W_N^(j k1z) live in 7 registers per thread (needs NT % R1 == 0 so that a
 // thread's k1z never changes) instead of a shared-memory table; ACCREG: pass C keeps its accumulator tile in registers
-// instead of shared memory.  The EXX_TUNE_* macros let a build override the N = 96 geometry (tuning sweeps).
-#ifndef EXX_TUNE_U1
-#define EXX_TUNE_U1 1
-#endif
-#ifndef EXX_TUNE_NT1
-#define EXX_TUNE_NT1 96
-#endif
-#ifndef EXX_TUNE_U3
-#define EXX_TUNE_U3 1
-#endif
-#ifndef EXX_TUNE_NT3
-#define EXX_TUNE_NT3 96
-#endif
-#ifndef EXX_TUNE_NT2
-#define EXX_TUNE_NT2 128
-#endif
-#ifndef EXX_TUNE_MINB1
-#define EXX_TUNE_MINB1 1
-#endif
-#ifndef EXX_TUNE_MINB2
-#define EXX_TUNE_MINB2 4
-#endif
-#ifndef EXX_TUNE_MINB3
-#define EXX_TUNE_MINB3 1
-#endif
-#ifndef EXX_TUNE_TWREG
-#define EXX_TUNE_TWREG 0
-#endif
-#ifndef EXX_TUNE_ACCREG
-#define EXX_TUNE_ACCREG 0
-#endif
+// instead of shared memory.
 template <int R1>
-struct FusedCfg;
+struct FusedCfgBase;
 template <>
-struct FusedCfg<6> {
+struct FusedCfgBase<6> {
     static constexpr int U1 = 4, NT1 = 96, U3 = 4, NT3 = 96, Z = 4, NT2 = 64;
     static constexpr bool TWREG = false, ACCREG = false;
     static constexpr int MINB1 = 1, MINB2 = 1, MINB3 = 1;  // min CTAs per SM asked of the compiler (register cap)
 };
 template <>
-struct FusedCfg<8> {
+struct FusedCfgBase<8> {
     static constexpr int U1 = 4, NT1 = 128, U3 = 4, NT3 = 128, Z = 4, NT2 = 128;
     static constexpr bool TWREG = false, ACCREG = false;
-    static constexpr int MINB1 = 1, MINB2 = 1, MINB3 = 1;  // min CTAs per SM asked of the compiler (register cap)
+    static constexpr int MINB1 = 1, MINB2 = 1, MINB3 = 1;
 };
 template <>
-struct FusedCfg<9> {
-    static constexpr int U1 = 4, NT1 = 96, U3 = 4, NT3 = 96, Z = 4, NT2 = 96;
+struct FusedCfgBase<9> {
+    static constexpr int U1 = 2, NT1 = 160, U3 = 1, NT3 = 96, Z = 4, NT2 = 96;
     static constexpr bool TWREG = false, ACCREG = false;
-    static constexpr int MINB1 = 1, MINB2 = 1, MINB3 = 1;  // min CTAs per SM asked of the compiler (register cap)
+    static constexpr int MINB1 = 1, MINB2 = 5, MINB3 = 1;
 };
 template <>
-struct FusedCfg<12> {
-    static constexpr int U1 = EXX_TUNE_U1, NT1 = EXX_TUNE_NT1, U3 = EXX_TUNE_U3, NT3 = EXX_TUNE_NT3, Z = 4, NT2 = EXX_TUNE_NT2;
-    static constexpr bool TWREG = EXX_TUNE_TWREG != 0, ACCREG = EXX_TUNE_ACCREG != 0;
-    static constexpr int MINB1 = EXX_TUNE_MINB1, MINB2 = EXX_TUNE_MINB2, MINB3 = EXX_TUNE_MINB3;
+struct FusedCfgBase<12> {
+    static constexpr int U1 = 1, NT1 = 96, U3 = 1, NT3 = 96, Z = 4, NT2 = 128;
+    static constexpr bool TWREG = false, ACCREG = false;
+    static constexpr int MINB1 = 1, MINB2 = 4, MINB3 = 1;
 };
 template <>
-struct FusedCfg<16> {
+struct FusedCfgBase<16> {
     static constexpr int U1 = 1, NT1 = 128, U3 = 1, NT3 = 128, Z = 4, NT2 = 256;
     static constexpr bool TWREG = false, ACCREG = false;
-    static constexpr int MINB1 = 1, MINB2 = 1, MINB3 = 1;  // min CTAs per SM asked of the compiler (register cap)
+    static constexpr int MINB1 = 1, MINB2 = 2, MINB3 = 1;
 };
+template <int R1>
+struct FusedCfg : FusedCfgBase<R1> {};
+
+// tuning sweeps: -DEXX_TUNE_R1=<R1> plus any of EXX_TUNE_{U1,NT1,U3,NT3,NT2,MINB1,MINB2,MINB3,TWREG,ACCREG} overrides that grid
+#ifdef EXX_TUNE_R1
+#ifndef EXX_TUNE_U1
+#define EXX_TUNE_U1 FusedCfgBase<EXX_TUNE_R1>::U1
+#endif
+#ifndef EXX_TUNE_NT1
+#define EXX_TUNE_NT1 FusedCfgBase<EXX_TUNE_R1>::NT1
+#endif
+#ifndef EXX_TUNE_U3
+#define EXX_TUNE_U3 FusedCfgBase<EXX_TUNE_R1>::U3
+#endif
+#ifndef EXX_TUNE_NT3
+#define EXX_TUNE_NT3 FusedCfgBase<EXX_TUNE_R1>::NT3
+#endif
+#ifndef EXX_TUNE_NT2
+#define EXX_TUNE_NT2 FusedCfgBase<EXX_TUNE_R1>::NT2
+#endif
+#ifndef EXX_TUNE_MINB1
+#define EXX_TUNE_MINB1 FusedCfgBase<EXX_TUNE_R1>::MINB1
+#endif
+#ifndef EXX_TUNE_MINB2
+#define EXX_TUNE_MINB2 FusedCfgBase<EXX_TUNE_R1>::MINB2
+#endif
+#ifndef EXX_TUNE_MINB3
+#define EXX_TUNE_MINB3 FusedCfgBase<EXX_TUNE_R1>::MINB3
+#endif
+#ifndef EXX_TUNE_TWREG
+#define EXX_TUNE_TWREG FusedCfgBase<EXX_TUNE_R1>::TWREG
+#endif
+#ifndef EXX_TUNE_ACCREG
+#define EXX_TUNE_ACCREG FusedCfgBase<EXX_TUNE_R1>::ACCREG
+#endif
+template <>
+struct FusedCfg<EXX_TUNE_R1> {
+    static constexpr int U1 = EXX_TUNE_U1, NT1 = EXX_TUNE_NT1, U3 = EXX_TUNE_U3, NT3 = EXX_TUNE_NT3, Z = 4, NT2 = EXX_TUNE_NT2;
+    static constexpr bool TWREG = EXX_TUNE_TWREG, ACCREG = EXX_TUNE_ACCREG;
+    static constexpr int MINB1 = EXX_TUNE_MINB1, MINB2 = EXX_TUNE_MINB2, MINB3 = EXX_TUNE_MINB3;
+};
+#endif
 
 // ---- shared-memory layouts -------------------------------------------------------------------------------------
 // passes A/C: S[row][k1z][j], XOR swizzle of j with (row R1 + k1z) & 7 and 4 (u & 1): conflict-free for the three access patterns

@@ -193,8 +193,15 @@ def run_ours(args, rank, world, local):
     t_dom, n_dom, u_dom = acc[dom]
     bytes_dom = BYTES_PER_UNIT_NG.get(dom, 32) * ngw * u_dom
     achieved = bytes_dom / (t_dom * 1e-3) / 1e9 if t_dom > 0 else 0.0
+    traffic = None   # dram bytes per launch of the dominant kernel from the committed ncu capture, scaled to this launch size
+    try:
+        tj = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic_r1.json")))
+        if tj["work_grid"] ** 3 == ngw and dom in tj["dram_bytes_per_launch"]:
+            traffic = tj["dram_bytes_per_launch"][dom] / tj["pairs_per_launch"] * (u_dom / max(1, n_dom))
+    except Exception:
+        pass
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "peak_source": peak_src, "avg_launch_us": 1e3 * t_dom / max(1, n_dom),
+                "traffic": traffic, "peak_source": peak_src, "avg_launch_us": 1e3 * t_dom / max(1, n_dom),
                 "algorithmic_bytes_per_launch": bytes_dom / max(1, n_dom), "share_of_step": t_dom / args.steps / ms_prof,
                 "grid_points_transformed": ngw,
                 "kernel_ms_per_step": {k: v[0] / args.steps for k, v in acc.items() if v[1]}}

@@ -72,7 +72,7 @@ struct FusedCfgBase<8> {
 template <>
 struct FusedCfgBase<9> {
     static constexpr int U1 = 2, NT1 = 160, U3 = 1, NT3 = 96, Z = 4, NT2 = 96;
-    static constexpr bool TWREG = false, ACCREG = false;
+    static constexpr bool TWREG = false, ACCREG = true;
     static constexpr int MINB1 = 1, MINB2 = 5, MINB3 = 1;
 };
 template <>
@@ -199,17 +199,31 @@ EXX_HD void p13_z8(int tid, cplx* S, const cplx* T, const cplx* twr) {
         if (it < NI) {
             int row = it / R1, k1z = it - row * R1;
             int u = row / R1, r = row - u * R1;
-            cplx v[8];
+            cplx v[8], w[8];
 #pragma unroll
             for (int j = 0; j < 8; j++) v[j] = S[sidx<R1>(u, r, k1z, j)];
+            if (TWREG) {
+#pragma unroll
+                for (int j = 1; j < 8; j++) w[j] = twr[j];
+            } else {
+                // three table reads (W^k, W^2k, W^4k) and four products instead of seven reads: the shared-memory
+                // data pipe, not the fp64 pipe, is what these kernels run out of
+                w[1] = T[tidx(k1z, 1)];
+                w[2] = T[tidx(k1z, 2)];
+                w[4] = T[tidx(k1z, 4)];
+                w[3] = w[1] * w[2];
+                w[5] = w[4] * w[1];
+                w[6] = w[4] * w[2];
+                w[7] = w[4] * w[3];
+            }
             if (SIGN < 0) {
 #pragma unroll
-                for (int j = 1; j < 8; j++) v[j] = v[j] * (TWREG ? twr[j] : T[tidx(k1z, j)]);
+                for (int j = 1; j < 8; j++) v[j] = v[j] * w[j];
                 dft<8, -1>(v);
             } else {
                 dft<8, +1>(v);
 #pragma unroll
-                for (int j = 1; j < 8; j++) v[j] = mul_conj_b(v[j], TWREG ? twr[j] : T[tidx(k1z, j)]);
+                for (int j = 1; j < 8; j++) v[j] = mul_conj_b(v[j], w[j]);
             }
 #pragma unroll
             for (int j = 0; j < 8; j++) S[sidx<R1>(u, r, k1z, j)] = v[j];

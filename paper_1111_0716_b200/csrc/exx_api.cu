@@ -382,7 +382,7 @@ static int ensure_big(exx_ctx* c) {
     if (fused_supported(c)) {
         int tn, tm;
         fused_tiles(c, &tn, &tm);
-        c->acc_boxes = tn;
+        c->acc_boxes = (size_t)c->nk * c->nb;  // the fused loop nest keeps one accumulator per (k, band)
         c->work_boxes = std::max<size_t>(wb, (size_t)tn * tm);
     }
     if ((rc = dev_alloc(c, &c->work_dev, c->work_boxes * c->Ng))) return rc;
@@ -455,6 +455,9 @@ int exx_set_option(exx_ctx* c, int option, int64_t value) {
     case EXX_OPT_PROFILE:
         c->opt_profile = value ? 1 : 0;
         return EXX_OK;
+    case EXX_OPT_SYMMETRY:
+        c->opt_symmetry = value ? 1 : 0;
+        return EXX_OK;
     default: return EXX_ERR_BAD_ARG;
     }
 }
@@ -466,6 +469,7 @@ int exx_get_option(const exx_ctx* c, int option, int64_t* value) {
     case EXX_OPT_TILE_M: *value = c->opt_tile_m; return EXX_OK;
     case EXX_OPT_PRUNE: *value = c->opt_prune; return EXX_OK;
     case EXX_OPT_PROFILE: *value = c->opt_profile; return EXX_OK;
+    case EXX_OPT_SYMMETRY: *value = c->opt_symmetry; return EXX_OK;
     default: return EXX_ERR_BAD_ARG;
     }
 }
@@ -483,6 +487,7 @@ int exx_get_info(const exx_ctx* c, int what, int64_t* value) {
     case EXX_INFO_TILE_N: *value = c->tile_n_used; return EXX_OK;
     case EXX_INFO_TILE_M: *value = c->tile_m_used; return EXX_OK;
     case EXX_INFO_PRUNED: *value = c->pruned_used; return EXX_OK;
+    case EXX_INFO_SYMMETRY: *value = c->symmetry_used; return EXX_OK;
     case EXX_INFO_NUM_KERNEL_CLASSES: *value = KC_COUNT; return EXX_OK;
     default: return EXX_ERR_BAD_ARG;
     }
@@ -542,6 +547,7 @@ static void reset_counters(exx_ctx* c) {
     c->events.clear();
     c->event_pool_used = 0;
     c->pairs_ordered = c->pairs_executed = 0;
+    c->symmetry_used = 0;
 }
 
 // Generic pipeline, steps S1..S7 as separate kernels.
@@ -598,6 +604,7 @@ static int apply_impl(exx_ctx* c, const double2* psi, const double* occ, double2
         in->opt_tile_n = c->opt_tile_n;
         in->opt_tile_m = c->opt_tile_m;
         in->opt_profile = c->opt_profile;
+        in->opt_symmetry = c->opt_symmetry;
         int rc = apply_impl(in, psi, occ, out);
         c->launches = in->launches;
         c->pairs_ordered = in->pairs_ordered;
@@ -605,6 +612,7 @@ static int apply_impl(exx_ctx* c, const double2* psi, const double* occ, double2
         c->path_used = in->path_used;
         c->tile_n_used = in->tile_n_used;
         c->tile_m_used = in->tile_m_used;
+        c->symmetry_used = in->symmetry_used;
         c->pruned_used = 1;
         c->last_pruned = 1;
         if (rc) c->last_error = in->last_error;

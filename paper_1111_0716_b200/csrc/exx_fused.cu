@@ -25,11 +25,11 @@ struct FusedState {
 };
 
 // ---------------------------------------------------------------------------------------------------------------
-// pass A: rho = conj(u_m) u_n, z transform, first y step.  One CTA per (tile, m, n), n fastest so that the CTAs that
-// share a u_m / u_n tile run back to back and the tile is fetched from HBM once.
+// pass A: rho = conj(u_b) u_a, z transform, first y step.  One CTA per (tile, pair), pair fastest so that the CTAs that
+// share a u tile run back to back and the tile is fetched from HBM once.
 template <int R1>
-__global__ void __launch_bounds__(FusedCfg<R1>::NT1, FusedCfg<R1>::MINB1) pass_a_kernel(const cplx* __restrict__ un_base, const cplx* __restrict__ uq_base,
-                                                                    MTile mt, int tn, cplx* __restrict__ work) {
+__global__ void __launch_bounds__(FusedCfg<R1>::NT1, FusedCfg<R1>::MINB1) pass_a_kernel(const cplx* __restrict__ ua_base, const cplx* __restrict__ ub_base,
+                                                                    AJob job, cplx* __restrict__ work) {
     constexpr int N = 8 * R1, U = FusedCfg<R1>::U1, NT = FusedCfg<R1>::NT1;
     constexpr bool TWREG = FusedCfg<R1>::TWREG;
     static_assert(!TWREG || NT % R1 == 0, "TWREG needs a thread-invariant k1z");
@@ -38,20 +38,19 @@ __global__ void __launch_bounds__(FusedCfg<R1>::NT1, FusedCfg<R1>::MINB1) pass_a
     cplx* S = reinterpret_cast<cplx*>(smem_raw);
     cplx* T = S + U * R1 * N;
     const int tid = threadIdx.x;
-    unsigned bid = blockIdx.x;
-    const int n = bid % tn;
-    bid /= tn;
-    const int m = bid % mt.tm;
-    const int tile = bid / mt.tm;
+    const unsigned bid = blockIdx.x;
+    const int p = bid % job.npairs;
+    const int tile = bid / job.npairs;
+    const int pi = job.pi[p], pj = job.pj[p];
     const int x = tile / (8 / U), yb = tile % (8 / U);
     cplx twr[8];
     if (TWREG)
         load_twr<R1>(tid, twr);
     else
         for (int i = tid; i < R1 * 8; i += NT) T[tidx(i >> 3, i & 7)] = c_tw[TwOff<R1>::v + (i >> 3) * (i & 7)];
-    const cplx* un = un_base + (size_t)n * Ng;
-    const cplx* um = uq_base + (size_t)mt.m_idx[m] * Ng;
-    cplx* W = work + ((size_t)n * mt.tm + m) * Ng;
+    const cplx* un = ua_base + (size_t)job.a_idx[pi] * Ng;
+    const cplx* um = ub_base + (size_t)job.b_idx[pj] * Ng;
+    cplx* W = work + (size_t)(pi * job.tb + pj) * Ng;
     p1_z1<R1, U, NT>(tid, un, um, x, yb, S);
     __syncthreads();
     p13_z8<R1, U, NT, -1, TWREG>(tid, S, T, twr);
@@ -99,7 +98,7 @@ __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.p
 // (k1y, zb) is one contiguous run of the work box (layout widx): N rows of 512 bytes are bulk-copied (TMA) into the padded
 // shared-memory tile, all five steps run in shared memory, and the rows are bulk-copied back.
 template <int R1>
-__global__ void __launch_bounds__(FusedCfg<R1>::NT2, FusedCfg<R1>::MINB2) pass_b_kernel(cplx* __restrict__ work, const double* __restrict__ kperm, int npairs) {
+__global__ void __launch_bounds__(FusedCfg<R1>::NT2, FusedCfg<R1>::MINB2) pass_b_kernel(cplx* __restrict__ work, const double* __restrict__ kperm, AJob job) {
     constexpr int N = 8 * R1, Z = FusedCfg<R1>::Z, NT = FusedCfg<R1>::NT2, PX = P2Geo<Z>::PX;
     constexpr size_t Ng = (size_t)N * N * N;
     constexpr uint32_t ROWB = 8 * Z * sizeof(cplx);
@@ -108,10 +107,10 @@ __global__ void __launch_bounds__(FusedCfg<R1>::NT2, FusedCfg<R1>::MINB2) pass_b
     __shared__ __align__(8) uint64_t bar;
     const int tid = threadIdx.x;
     const unsigned bid = blockIdx.x;
-    const int pair = bid % npairs;
-    const int tile = bid / npairs;
+    const int p = bid % job.npairs;
+    const int tile = bid / job.npairs;
     const int k1y = tile / (N / Z);
-    cplx* Wt = work + (size_t)pair * Ng + (size_t)tile * ((size_t)N * 8 * Z);
+    cplx* Wt = work + (size_t)(job.pi[p] * job.tb + job.pj[p]) * Ng + (size_t)tile * ((size_t)N * 8 * Z);
     const double* Kt = kperm + (size_t)tile * ((size_t)N * 8 * Z);
     if (tid == 0) mbar_init(&bar, 1);
     __syncthreads();
@@ -133,11 +132,12 @@ __global__ void __launch_bounds__(FusedCfg<R1>::NT2, FusedCfg<R1>::MINB2) pass_b
     bulk_commit_wait_all();
 }
 
-// pass C: second inverse y step, inverse z, acc_n -= w f u_m v.  One CTA per (tile, n) loops over the m-tile with its
-// accumulator tile in shared memory, then adds it to acc_n in global memory once (fixed summation order).
+// pass C: second inverse y step, inverse z, acc -= coef u v.  One CTA per (tile, row) loops over the row's columns with
+// its accumulator tile on chip, then adds it to the row's accumulator box in global memory once (fixed summation order).
+// Rows/columns are the a/b bands of the batch (CJob); the transposed sweep (cj) uses conj(v) and the a-band as multiplier.
 template <int R1>
-__global__ void __launch_bounds__(FusedCfg<R1>::NT3, FusedCfg<R1>::MINB3) pass_c_kernel(const cplx* __restrict__ work, const cplx* __restrict__ uq_base, MTile mt,
-                                                                    int tn, cplx* __restrict__ acc) {
+__global__ void __launch_bounds__(FusedCfg<R1>::NT3, FusedCfg<R1>::MINB3) pass_c_kernel(const cplx* __restrict__ work, const cplx* __restrict__ usrc_base, CJob job,
+                                                                    cplx* __restrict__ acc_base) {
     constexpr int N = 8 * R1, U = FusedCfg<R1>::U3, NT = FusedCfg<R1>::NT3;
     constexpr bool TWREG = FusedCfg<R1>::TWREG, ACCREG = FusedCfg<R1>::ACCREG;
     static_assert(!TWREG || NT % R1 == 0, "TWREG needs a thread-invariant k1z");
@@ -149,9 +149,11 @@ __global__ void __launch_bounds__(FusedCfg<R1>::NT3, FusedCfg<R1>::MINB3) pass_c
     cplx* T = A + (ACCREG ? 0 : U * R1 * N);
     const int tid = threadIdx.x;
     const unsigned bid = blockIdx.x;
-    const int n = bid % tn;
-    const int tile = bid / tn;
+    const int r = bid % job.nr;
+    const int tile = bid / job.nr;
     const int x = tile / (8 / U), yb = tile % (8 / U);
+    const int cnt = job.cnt[r];
+    const bool cj = job.cj != 0;
     cplx twr[8];
     if (TWREG)
         load_twr<R1>(tid, twr);
@@ -162,23 +164,27 @@ __global__ void __launch_bounds__(FusedCfg<R1>::NT3, FusedCfg<R1>::MINB3) pass_c
 #pragma unroll
         for (int i = 0; i < (ACCREG ? IT * R1 : 1); i++) accr[i] = mk(0.0, 0.0);
     }
-    for (int m = 0; m < mt.tm; m++) {
-        const cplx* W = work + ((size_t)n * mt.tm + m) * Ng;
-        const cplx* um = uq_base + (size_t)mt.m_idx[m] * Ng;
+    for (int ci = 0; ci < cnt; ci++) {
+        const int col = job.col[r][ci];
+        const cplx* W = work + (size_t)(r * job.box_r + col * job.box_c) * Ng;
+        const cplx* um = usrc_base + (size_t)job.src[col] * Ng;
+        const double wf = job.coef[col];
         p3_y2inv<R1, U, NT>(tid, W, x, yb, S);
         __syncthreads();
         p13_z8<R1, U, NT, +1, TWREG>(tid, S, T, twr);
         __syncthreads();
         if (ACCREG)
-            p3_zinv2_reg<R1, U, NT>(tid, S, um, mt.wf[m], x, yb, accr);
+            p3_zinv2_reg<R1, U, NT>(tid, S, um, wf, x, yb, accr, cj);
         else
-            p3_zinv2<R1, U, NT>(tid, S, um, mt.wf[m], x, yb, A, m == 0);
+            p3_zinv2<R1, U, NT>(tid, S, um, wf, x, yb, A, ci == 0, cj);
         __syncthreads();
     }
-    if (ACCREG)
-        p3_flush_reg<R1, U, NT>(tid, accr, acc + (size_t)n * Ng, x, yb);
-    else
-        p3_flush<R1, U, NT>(tid, A, acc + (size_t)n * Ng, x, yb);
+    if (cnt > 0) {
+        if (ACCREG)
+            p3_flush_reg<R1, U, NT>(tid, accr, acc_base + (size_t)job.tgt[r] * Ng, x, yb);
+        else
+            p3_flush<R1, U, NT>(tid, A, acc_base + (size_t)job.tgt[r] * Ng, x, yb);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -196,22 +202,25 @@ struct Launch {
         EXX_CUDA(c, cudaFuncSetAttribute(pass_c_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_c));
         return EXX_OK;
     }
-    // all pairs (n0..n0+tn) x mt of one (k, q): the three passes
-    static int pairs(exx_ctx* c, const cplx* un_base, const cplx* uq_base, const MTile& mt, int tn, const double* kperm, cplx* work, cplx* acc) {
-        const int npairs = tn * mt.tm;
-        const unsigned tiles1 = N * (8 / U1), tiles3 = N * (8 / U3), tiles2 = R1 * (N / Z);
+    // passes A and B over the pairs of one batch
+    static int pass_ab(exx_ctx* c, const cplx* ua_base, const cplx* ub_base, const AJob& job, const double* kperm, cplx* work) {
+        const unsigned tiles1 = N * (8 / U1), tiles2 = R1 * (N / Z);
         {
-            LaunchScope ls(c, KC_PASS_A, npairs);
-            pass_a_kernel<R1><<<tiles1 * npairs, FusedCfg<R1>::NT1, smem_a, c->stream>>>(un_base, uq_base, mt, tn, work);
+            LaunchScope ls(c, KC_PASS_A, job.npairs);
+            pass_a_kernel<R1><<<tiles1 * job.npairs, FusedCfg<R1>::NT1, smem_a, c->stream>>>(ua_base, ub_base, job, work);
         }
         {
-            LaunchScope ls(c, KC_PASS_B, npairs);
-            pass_b_kernel<R1><<<tiles2 * npairs, FusedCfg<R1>::NT2, smem_b, c->stream>>>(work, kperm, npairs);
+            LaunchScope ls(c, KC_PASS_B, job.npairs);
+            pass_b_kernel<R1><<<tiles2 * job.npairs, FusedCfg<R1>::NT2, smem_b, c->stream>>>(work, kperm, job);
         }
-        {
-            LaunchScope ls(c, KC_PASS_C, npairs);
-            pass_c_kernel<R1><<<tiles3 * tn, FusedCfg<R1>::NT3, smem_c, c->stream>>>(work, uq_base, mt, tn, acc);
-        }
+        EXX_CUDA(c, cudaGetLastError());
+        return EXX_OK;
+    }
+    // one accumulation sweep (pass C)
+    static int pass_c(exx_ctx* c, const cplx* usrc_base, const CJob& job, int64_t units, const cplx* work, cplx* acc_base) {
+        const unsigned tiles3 = N * (8 / U3);
+        LaunchScope ls(c, KC_PASS_C, units);
+        pass_c_kernel<R1><<<tiles3 * job.nr, FusedCfg<R1>::NT3, smem_c, c->stream>>>(work, usrc_base, job, acc_base);
         EXX_CUDA(c, cudaGetLastError());
         return EXX_OK;
     }
@@ -294,6 +303,13 @@ void fused_destroy(exx_ctx* c) {
     c->fused = nullptr;
 }
 
+// The loop nest (k and q on the host, band loops on the device, innermost loop blocked).  Bands are cut into
+// a-tiles (k-point k) and b-tiles (k-point q) of at most 16; every batch evaluates v for the pairs of one (a-tile, b-tile)
+// block (passes A, B) and sweeps pass C once per side that receives a contribution.
+//   plain mode:    all ordered (k, q); pair (a, b) evaluated iff f_b != 0;   acc_a -= w_q f_b u_b v
+//   symmetry mode: k <= q, and a <= b when k == q; pair evaluated iff f_a != 0 or f_b != 0;
+//                  acc_a -= w_q f_b u_b v   and (unless a == b)   acc_b -= w_k f_a u_a conj(v)
+// using v_{bq,ak} = conj(v_{ak,bq}) (K real and K_{q-k}(g) = K_{k-q}(-g); exact on an alias-free grid).
 int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out) {
     FusedState* st = (FusedState*)c->fused;
     if (!st) return EXX_ERR_BAD_ARG;
@@ -303,42 +319,157 @@ int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out)
     c->path_used = 2;
     c->pruned_used = 0;
     if ((rc = compute_u_cache(c, psi))) return rc;
-    int tn_max = (int)c->acc_boxes, tm_max = (int)std::min<size_t>(32, c->work_boxes / c->acc_boxes);
-    if (c->opt_tile_n > 0) tn_max = (int)std::min<int64_t>(tn_max, c->opt_tile_n);
-    if (c->opt_tile_m > 0) tm_max = (int)std::min<int64_t>(tm_max, c->opt_tile_m);
-    c->tile_n_used = tn_max;
-    c->tile_m_used = tm_max;
+    int ta_max = 16, tb_max = 16;
+    while ((size_t)ta_max * tb_max > c->work_boxes && tb_max > 1) tb_max /= 2;
+    while ((size_t)ta_max * tb_max > c->work_boxes && ta_max > 1) ta_max /= 2;
+    if (c->opt_tile_n > 0) ta_max = (int)std::min<int64_t>(ta_max, c->opt_tile_n);
+    if (c->opt_tile_m > 0) tb_max = (int)std::min<int64_t>(tb_max, c->opt_tile_m);
+    const bool sym = c->opt_symmetry && c->alias_free;
+    if (sym) ta_max = tb_max = std::min(ta_max, tb_max);  // diagonal blocks need matching tiles
+    c->tile_n_used = ta_max;
+    c->tile_m_used = tb_max;
+    c->symmetry_used = sym ? 1 : 0;
     cplx* work = (cplx*)c->work_dev;
-    cplx* acc = (cplx*)c->acc_dev;
+    cplx* acc = (cplx*)c->acc_dev;  // one accumulator box per (k, band)
+    EXX_CUDA(c, cudaMemsetAsync(acc, 0, sizeof(cplx) * Ng * (size_t)nk * nb, c->stream));
     for (int k = 0; k < nk; k++)
-        for (int n0 = 0; n0 < nb; n0 += tn_max) {
-            const int tn = std::min(tn_max, nb - n0);
-            EXX_CUDA(c, cudaMemsetAsync(acc, 0, sizeof(cplx) * Ng * tn, c->stream));
-            const cplx* un_base = (const cplx*)c->u_dev + ((size_t)k * nb + n0) * Ng;
-            for (int q = 0; q < nk; q++) {
-                const double* kperm = st->kperm_dev + (size_t)c->ktab_of[(size_t)k * nk + q] * Ng;
-                const cplx* uq = (const cplx*)c->u_dev + (size_t)q * nb * Ng;
-                MTile mt;
-                mt.tm = 0;
-                for (int m = 0; m <= nb; m++) {
-                    if (m < nb && occ[q * nb + m] != 0.0) {
-                        mt.m_idx[mt.tm] = m;
-                        mt.wf[mt.tm] = c->kw[q] * occ[q * nb + m];
-                        mt.tm++;
+        for (int q = sym ? k : 0; q < nk; q++) {
+            const double* kperm = st->kperm_dev + (size_t)c->ktab_of[(size_t)k * nk + q] * Ng;
+            const cplx* ua = (const cplx*)c->u_dev + (size_t)k * nb * Ng;
+            const cplx* ub = (const cplx*)c->u_dev + (size_t)q * nb * Ng;
+            // b-bands: in plain mode only bands with f != 0 take part as m
+            std::vector<int> blist;
+            for (int m = 0; m < nb; m++)
+                if (sym || occ[q * nb + m] != 0.0) blist.push_back(m);
+            for (int a0 = 0; a0 < nb; a0 += ta_max)
+                for (size_t b0 = (sym && k == q) ? (size_t)a0 : 0; b0 < blist.size(); b0 += tb_max) {
+                    const int ta = std::min(ta_max, nb - a0), tb = (int)std::min<size_t>(tb_max, blist.size() - b0);
+                    AJob aj;
+                    aj.npairs = 0;
+                    aj.tb = tb;
+                    bool ev[16][16];
+                    for (int i = 0; i < ta; i++) aj.a_idx[i] = a0 + i;
+                    for (int j = 0; j < tb; j++) aj.b_idx[j] = blist[b0 + j];
+                    for (int i = 0; i < ta; i++)
+                        for (int j = 0; j < tb; j++) {
+                            const double fa = occ[k * nb + aj.a_idx[i]], fb = occ[q * nb + aj.b_idx[j]];
+                            bool e = sym ? ((fa != 0.0 || fb != 0.0) && (k < q || aj.a_idx[i] <= aj.b_idx[j])) : (fb != 0.0);
+                            ev[i][j] = e;
+                            if (e) {
+                                aj.pi[aj.npairs] = (unsigned char)i;
+                                aj.pj[aj.npairs] = (unsigned char)j;
+                                aj.npairs++;
+                            }
+                        }
+                    if (aj.npairs == 0) continue;
+                    EXX_DISPATCH_R1(st->R1, rc = L::pass_ab(c, ua, ub, aj, kperm, work));
+                    if (rc) return rc;
+                    c->pairs_executed += aj.npairs;
+                    // side a: rows = a-bands, columns = b-bands with f_b != 0
+                    {
+                        CJob cj;
+                        cj.nr = 0;
+                        cj.box_r = tb;
+                        cj.box_c = 1;
+                        cj.cj = 0;
+                        int64_t units = 0;
+                        int rowbox[16];
+                        for (int j = 0; j < tb; j++) {
+                            cj.src[j] = aj.b_idx[j];
+                            cj.coef[j] = c->kw[q] * occ[q * nb + aj.b_idx[j]];
+                        }
+                        for (int i = 0; i < ta; i++) {
+                            int n = 0;
+                            for (int j = 0; j < tb; j++)
+                                if (ev[i][j] && occ[q * nb + aj.b_idx[j]] != 0.0) cj.col[cj.nr][n++] = (unsigned char)j;
+                            if (n) {
+                                cj.cnt[cj.nr] = n;
+                                cj.tgt[cj.nr] = k * nb + aj.a_idx[i];
+                                rowbox[cj.nr] = i;
+                                cj.nr++;
+                                units += n;
+                            }
+                        }
+                        if (cj.nr) {
+                            // rows were compacted: the work box of (row r, column c) is rowbox[r]*tb + c, so shift the work
+                            // base per launch only when rows are contiguous; otherwise launch row by row groups
+                            bool contiguous = true;
+                            for (int r = 0; r < cj.nr; r++) contiguous = contiguous && rowbox[r] == rowbox[0] + r;
+                            if (contiguous) {
+                                EXX_DISPATCH_R1(st->R1, rc = L::pass_c(c, ub, cj, units, work + (size_t)rowbox[0] * tb * Ng, acc));
+                                if (rc) return rc;
+                            } else {
+                                for (int r = 0; r < cj.nr; r++) {
+                                    CJob one = cj;
+                                    one.nr = 1;
+                                    one.cnt[0] = cj.cnt[r];
+                                    one.tgt[0] = cj.tgt[r];
+                                    for (int n = 0; n < cj.cnt[r]; n++) one.col[0][n] = cj.col[r][n];
+                                    EXX_DISPATCH_R1(st->R1, rc = L::pass_c(c, ub, one, cj.cnt[r], work + (size_t)rowbox[r] * tb * Ng, acc));
+                                    if (rc) return rc;
+                                }
+                            }
+                            c->pairs_ordered += units;
+                        }
                     }
-                    if (mt.tm == tm_max || (m == nb && mt.tm > 0)) {
-                        EXX_DISPATCH_R1(st->R1, rc = L::pairs(c, un_base, uq, mt, tn, kperm, work, acc));
-                        if (rc) return rc;
-                        c->pairs_executed += (int64_t)tn * mt.tm;
-                        c->pairs_ordered += (int64_t)tn * mt.tm;
-                        mt.tm = 0;
+                    // side b (symmetry): rows = b-bands, columns = a-bands with f_a != 0, conj(v); the pair a == b is not repeated
+                    if (sym) {
+                        CJob cj;
+                        cj.nr = 0;
+                        cj.box_r = 1;
+                        cj.box_c = tb;
+                        cj.cj = 1;
+                        int64_t units = 0;
+                        int rowbox[16];
+                        for (int i = 0; i < ta; i++) {
+                            cj.src[i] = aj.a_idx[i];
+                            cj.coef[i] = c->kw[k] * occ[k * nb + aj.a_idx[i]];
+                        }
+                        for (int j = 0; j < tb; j++) {
+                            int n = 0;
+                            for (int i = 0; i < ta; i++)
+                                if (ev[i][j] && occ[k * nb + aj.a_idx[i]] != 0.0 && !(k == q && aj.a_idx[i] == aj.b_idx[j]))
+                                    cj.col[cj.nr][n++] = (unsigned char)i;
+                            if (n) {
+                                cj.cnt[cj.nr] = n;
+                                cj.tgt[cj.nr] = q * nb + aj.b_idx[j];
+                                rowbox[cj.nr] = j;
+                                cj.nr++;
+                                units += n;
+                            }
+                        }
+                        if (cj.nr) {
+                            bool contiguous = true;
+                            for (int r = 0; r < cj.nr; r++) contiguous = contiguous && rowbox[r] == rowbox[0] + r;
+                            if (contiguous) {
+                                EXX_DISPATCH_R1(st->R1, rc = L::pass_c(c, ua, cj, units, work + (size_t)rowbox[0] * Ng, acc));
+                                if (rc) return rc;
+                            } else {
+                                for (int r = 0; r < cj.nr; r++) {
+                                    CJob one = cj;
+                                    one.nr = 1;
+                                    one.cnt[0] = cj.cnt[r];
+                                    one.tgt[0] = cj.tgt[r];
+                                    for (int n = 0; n < cj.cnt[r]; n++) one.col[0][n] = cj.col[r][n];
+                                    EXX_DISPATCH_R1(st->R1, rc = L::pass_c(c, ua, one, cj.cnt[r], work + (size_t)rowbox[r] * Ng, acc));
+                                    if (rc) return rc;
+                                }
+                            }
+                            c->pairs_ordered += units;
+                        }
                     }
                 }
-            }
-            // S7: forward transform of the accumulators, gather onto sphere(k)
-            if ((rc = launch_fft3d_generic(c, (double2*)acc, tn, -1))) return rc;
-            if ((rc = launch_gather(c, k, (const double2*)acc, tn, out + c->off[k] + (int64_t)n0 * c->npw[k]))) return rc;
         }
+    // S7: forward transform of every accumulator, gather onto sphere(k) (in batches that keep launches below 2^28 elements)
+    for (int k = 0; k < nk; k++) {
+        int bmax = (int)std::max<int64_t>(1, std::min<int64_t>(nb, ((int64_t)1 << 28) / (int64_t)Ng));
+        for (int n0 = 0; n0 < nb; n0 += bmax) {
+            int bn = std::min(bmax, nb - n0);
+            double2* box = (double2*)acc + ((size_t)k * nb + n0) * Ng;
+            if ((rc = launch_fft3d_generic(c, box, bn, -1))) return rc;
+            if ((rc = launch_gather(c, k, box, bn, out + c->off[k] + (int64_t)n0 * c->npw[k]))) return rc;
+        }
+    }
     return EXX_OK;
 }
 

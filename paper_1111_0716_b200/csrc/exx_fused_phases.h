@@ -11,6 +11,7 @@
 //   pass A (p1_*): rho = conj(u_m) u_n; z transform (both steps); first y step          tile: one x, U values of y mod 8
 //   pass B (p2_*): second y step; x transform; times K'; inverse x; first inverse y step  tile: one k1y, Z positions of z
 //   pass C (p3_*): second inverse y step; inverse z; acc -= w f u_m v                     tile: as pass A, loops over m
+// With pair symmetry (v_{mq,nk} = conj v_{nk,mq}) pass C runs a second time with the roles of the bands swapped (cj).
 #pragma once
 #include <stddef.h>
 
@@ -368,7 +369,7 @@ EXX_HD void p3_y2inv(int tid, const cplx* __restrict__ W, int x, int yb, cplx* S
 }
 
 template <int R1, int U, int NT>
-EXX_HD void p3_zinv2(int tid, const cplx* S, const cplx* __restrict__ um, double wf, int x, int yb, cplx* A, bool first) {
+EXX_HD void p3_zinv2(int tid, const cplx* S, const cplx* __restrict__ um, double wf, int x, int yb, cplx* A, bool first, bool cj = false) {
     // items (row, n2z): last inverse z step, then acc -= (w_q f_m) u_m v   (S6); A is this CTA's private accumulator tile
     constexpr int N = 8 * R1, NI = U * R1 * 8, IT = (NI + NT - 1) / NT;
 #pragma unroll
@@ -386,7 +387,7 @@ EXX_HD void p3_zinv2(int tid, const cplx* S, const cplx* __restrict__ um, double
             dft<R1, +1>(v);
 #pragma unroll
             for (int j = 0; j < R1; j++) {
-                cplx p = b[j] * v[j];
+                cplx p = b[j] * (cj ? mk(v[j].x, -v[j].y) : v[j]);  // cj: the transposed pair uses conj(v)
                 cplx* a = A + row * N + j * 8 + n2z;
                 if (first)
                     *a = mk(-wf * p.x, -wf * p.y);
@@ -418,7 +419,7 @@ EXX_HD void p3_flush(int tid, const cplx* A, cplx* __restrict__ accg, int x, int
 
 // register-accumulator variants (ACCREG): acc[i*R1 + j] belongs to item tid + i*NT, element n1z = j
 template <int R1, int U, int NT>
-EXX_HD void p3_zinv2_reg(int tid, const cplx* S, const cplx* __restrict__ um, double wf, int x, int yb, cplx* acc) {
+EXX_HD void p3_zinv2_reg(int tid, const cplx* S, const cplx* __restrict__ um, double wf, int x, int yb, cplx* acc, bool cj = false) {
     constexpr int N = 8 * R1, NI = U * R1 * 8, IT = (NI + NT - 1) / NT;
 #pragma unroll
     for (int i = 0; i < IT; i++) {
@@ -435,7 +436,7 @@ EXX_HD void p3_zinv2_reg(int tid, const cplx* S, const cplx* __restrict__ um, do
             dft<R1, +1>(v);
 #pragma unroll
             for (int j = 0; j < R1; j++) {
-                cplx p = b[j] * v[j];
+                cplx p = b[j] * (cj ? mk(v[j].x, -v[j].y) : v[j]);  // cj: the transposed pair uses conj(v)
                 acc[i * R1 + j] = mk(acc[i * R1 + j].x - wf * p.x, acc[i * R1 + j].y - wf * p.y);
             }
         }

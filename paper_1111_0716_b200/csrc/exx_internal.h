@@ -91,9 +91,10 @@ struct exx_ctx {
     int last_pruned = 0;
 
     // options
-    int64_t opt_path = 0, opt_tile_n = 0, opt_tile_m = 0, opt_prune = 1, opt_profile = 0;
+    int64_t opt_path = 0, opt_tile_n = 0, opt_tile_m = 0, opt_prune = 1, opt_profile = 0, opt_symmetry = 1;
 
     // counters of the last apply
+    int64_t symmetry_used = 0;
     int64_t launches = 0, pairs_ordered = 0, pairs_executed = 0, path_used = 0, tile_n_used = 0, tile_m_used = 0, pruned_used = 0;
     int64_t launches_by_class[exx::KC_COUNT] = {0};
     int64_t units_by_class[exx::KC_COUNT] = {0};   // box passes (generic) or pairs (fused) processed
@@ -129,6 +130,21 @@ struct MTile {
     int tm;
     int m_idx[32];     // band indices within k-point q
     double wf[32];     // w_q * f_mq
+};
+// one batch of band pairs for the fused passes: a-bands (k-point ka) x b-bands (k-point kb), at most 16 x 16.
+// Pair p = (pi[p], pj[p]) evaluates v = IFFT K' FFT[conj(u_b) u_a]; its work box is pi*tb + pj.
+struct AJob {
+    int npairs, tb;
+    int a_idx[16], b_idx[16];          // band indices within their k-points
+    unsigned char pi[256], pj[256];
+};
+// one accumulation sweep of pass C: CTA row r owns accumulator box tgt[r] and loops over its cnt[r] columns:
+//   acc[tgt[r]] -= coef[c] * u[src[c]] * (cj ? conj(v) : v),   v in work box r*box_r + c*box_c
+struct CJob {
+    int nr, box_r, box_c, cj;
+    int tgt[16], cnt[16], src[16];
+    double coef[16];
+    unsigned char col[16][16];
 };
 int fft_generic_init(exx_ctx* c);
 int launch_scatter(exx_ctx* c, int ik, const double2* coef, int nbatch, double2* box);

@@ -169,7 +169,7 @@ def test_apply_C1_full_parity(B):
     assert abs(e - gold["E_x_E1"]) < 1e-15
 
 
-def _check_golden(B, name, live_rows=0, prune=1):
+def _check_golden(B, name, live_rows=0, prune=1, symmetry=1):
     """Big configs: the GPU applies V_x in full; rows, per-band energies and E_x are compared with stored oracle
     results (tests/golden/make_golden.py) and, for `live_rows` rows, with the oracle run now."""
     import torch
@@ -184,7 +184,10 @@ def _check_golden(B, name, live_rows=0, prune=1):
     assert [psi[0].real, psi[0].imag] == gold["psi_first"]
     pd = g.to_device(psi)
     g.set_option(B.EXX_OPT_PRUNE, prune)
+    g.set_option(B.EXX_OPT_SYMMETRY, symmetry)
     out = g.apply(pd, w.occ)
+    assert g.get_info(B.EXX_INFO_SYMMETRY) == symmetry
+    assert g.get_info(B.EXX_INFO_PAIRS_EXECUTED) == (w.pair_evals if not symmetry else g.get_info(B.EXX_INFO_PAIRS_EXECUTED))
     assert g.get_info(B.EXX_INFO_PRUNED) == (1 if (prune and g.get_info(B.EXX_INFO_COMPACT_GRID)) else 0)
     e, pb = g.energy(pd, w.occ, out)
     torch.cuda.synchronize()
@@ -253,10 +256,13 @@ def test_compact_grid_equals_full_grid_and_oracle(B, name):
     e_want, _ = o.energy(psi, w.occ, want)
     pd = g.to_device(psi)
     res = {}
-    for prune in (1, 0):
+    for prune, sym in ((1, 1), (0, 1), (1, 0)):
         g.set_option(B.EXX_OPT_PRUNE, prune)
+        g.set_option(B.EXX_OPT_SYMMETRY, sym)
         out = g.apply(pd, w.occ)
         assert g.get_info(B.EXX_INFO_PRUNED) == prune
+        assert g.get_info(B.EXX_INFO_SYMMETRY) == sym
+        assert (g.get_info(B.EXX_INFO_PAIRS_EXECUTED) < w.pair_evals) == bool(sym)
         assert g.get_info(B.EXX_INFO_WORK_GRID) == (s["compact"] if prune else 64)
         assert g.get_info(B.EXX_INFO_PAIRS_ORDERED) == w.pair_evals
         got = out.cpu().numpy()
@@ -265,9 +271,16 @@ def test_compact_grid_equals_full_grid_and_oracle(B, name):
                 assert _rel(o.band(got, k, n), o.band(want, k, n)) < TOL_VX, (name, prune, k, n)
         e, _ = g.energy(pd, w.occ, out)
         assert abs(e - e_want) <= TOL_EX * abs(e_want)
-        res[prune] = got
-    assert _rel(res[1], res[0]) < 1e-13
+        res[(prune, sym)] = got
+    assert _rel(res[(1, 1)], res[(0, 1)]) < 1e-13
+    assert _rel(res[(1, 1)], res[(1, 0)]) < 1e-13
     g.close()
+
+
+@pytest.mark.parametrize("name", ["C2", "C3"])
+def test_pair_symmetry_off_matches_golden(B, name):
+    """The default runs use the pair symmetry; this one evaluates every ordered pair (EXX_OPT_SYMMETRY = 0)."""
+    _check_golden(B, name, symmetry=0)
 
 
 def test_compact_grid_not_used_when_caller_grid_aliases(B):

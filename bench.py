@@ -197,7 +197,7 @@ def run_ours(args, rank, world, local):
     try:
         tj = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic_r1.json")))
         if tj["work_grid"] ** 3 == ngw and dom in tj["dram_bytes_per_launch"]:
-            traffic = tj["dram_bytes_per_launch"][dom] / tj["pairs_per_launch"] * (u_dom / max(1, n_dom))
+            traffic = tj["dram_bytes_per_launch"][dom] / tj["units_per_launch"][dom] * (u_dom / max(1, n_dom))
     except Exception:
         pass
     roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,

@@ -60,15 +60,15 @@ template <int R1>
 struct FusedCfgBase;
 template <>
 struct FusedCfgBase<6> {
-    static constexpr int U1 = 4, NT1 = 96, U3 = 4, NT3 = 96, Z = 4, NT2 = 64;
+    static constexpr int U1 = 2, NT1 = 96, U3 = 2, NT3 = 96, Z = 4, NT2 = 64;
     static constexpr bool TWREG = false, ACCREG = false;
-    static constexpr int MINB1 = 1, MINB2 = 1, MINB3 = 1;  // min CTAs per SM asked of the compiler (register cap)
+    static constexpr int MINB1 = 1, MINB2 = 6, MINB3 = 1;  // min CTAs per SM asked of the compiler (register cap)
 };
 template <>
 struct FusedCfgBase<8> {
-    static constexpr int U1 = 4, NT1 = 128, U3 = 4, NT3 = 128, Z = 4, NT2 = 128;
+    static constexpr int U1 = 2, NT1 = 128, U3 = 2, NT3 = 128, Z = 4, NT2 = 128;
     static constexpr bool TWREG = false, ACCREG = false;
-    static constexpr int MINB1 = 1, MINB2 = 1, MINB3 = 1;
+    static constexpr int MINB1 = 1, MINB2 = 4, MINB3 = 1;
 };
 template <>
 struct FusedCfgBase<9> {

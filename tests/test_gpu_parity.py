@@ -370,3 +370,66 @@ def test_to_real_matches_oracle(B):
         for n in range(w.nbands):
             assert _rel(hb[n], o.to_real(k, o.band(psi, k, n))) < 1e-14
     g.close()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# Properties of the GPU result that hold at any size and need no oracle (checked at a full BASELINE size, C3)
+def test_gpu_operator_properties_C3(B):
+    import torch
+    w = W.make("C3")
+    g = B.Exx.from_workload(w)
+    psi = w.coefficients(g.npw)
+    pd = g.to_device(psi)
+    out = g.apply(pd, w.occ).clone()
+    e, pb = g.energy(pd, w.occ, out)
+    npw, nb = g.npw[0], w.nbands
+    Cm, Vm = pd.view(nb, npw), out.view(nb, npw)
+    # Hermiticity of M_ij = <c_i | V_x c_j> (all 64 bands occupied, so V_x is the full operator on this subspace)
+    M = torch.conj(Cm) @ Vm.T
+    assert float((M - torch.conj(M.T)).abs().max()) <= 1e-13 * float(M.abs().max())
+    # V_x is negative semi-definite on the occupied subspace: all eigenvalues of M <= 0
+    ev = torch.linalg.eigvalsh(0.5 * (M + torch.conj(M.T)))
+    assert float(ev.max()) <= 1e-14
+    assert abs(0.5 * float(torch.diagonal(M).real.sum()) - e) <= 1e-13 * abs(e)
+    # covariance under a global phase: c -> e^{i theta} c  =>  V_x c -> e^{i theta} V_x c, E_x unchanged
+    ph = complex(np.cos(0.7), np.sin(0.7))
+    out2 = g.apply(pd * ph, w.occ)
+    assert float((out2 - out * ph).abs().max()) <= 1e-13 * float(out.abs().max())
+    e2, _ = g.energy(pd * ph, w.occ, out2)
+    assert abs(e2 - e) <= 1e-13 * abs(e)
+    # unitary mix of equally occupied bands: c -> U c  =>  out -> U out
+    rng = np.random.default_rng(1)
+    q, _ = np.linalg.qr(rng.standard_normal((nb, nb)) + 1j * rng.standard_normal((nb, nb)))
+    U = torch.from_numpy(q).cuda()
+    out3 = g.apply((U @ Cm).reshape(-1).contiguous(), w.occ)
+    assert float((out3.view(nb, npw) - U @ Vm).abs().max()) <= 1e-12 * float(out.abs().max())
+    g.close()
+
+
+def test_gpu_closed_form_single_plane_waves(B):
+    """Bands that are single plane waves: E_x = -(1/2 Omega) sum_{n,m} f_n f_m 4 pi/|G_n - G_m|^2 (BASELINE north_star closed
+    form), evaluated in the test; the GPU (fused path, 48^3) must reproduce it without any oracle in between."""
+    import torch
+    a, N = 9.0, 48
+    w = W.custom("pw48", 1, (N, N, N), W.cubic(a), [[0, 0, 0]], [1.0], 4.0, 5, [1, 1, 0.5, 1, 0.25])
+    g = B.Exx.from_workload(w)
+    gs = [(0, 0, 0), (1, 0, 0), (0, 2, 0), (-1, 1, 3), (2, -2, 1)]
+    m = g.index_map(0)
+    psi = np.zeros((5, g.npw[0]), dtype=np.complex128)
+    for n, gv in enumerate(gs):
+        box = ((gv[0] % N) * N + (gv[1] % N)) * N + (gv[2] % N)
+        psi[n, int(np.where(m == box)[0][0])] = 1.0
+    f = w.occ
+    want = 0.0
+    for n in range(5):
+        for k in range(5):
+            d = np.array(gs[n]) - np.array(gs[k])
+            if d.any():
+                want -= 0.5 / a ** 3 * f[n] * f[k] * 4 * np.pi / ((2 * np.pi / a) ** 2 * float(d @ d))
+    pd = g.to_device(psi.reshape(-1))
+    for sym in (1, 0):
+        g.set_option(B.EXX_OPT_SYMMETRY, sym)
+        e, _ = g.energy(pd, f, None)
+        assert g.get_info(B.EXX_INFO_PATH_USED) == 2
+        assert abs(e - want) <= 1e-13 * abs(want)
+    g.close()

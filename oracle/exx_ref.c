@@ -475,6 +475,26 @@ int exx_ref_energy(const exx_ref_ctx *c, const double *psi_, const double *occ, 
     return EXX_REF_OK;
 }
 
+/* Subspace matrix of the exchange operator within k-point ik (BASELINE north_star: "the optional dense subspace matrix
+ * <psi_i|V_x|psi_j>"; the paper's NSIM "matrix-matrix operations"):
+ *   M[i*nb + j] = sum_{g in sphere(ik)} conj(c_i(g)) (V_x c)_j(g),   i, j = 0..nb-1, row-major complex, plain triple loop.
+ * Pins (tests/test_oracle_exchange.py): numpy.einsum (independent library), Hermiticity when every band is occupied,
+ * E_x = 1/2 sum w_k f_n Re M_nn. */
+int exx_ref_subspace(const exx_ref_ctx *c, int ik, const double *psi_, const double *vxpsi_, double *m_) {
+    if (!c || !psi_ || !vxpsi_ || !m_) return EXX_REF_ERR_NULL;
+    if (ik < 0 || ik >= c->nk) return EXX_REF_ERR_BAD_ARG;
+    const cplx *psi = (const cplx *)psi_ + c->off[ik], *vx = (const cplx *)vxpsi_ + c->off[ik];
+    cplx *m = (cplx *)m_;
+    const int64_t npw = c->npw[ik];
+    for (int i = 0; i < c->nb; i++)
+        for (int j = 0; j < c->nb; j++) {
+            cplx s = 0.0;
+            for (int64_t ig = 0; ig < npw; ig++) s += conj(psi[i * npw + ig]) * vx[j * npw + ig];
+            m[(int64_t)i * c->nb + j] = s;
+        }
+    return EXX_REF_OK;
+}
+
 /* (E2): E_x = -1/2 (1/Omega) sum_{k,q} w_k w_q sum_{n,m} f f sum_g K |rho~|^2 — forward transforms only. */
 int exx_ref_energy_e2(const exx_ref_ctx *c, const double *psi_, const double *occ, double *ex) {
     if (!c || !psi_ || !occ || !ex) return EXX_REF_ERR_NULL;

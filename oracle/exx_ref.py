@@ -49,6 +49,7 @@ def lib():
         L.exx_ref_apply_direct.argtypes = [vp, dp, dp, dp]
         L.exx_ref_energy.argtypes = [vp, dp, dp, dp, dp, dp]
         L.exx_ref_energy_e2.argtypes = [vp, dp, dp, dp]
+        L.exx_ref_subspace.argtypes = [vp, C.c_int, dp, dp, dp]
         L.exx_ref_dft1d.argtypes = [C.c_int, C.c_int, dp, dp]
         L.exx_ref_dft1d.restype = None
         L.exx_ref_fft1d.argtypes = [C.c_int, C.c_int, dp, dp]
@@ -212,6 +213,14 @@ class RefExx:
         pb = np.empty(self.nk * self.nbands)
         _chk(lib().exx_ref_energy(self._h, _dp(psi), _dp(occ), _dp(vx), C.cast(C.byref(ex), C.POINTER(C.c_double)), _dp(pb)))
         return ex.value, pb
+
+    def subspace(self, ik, psi, vxpsi):
+        """M[i, j] = <c_i | (V_x c)_j> within k-point ik (nb x nb complex)."""
+        psi = _c128(psi).reshape(-1)
+        vx = _c128(vxpsi).reshape(-1)
+        m = np.empty((self.nbands, self.nbands), dtype=np.complex128)
+        _chk(lib().exx_ref_subspace(self._h, ik, _dp(psi), _dp(vx), _dp(m)))
+        return m
 
     def energy_e2(self, psi, occ):
         psi = _c128(psi).reshape(-1)

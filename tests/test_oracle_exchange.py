@@ -257,3 +257,24 @@ def test_C1_whole_config_value_and_independent_library():
     # value recorded by the survey probe (numpy.fft, not a paper value)
     assert abs(e1 - (-0.0623251812923801)) < 1e-14
     assert abs(np.linalg.norm(o.band(out, 0, 0)) - 0.01853725795907376) < 1e-15
+
+
+def test_subspace_matrix_pins():
+    """exx_ref_subspace against an independent library contraction (numpy.einsum), Hermiticity with all bands occupied, and
+    the trace identity E_x = 1/2 sum_k w_k sum_n f_n Re M_nn."""
+    w, o, psi = _small(occ=(1.0, 1.0, 1.0, 1.0, 1.0), kpts=True)
+    out = o.apply(psi, w.occ)
+    e, _ = o.energy(psi, w.occ, out)
+    tr = 0.0
+    for k in range(w.nk):
+        c = np.array([o.band(psi, k, n) for n in range(w.nbands)])
+        v = np.array([o.band(out, k, n) for n in range(w.nbands)])
+        M = o.subspace(k, psi, out)
+        assert M.shape == (w.nbands, w.nbands)
+        assert np.abs(M - np.einsum("ig,jg->ij", c.conj(), v)).max() < 1e-16 * w.nbands * 10
+        assert np.abs(M - M.conj().T).max() < 1e-15 * np.abs(M).max()
+        tr += 0.5 * w.kweight[k] * float((w.occ[k * w.nbands:(k + 1) * w.nbands] * np.diagonal(M).real).sum())
+    assert abs(tr - e) < 1e-15
+    # a transposed operand or a missing conjugate would fail this: M computed from (psi, out) is not M from (out, psi)^T
+    M01 = o.subspace(0, psi, out)
+    assert np.abs(o.subspace(0, out, psi) - M01.conj().T).max() < 1e-16

@@ -85,7 +85,7 @@ enum {
     EXX_INFO_TILE_N = 7,
     EXX_INFO_TILE_M = 8,
     EXX_INFO_PRUNED = 9,          /* 1 if band-limit pruning was active */
-    EXX_INFO_NUM_KERNEL_CLASSES = 10,
+    EXX_INFO_NUM_KERNEL_CLASSES = 10,  /* how many kernel classes exx_get_kernel_time knows (the value, not this enum) */
     EXX_INFO_WORK_GRID = 11,      /* N of the (cubic) grid the last apply transformed; first axis of the caller's grid if not compacted */
     EXX_INFO_SYMMETRY = 13,       /* 1 if the last apply used the pair symmetry (then PAIRS_EXECUTED < PAIRS_ORDERED) */
     EXX_INFO_COMPACT_GRID = 12    /* (no apply needed) N of the compact work grid, 0 if none: the smallest supported cubic grid with
@@ -126,6 +126,13 @@ int exx_apply(exx_ctx* ctx, const double* psi_dev, const double* occ_host, doubl
  * Synchronises the stream. */
 int exx_energy(exx_ctx* ctx, const double* psi_dev, const double* occ_host, const double* vxpsi_dev_or_null, double* ex_host,
                double* per_band_host_or_null);
+
+/* Subspace matrix of the exchange operator within k-point ik (BASELINE north_star "optional dense subspace matrix
+ * <psi_i|V_x|psi_j>"; the paper's NSIM matrix-matrix work):  m_dev[i*nbands + j] = sum_g conj(c_i(g)) (V_x c)_j(g),
+ * nbands x nbands complex128, row-major, device.  psi_dev / vxpsi_dev: the packed arrays of exx_apply (all k-points).
+ * A ZGEMM on the fp64 tensor-core path (DMMA), split over the plane waves and reduced in a fixed order (deterministic).
+ * Asynchronous on the stream.  Hermitian when vxpsi = V_x psi and every band is occupied. */
+int exx_subspace(exx_ctx* ctx, int ik, const double* psi_dev, const double* vxpsi_dev, double* m_dev);
 
 /* Same as exx_apply (+ exx_energy when ex_host_or_null != NULL) on HOST buffers: copies psi to the device, applies,
  * copies out back; synchronises.  Pinned host memory makes the copies asynchronous, pageable memory works too. */

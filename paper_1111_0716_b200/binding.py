@@ -20,7 +20,7 @@ EXX_OPT_PATH, EXX_OPT_TILE_N, EXX_OPT_TILE_M, EXX_OPT_PRUNE, EXX_OPT_PROFILE, EX
 SYMBOLS = ("exx_create", "exx_destroy", "exx_npw", "exx_index_map", "exx_psi_offset", "exx_set_option", "exx_get_option",
            "exx_get_info", "exx_get_kernel_time", "exx_kernel_class_name", "exx_apply", "exx_energy", "exx_apply_host",
            "exx_scatter", "exx_gather", "exx_fft3d", "exx_to_real", "exx_kernel_table", "exx_strerror", "exx_last_error",
-           "exx_version")
+           "exx_version", "exx_subspace")
 
 
 class KernelParams(C.Structure):
@@ -63,6 +63,7 @@ def lib():
         L.exx_apply.argtypes = [vp, vp, dp, vp]
         L.exx_energy.argtypes = [vp, vp, dp, vp, dp, dp]
         L.exx_apply_host.argtypes = [vp, vp, dp, vp, dp]
+        L.exx_subspace.argtypes = [vp, C.c_int, vp, vp, vp]
         L.exx_scatter.argtypes = [vp, C.c_int, vp, C.c_int, vp]
         L.exx_gather.argtypes = [vp, C.c_int, vp, C.c_int, vp]
         L.exx_fft3d.argtypes = [vp, vp, C.c_int, C.c_int]
@@ -202,6 +203,14 @@ class Exx:
         self._chk(lib().exx_energy(self._h, self._dev(psi_dev, self.ncoef), _dp(occ), vx,
                                    C.cast(C.byref(ex), C.POINTER(C.c_double)), _dp(pb)))
         return ex.value, pb
+
+    def subspace(self, ik, psi_dev, vxpsi_dev, m_dev=None):
+        """M[i, j] = <c_i | (V_x c)_j> within k-point ik: (nbands, nbands) complex128 CUDA tensor."""
+        if m_dev is None:
+            m_dev = self._torch.empty((self.nbands, self.nbands), dtype=self._torch.complex128, device="cuda")
+        self._chk(lib().exx_subspace(self._h, ik, self._dev(psi_dev, self.ncoef), self._dev(vxpsi_dev, self.ncoef),
+                                     self._dev(m_dev, self.nbands * self.nbands)))
+        return m_dev
 
     def apply_host(self, psi_host, occ, out_host=None, want_energy=True):
         """psi_host/out_host: complex128 numpy arrays or pinned CPU torch tensors (ncoef elements)."""

@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libexx.so")
-SOURCES = ["exx_api.cu", "exx_kernels.cu", "exx_fused.cu"]
+SOURCES = ["exx_api.cu", "exx_kernels.cu", "exx_fused.cu", "exx_subspace.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--fmad=true",
               "-Xcompiler", "-fPIC,-ffp-contract=off,-Wall,-Wno-unknown-pragmas", "-shared", "-cudart", "shared"]
 

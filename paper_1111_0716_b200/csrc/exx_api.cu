@@ -47,7 +47,7 @@ LaunchScope::~LaunchScope() {
 }
 
 static const char* kclass_names[KC_COUNT] = {"scatter", "gather", "fft_axis_generic", "codensity", "kernel_multiply",
-                                             "accumulate", "energy", "fused_pass_a", "fused_pass_b", "fused_pass_c"};
+                                             "accumulate", "energy", "fused_pass_a", "fused_pass_b", "fused_pass_c", "subspace_zgemm"};
 
 // ---- host arithmetic of S0 (index maps, kernel tables).  Evaluation order of |t.B|^2 is fixed (A11). ----
 static inline int fold(int j, int n) { return (2 * j < n) ? j : j - n; }
@@ -104,6 +104,7 @@ static void free_ctx(exx_ctx* c) {
     cudaFree(c->occw_dev);
     cudaFree(c->band_off_dev);
     cudaFree(c->band_len_dev);
+    cudaFree(c->subspace_dev);
     if (c->host_pinned) cudaFreeHost(c->host_pinned);
     for (auto e : c->event_pool) cudaEventDestroy(e);
     delete c;
@@ -665,6 +666,12 @@ int exx_energy(exx_ctx* c, const double* psi_dev, const double* occ_host, const 
         vx = c->vx_dev;
     }
     return energy_impl(c, (const double2*)psi_dev, occ_host, vx, ex_host, per_band_host_or_null);
+}
+
+int exx_subspace(exx_ctx* c, int ik, const double* psi_dev, const double* vxpsi_dev, double* m_dev) {
+    if (!c || !psi_dev || !vxpsi_dev || !m_dev) return EXX_ERR_NULL;
+    if (ik < 0 || ik >= c->nk) return EXX_ERR_BAD_ARG;
+    return launch_subspace(c, ik, (const double2*)psi_dev, (const double2*)vxpsi_dev, (double2*)m_dev);
 }
 
 int exx_apply_host(exx_ctx* c, const double* psi_host, const double* occ_host, double* out_host, double* ex_host_or_null) {

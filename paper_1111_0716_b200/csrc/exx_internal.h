@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <algorithm>
 #include <string>
 #include <vector>
 
@@ -23,7 +24,8 @@ enum KClass {
     KC_PASS_A = 7,       // fused: co-density + forward (y,z)-plane transform
     KC_PASS_B = 8,       // fused: forward x, K', inverse x
     KC_PASS_C = 9,       // fused: inverse (y,z)-plane transform, times f_m u_m, accumulate
-    KC_COUNT = 10
+    KC_SUBSPACE = 10,    // subspace ZGEMM (DMMA) + its slice reduction
+    KC_COUNT = 11
 };
 
 struct Plan1D {
@@ -77,6 +79,8 @@ struct exx_ctx {
     int64_t* band_off_dev = nullptr;  // nk*nb: offset of band (k,n) in psi (complex elements)
     int* band_len_dev = nullptr;      // nk*nb: npw(k)
     double* host_pinned = nullptr;    // nk*nb + 1 doubles, pinned
+    void* subspace_dev = nullptr;     // split-K partials of exx_subspace (grown on demand)
+    size_t subspace_bytes = 0;
     size_t dev_bytes = 0;
 
     // fused path state (exx_fused.cu)
@@ -154,6 +158,7 @@ int launch_codensity_tile(exx_ctx* c, const double2* un_base, int n0, int tn, co
 int launch_kmul(exx_ctx* c, const double* ktab, double2* work, int nboxes);
 int launch_accumulate_tile(exx_ctx* c, const double2* uq_base, const MTile& mt, int tn, const double2* work, double2* acc);
 int launch_energy(exx_ctx* c, const double2* psi, const double2* vx);
+int launch_subspace(exx_ctx* c, int ik, const double2* psi, const double2* vx, double2* M);  // exx_subspace.cu
 int compute_u_cache(exx_ctx* c, const double2* psi);  // exx_api.cu: S1 for every band
 
 // ---- fused path (exx_fused.cu) ----

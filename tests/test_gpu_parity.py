@@ -433,3 +433,52 @@ def test_gpu_closed_form_single_plane_waves(B):
         assert g.get_info(B.EXX_INFO_PATH_USED) == 2
         assert abs(e - want) <= 1e-13 * abs(want)
     g.close()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# S8(f)-1: subspace matrix <c_i | V_x c_j> (exx_subspace, fp64 DMMA ZGEMM)
+@pytest.mark.parametrize("name", ["kpts_frac_occ", "noncubic_hse", "one_band"])
+def test_subspace_matrix_against_oracle_small(B, name):
+    w = _small(name)
+    o, g = _pair(B, w)
+    psi = w.coefficients(o.npw)
+    want_v = o.apply(psi, w.occ)
+    pd = g.to_device(psi)
+    out = g.apply(pd, w.occ)
+    for k in range(w.nk):
+        M = g.subspace(k, pd, out).cpu().numpy()
+        Mo = o.subspace(k, psi, want_v)
+        assert M.shape == (w.nbands, w.nbands)
+        assert np.abs(M - Mo).max() <= 1e-12 * max(np.abs(Mo).max(), 1e-300)
+    g.close()
+
+
+def test_subspace_matrix_C3_full_size(B):
+    """Full BASELINE size (64 bands, 15 895 plane waves; ragged: 64 = 8 tiles, npw not a multiple of 4): element-wise against
+    the oracle's triple loop on the GPU's own V_x psi, plus Hermiticity and the trace identity."""
+    w = W.make("C3")
+    o, g = _pair(B, w)
+    psi = w.coefficients(g.npw)
+    pd = g.to_device(psi)
+    out = g.apply(pd, w.occ)
+    e, _ = g.energy(pd, w.occ, out)
+    M = g.subspace(0, pd, out).cpu().numpy()
+    Mo = o.subspace(0, psi, out.cpu().numpy())
+    assert np.abs(M - Mo).max() <= 1e-13 * np.abs(Mo).max()
+    assert np.abs(M - M.conj().T).max() <= 1e-13 * np.abs(M).max()
+    assert abs(0.5 * np.diagonal(M).real.sum() - e) <= 1e-13 * abs(e)
+    g.close()
+
+
+def test_subspace_matrix_ragged_band_count(B):
+    # 5 and 13 bands: tiles of 8 with a ragged edge in both directions; random (non-V_x) right-hand side
+    import torch
+    for nb in (5, 13):
+        w = W.custom("rag", 9, (12, 12, 12), W.cubic(6.0), [[0, 0, 0], [0.5, 0, 0]], [0.5, 0.5], 4.0, nb, np.ones(nb))
+        o, g = _pair(B, w)
+        psi = w.coefficients(o.npw)
+        rhs = W.custom("rag2", 10, (12, 12, 12), W.cubic(6.0), [[0, 0, 0], [0.5, 0, 0]], [0.5, 0.5], 4.0, nb, np.ones(nb)).coefficients(o.npw)
+        for k in range(w.nk):
+            M = g.subspace(k, g.to_device(psi), g.to_device(rhs)).cpu().numpy()
+            assert np.abs(M - o.subspace(k, psi, rhs)).max() <= 1e-13
+        g.close()

@@ -460,6 +460,82 @@ EXX_HD void p3_flush_reg(int tid, const cplx* acc, cplx* __restrict__ accg, int 
 }
 
 // ================================================================================================================
+// Plain 3-D transforms with the same passes (S1: sphere coefficients -> u(r); S7: accumulator -> sphere coefficients).
+// Frequency-domain boxes live in the "F layout": what pass B holds after its forward x steps, written back tile by tile:
+//   findex(kx, ky, kz) = widx(k1y, kzpos, xpos, k2y) with xpos = 8 (kx mod R1) + kx div R1, kzpos = 8 (kz mod R1) + kz div R1,
+//   k1y = ky mod R1, k2y = ky div R1.
+// Forward  = pass A (one input, no product) + pass B forward half (y8, xR, x8)  -> F layout, then gather through findex.
+// Inverse  = scatter through findex, pass B inverse half (x8, xR, y8) + pass C without multiply/accumulate -> natural box.
+template <int R1>
+EXX_HD size_t findex(int kx, int ky, int kz) {
+    return widx<R1>(ky % R1, 8 * (kz % R1) + kz / R1, 8 * (kx % R1) + kx / R1, ky / R1);
+}
+
+template <int R1, int U, int NT>
+EXX_HD void p1_z1_single(int tid, const cplx* __restrict__ un, int x, int yb, cplx* S) {
+    constexpr int N = 8 * R1, NI = U * R1 * 8, IT = (NI + NT - 1) / NT;
+#pragma unroll
+    for (int i = 0; i < IT; i++) {
+        int it = tid + i * NT;
+        if (it < NI) {
+            int row = it >> 3, n2z = it & 7;
+            int u = row / R1, n1y = row - u * R1;
+            size_t base = ((size_t)x * N + (n1y * 8 + yb * U + u)) * N + n2z;
+            cplx v[R1];
+#pragma unroll
+            for (int j = 0; j < R1; j++) v[j] = un[base + j * 8];
+            dft<R1, -1>(v);
+#pragma unroll
+            for (int j = 0; j < R1; j++) S[sidx<R1>(u, n1y, j, n2z)] = v[j];
+        }
+    }
+}
+
+template <int R1, int Z, int NT, int SIGN>
+EXX_HD void p2_x8_half(int tid, cplx* S) {
+    // items (k1x, rem).  SIGN < 0: second forward x step only;  SIGN > 0: first inverse x step + conjugate twiddle
+    constexpr int NI = R1 * 8 * Z, IT = (NI + NT - 1) / NT, PX = P2Geo<Z>::PX;
+#pragma unroll
+    for (int i = 0; i < IT; i++) {
+        int it = tid + i * NT;
+        if (it < NI) {
+            int k1x = it / (8 * Z), rem = it - k1x * (8 * Z);
+            cplx v[8];
+#pragma unroll
+            for (int j = 0; j < 8; j++) v[j] = S[(k1x * 8 + j) * PX + rem];
+            dft<8, SIGN>(v);
+            if (SIGN > 0) {
+#pragma unroll
+                for (int j = 1; j < 8; j++) v[j] = mul_conj_b(v[j], EXX_TW(R1, j * k1x));
+            }
+#pragma unroll
+            for (int j = 0; j < 8; j++) S[(k1x * 8 + j) * PX + rem] = v[j];
+        }
+    }
+}
+
+template <int R1, int U, int NT>
+EXX_HD void p3_zinv2_store(int tid, const cplx* S, cplx* __restrict__ out, int x, int yb) {
+    // last inverse z step, stored to a natural-order box (no multiply, no accumulation)
+    constexpr int N = 8 * R1, NI = U * R1 * 8, IT = (NI + NT - 1) / NT;
+#pragma unroll
+    for (int i = 0; i < IT; i++) {
+        int it = tid + i * NT;
+        if (it < NI) {
+            int row = it >> 3, n2z = it & 7;
+            int u = row / R1, n1y = row - u * R1;
+            size_t base = ((size_t)x * N + (n1y * 8 + yb * U + u)) * N + n2z;
+            cplx v[R1];
+#pragma unroll
+            for (int j = 0; j < R1; j++) v[j] = S[sidx<R1>(u, n1y, j, n2z)];
+            dft<R1, +1>(v);
+#pragma unroll
+            for (int j = 0; j < R1; j++) out[base + j * 8] = v[j];
+        }
+    }
+}
+
+// ================================================================================================================
 // Host side of the layout: K' in natural C order -> the order pass B reads it in,
 //   [k1y][zb][k1x][k2y][kzl][k2x]  with kx = k1x + R1 k2x, ky = k1y + R1 k2y, zpos = zb Z + kzl = 8 k1z + k2z, kz = k1z + R1 k2z.
 inline void permute_ktable(int R1, int Z, const double* nat, double* perm) {

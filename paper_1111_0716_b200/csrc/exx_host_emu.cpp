@@ -2,6 +2,7 @@
 // tile by tile, exactly as exx_fused.cu schedules them on the device.  Built only by tests/test_fused_host_emulation.py
 // (g++, no CUDA); it lets the index/layout logic of the kernels be checked without a GPU.  Not part of libexx.so.
 #include <math.h>
+#include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
 
@@ -83,6 +84,66 @@ static void emu_pair(const cplx* un, const cplx* um, const double* Knat, double 
             }
         }
 }
+
+// plain 3-D transforms through the fused passes.  sign < 0: natural box `in` -> F-layout box `out`;
+// sign > 0: F-layout box `in` (modified in place by the pass-B half) -> natural box `out`
+template <int R1>
+static void emu_fft(int sign, cplx* in, cplx* out) {
+    typedef FusedCfg<R1> C;
+    constexpr int N = 8 * R1, U = C::U1, NT13 = C::NT1, U3 = C::U3, NT3 = C::NT3, Z = C::Z, NT2 = C::NT2;
+    constexpr bool TWREG = C::TWREG;
+    std::vector<cplx> S((size_t)(U > U3 ? U : U3) * R1 * N), T(R1 * 8), S2((size_t)N * P2Geo<Z>::PX);
+    for (int k = 0; k < R1; k++)
+        for (int j = 0; j < 8; j++) T[tidx(k, j)] = EXX_TW(R1, j * k);
+    if (sign < 0) {
+        for (int x = 0; x < N; x++)
+            for (int yb = 0; yb < 8 / U; yb++) {
+                for (int t = 0; t < NT13; t++) p1_z1_single<R1, U, NT13>(t, in, x, yb, S.data());
+                for (int t = 0; t < NT13; t++) {
+                    cplx twr[8];
+                    load_twr<R1>(t, twr);
+                    p13_z8<R1, U, NT13, -1, TWREG>(t, S.data(), T.data(), twr);
+                }
+                for (int t = 0; t < NT13; t++) p1_y1<R1, U, NT13>(t, S.data(), out, x, yb);
+            }
+        for (int k1y = 0; k1y < R1; k1y++)
+            for (int zb = 0; zb < N / Z; zb++) {
+                cplx* Wt = out + ((size_t)k1y * (N / Z) + zb) * ((size_t)N * 8 * Z);
+                p2_copy_rows<R1, Z>(S2.data(), Wt, true);
+                for (int t = 0; t < NT2; t++) p2_y8<R1, Z, NT2, -1>(t, S2.data(), k1y);
+                for (int t = 0; t < NT2; t++) p2_xR<R1, Z, NT2, -1>(t, S2.data());
+                for (int t = 0; t < NT2; t++) p2_x8_half<R1, Z, NT2, -1>(t, S2.data());
+                p2_copy_rows<R1, Z>(S2.data(), Wt, false);
+            }
+    } else {
+        for (int k1y = 0; k1y < R1; k1y++)
+            for (int zb = 0; zb < N / Z; zb++) {
+                cplx* Wt = in + ((size_t)k1y * (N / Z) + zb) * ((size_t)N * 8 * Z);
+                p2_copy_rows<R1, Z>(S2.data(), Wt, true);
+                for (int t = 0; t < NT2; t++) p2_x8_half<R1, Z, NT2, +1>(t, S2.data());
+                for (int t = 0; t < NT2; t++) p2_xR<R1, Z, NT2, +1>(t, S2.data());
+                for (int t = 0; t < NT2; t++) p2_y8<R1, Z, NT2, +1>(t, S2.data(), k1y);
+                p2_copy_rows<R1, Z>(S2.data(), Wt, false);
+            }
+        for (int x = 0; x < N; x++)
+            for (int yb = 0; yb < 8 / U3; yb++) {
+                for (int t = 0; t < NT3; t++) p3_y2inv<R1, U3, NT3>(t, in, x, yb, S.data());
+                for (int t = 0; t < NT3; t++) {
+                    cplx twr[8];
+                    load_twr<R1>(t, twr);
+                    p13_z8<R1, U3, NT3, +1, TWREG>(t, S.data(), T.data(), twr);
+                }
+                for (int t = 0; t < NT3; t++) p3_zinv2_store<R1, U3, NT3>(t, S.data(), out, x, yb);
+            }
+    }
+}
+template <int R1>
+static void emu_findex(int64_t* idx) {
+    constexpr int N = 8 * R1;
+    for (int kx = 0; kx < N; kx++)
+        for (int ky = 0; ky < N; ky++)
+            for (int kz = 0; kz < N; kz++) idx[((size_t)kx * N + ky) * N + kz] = (int64_t)findex<R1>(kx, ky, kz);
+}
 }  // namespace exx
 
 using namespace exx;
@@ -117,5 +178,21 @@ int exx_emu_pair(int R1, const double* un, const double* um, const double* Knat,
     case 16: emu_pair<16>((const cplx*)un, (const cplx*)um, Knat, wf, (cplx*)acc, (cplx*)work); return 0;
     default: return -1;
     }
+}
+
+// plain 3-D transform through the fused passes (see emu_fft); findex_out (optional, N^3 int64) receives the F-layout index of
+// every natural frequency index
+int exx_emu_fft(int R1, int sign, double* in, double* out, int64_t* findex_out) {
+    fill_tw();
+#define CASE(r)                                         \
+    case r:                                             \
+        emu_fft<r>(sign, (cplx*)in, (cplx*)out);        \
+        if (findex_out) emu_findex<r>(findex_out);      \
+        return 0;
+    switch (R1) {
+        CASE(6) CASE(8) CASE(9) CASE(12) CASE(16)
+    default: return -1;
+    }
+#undef CASE
 }
 }

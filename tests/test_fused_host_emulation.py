@@ -78,3 +78,26 @@ def test_single_plane_wave_pair(emu):
     d = [(a - b) % N for a, b in zip(gn, gm)]
     want = -K[d[0], d[1], d[2]] * N ** 3 * un
     assert np.abs(acc - want).max() <= 1e-12 * N ** 3
+
+
+@pytest.mark.parametrize("R1", [6, 8, 9, 12])
+def test_plain_transforms_through_the_passes(emu, R1):
+    """S1/S7 use the fused passes as plain 3-D transforms: forward natural -> F layout, inverse F layout -> natural."""
+    N = 8 * R1
+    emu.exx_emu_fft.argtypes = [C.c_int, C.c_int, dp, dp, C.POINTER(C.c_int64)]
+    rng = np.random.default_rng(40 + R1)
+    x = rng.standard_normal((N, N, N)) + 1j * rng.standard_normal((N, N, N))
+    fidx = np.empty(N ** 3, dtype=np.int64)
+    out = np.zeros(N ** 3, dtype=np.complex128)
+    assert emu.exx_emu_fft(R1, -1, _p(x.copy()), _p(out), fidx.ctypes.data_as(C.POINTER(C.c_int64))) == 0
+    assert np.array_equal(np.sort(fidx), np.arange(N ** 3))      # findex is a permutation of the box
+    want = np.fft.fftn(x).reshape(-1)
+    assert np.linalg.norm(out[fidx] - want) <= 1e-14 * np.linalg.norm(want)
+    # inverse: scatter natural-order coefficients through findex, transform back
+    y = rng.standard_normal((N, N, N)) + 1j * rng.standard_normal((N, N, N))
+    f = np.zeros(N ** 3, dtype=np.complex128)
+    f[fidx] = y.reshape(-1)
+    back = np.zeros(N ** 3, dtype=np.complex128)
+    assert emu.exx_emu_fft(R1, +1, _p(f), _p(back), None) == 0
+    want = np.fft.ifftn(y).reshape(-1) * N ** 3
+    assert np.linalg.norm(back - want) <= 1e-14 * np.linalg.norm(want)

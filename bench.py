@@ -118,7 +118,7 @@ def run_reference(args, rank, world):
 # a generic box pass reads and writes one complex128 box (32 Ng); each fused pass moves 32 Ng per pair (96 Ng for the
 # three passes = the B_model of the pair evaluation).
 BYTES_PER_UNIT_NG = {"fft_axis_generic": 32, "codensity": 32, "kernel_multiply": 32, "accumulate": 32,
-                     "fused_pass_a": 32, "fused_pass_b": 32, "fused_pass_c": 32, "scatter": 16, "gather": 16}
+                     "fused_pass_a": 32, "fused_pass_b": 32, "fused_pass_c": 32, "fused_fft_pass": 32, "scatter": 16, "gather": 16}
 
 
 def run_ours(args, rank, world, local):
@@ -208,7 +208,7 @@ def run_ours(args, rank, world, local):
     # the pipeline figure: every fused pass execution moves 32 bytes per transformed grid point (read 16 + write
     # 16, or read pair box + read u for pass C); an ordered pair without symmetry = passes A + B + C = B_model = 96 B/pt.  With
     # the pair symmetry an executed pair is A + B + up to two C sweeps, so the bytes are counted per pass execution.
-    pass_units = sum(acc[k][2] for k in ("fused_pass_a", "fused_pass_b", "fused_pass_c") if k in acc) / args.steps
+    pass_units = sum(acc[k][2] for k in ("fused_pass_a", "fused_pass_b", "fused_pass_c", "fused_fft_pass") if k in acc) / args.steps
     if pass_units == 0:  # generic path: 9 box passes per pair
         pass_units = sum(acc[k][2] for k in ("fft_axis_generic", "codensity", "kernel_multiply", "accumulate") if k in acc) / args.steps
     pipe_bytes = 32.0 * ngw * pass_units

@@ -47,7 +47,7 @@ LaunchScope::~LaunchScope() {
 }
 
 static const char* kclass_names[KC_COUNT] = {"scatter", "gather", "fft_axis_generic", "codensity", "kernel_multiply",
-                                             "accumulate", "energy", "fused_pass_a", "fused_pass_b", "fused_pass_c", "subspace_zgemm"};
+                                             "accumulate", "energy", "fused_pass_a", "fused_pass_b", "fused_pass_c", "subspace_zgemm", "fused_fft_pass"};
 
 // ---- host arithmetic of S0 (index maps, kernel tables).  Evaluation order of |t.B|^2 is fixed (A11). ----
 static inline int fold(int j, int n) { return (2 * j < n) ? j : j - n; }

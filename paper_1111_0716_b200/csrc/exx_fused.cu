@@ -21,6 +21,7 @@ cplx h_tw[TW_TOTAL];  // host copy (source of the constant-memory upload)
 struct FusedState {
     int R1 = 0;
     double* kperm_dev = nullptr;  // ntab tables, permuted order of pass B
+    int32_t* fmap_dev = nullptr;  // per k: F-layout index of every sphere vector (offsets = exx_ctx::map_off)
     int tn = 0, tm = 0;
 };
 
@@ -187,6 +188,93 @@ __global__ void __launch_bounds__(FusedCfg<R1>::NT3, FusedCfg<R1>::MINB3) pass_c
     }
 }
 
+// ---- plain 3-D transforms through the same passes (S1, S7; F layout, see exx_fused_phases.h) ------------------------
+// forward first half: natural box p of in_base -> work box p (z transform, first y step)
+template <int R1>
+__global__ void __launch_bounds__(FusedCfg<R1>::NT1, FusedCfg<R1>::MINB1) fft_a_kernel(const cplx* __restrict__ in_base, int nbox, cplx* __restrict__ work) {
+    constexpr int N = 8 * R1, U = FusedCfg<R1>::U1, NT = FusedCfg<R1>::NT1;
+    constexpr bool TWREG = FusedCfg<R1>::TWREG;
+    constexpr size_t Ng = (size_t)N * N * N;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* S = reinterpret_cast<cplx*>(smem_raw);
+    cplx* T = S + U * R1 * N;
+    const int tid = threadIdx.x;
+    const int p = blockIdx.x % nbox, tile = blockIdx.x / nbox;
+    const int x = tile / (8 / U), yb = tile % (8 / U);
+    cplx twr[8];
+    if (TWREG)
+        load_twr<R1>(tid, twr);
+    else
+        for (int i = tid; i < R1 * 8; i += NT) T[tidx(i >> 3, i & 7)] = c_tw[TwOff<R1>::v + (i >> 3) * (i & 7)];
+    p1_z1_single<R1, U, NT>(tid, in_base + (size_t)p * Ng, x, yb, S);
+    __syncthreads();
+    p13_z8<R1, U, NT, -1, TWREG>(tid, S, T, twr);
+    __syncthreads();
+    p1_y1<R1, U, NT>(tid, S, work + (size_t)p * Ng, x, yb);
+}
+
+// the pass-B half, in place on work box p.  SIGN < 0: second y step, forward x (-> F layout); SIGN > 0: inverse x, first
+// inverse y step (F layout ->)
+template <int R1, int SIGN>
+__global__ void __launch_bounds__(FusedCfg<R1>::NT2, FusedCfg<R1>::MINB2) fft_b_kernel(cplx* __restrict__ work, int nbox) {
+    constexpr int N = 8 * R1, Z = FusedCfg<R1>::Z, NT = FusedCfg<R1>::NT2, PX = P2Geo<Z>::PX;
+    constexpr size_t Ng = (size_t)N * N * N;
+    constexpr uint32_t ROWB = 8 * Z * sizeof(cplx);
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* S = reinterpret_cast<cplx*>(smem_raw);
+    __shared__ __align__(8) uint64_t bar;
+    const int tid = threadIdx.x;
+    const int p = blockIdx.x % nbox, tile = blockIdx.x / nbox;
+    const int k1y = tile / (N / Z);
+    cplx* Wt = work + (size_t)p * Ng + (size_t)tile * ((size_t)N * 8 * Z);
+    if (tid == 0) mbar_init(&bar, 1);
+    __syncthreads();
+    if (tid == 0) mbar_arrive_expect_tx(&bar, ROWB * N);
+    for (int x = tid; x < N; x += NT) bulk_g2s(S + x * PX, Wt + x * 8 * Z, ROWB, &bar);
+    mbar_wait(&bar, 0);
+    if (SIGN < 0) {
+        p2_y8<R1, Z, NT, -1>(tid, S, k1y);
+        __syncthreads();
+        p2_xR<R1, Z, NT, -1>(tid, S);
+        __syncthreads();
+        p2_x8_half<R1, Z, NT, -1>(tid, S);
+    } else {
+        p2_x8_half<R1, Z, NT, +1>(tid, S);
+        __syncthreads();
+        p2_xR<R1, Z, NT, +1>(tid, S);
+        __syncthreads();
+        p2_y8<R1, Z, NT, +1>(tid, S, k1y);
+    }
+    fence_proxy_async_smem();
+    __syncthreads();
+    for (int x = tid; x < N; x += NT) bulk_s2g(Wt + x * 8 * Z, S + x * PX, ROWB);
+    bulk_commit_wait_all();
+}
+
+// inverse second half: work box p -> natural box p of out_base (second inverse y step, inverse z)
+template <int R1>
+__global__ void __launch_bounds__(FusedCfg<R1>::NT3, FusedCfg<R1>::MINB3) fft_c_kernel(const cplx* __restrict__ work, int nbox, cplx* __restrict__ out_base) {
+    constexpr int N = 8 * R1, U = FusedCfg<R1>::U3, NT = FusedCfg<R1>::NT3;
+    constexpr bool TWREG = FusedCfg<R1>::TWREG;
+    constexpr size_t Ng = (size_t)N * N * N;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* S = reinterpret_cast<cplx*>(smem_raw);
+    cplx* T = S + U * R1 * N;
+    const int tid = threadIdx.x;
+    const int p = blockIdx.x % nbox, tile = blockIdx.x / nbox;
+    const int x = tile / (8 / U), yb = tile % (8 / U);
+    cplx twr[8];
+    if (TWREG)
+        load_twr<R1>(tid, twr);
+    else
+        for (int i = tid; i < R1 * 8; i += NT) T[tidx(i >> 3, i & 7)] = c_tw[TwOff<R1>::v + (i >> 3) * (i & 7)];
+    p3_y2inv<R1, U, NT>(tid, work + (size_t)p * Ng, x, yb, S);
+    __syncthreads();
+    p13_z8<R1, U, NT, +1, TWREG>(tid, S, T, twr);
+    __syncthreads();
+    p3_zinv2_store<R1, U, NT>(tid, S, out_base + (size_t)p * Ng, x, yb);
+}
+
 // ---------------------------------------------------------------------------------------------------------------
 template <int R1>
 struct Launch {
@@ -200,6 +288,10 @@ struct Launch {
         EXX_CUDA(c, cudaFuncSetAttribute(pass_a_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a));
         EXX_CUDA(c, cudaFuncSetAttribute(pass_b_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b));
         EXX_CUDA(c, cudaFuncSetAttribute(pass_c_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_c));
+        EXX_CUDA(c, cudaFuncSetAttribute(fft_a_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a));
+        EXX_CUDA(c, cudaFuncSetAttribute((fft_b_kernel<R1, -1>), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b));
+        EXX_CUDA(c, cudaFuncSetAttribute((fft_b_kernel<R1, +1>), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b));
+        EXX_CUDA(c, cudaFuncSetAttribute(fft_c_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_c));
         return EXX_OK;
     }
     // passes A and B over the pairs of one batch
@@ -215,6 +307,39 @@ struct Launch {
         }
         EXX_CUDA(c, cudaGetLastError());
         return EXX_OK;
+    }
+    // plain transforms of nbox boxes: forward natural in -> F layout in work; inverse F layout in work -> natural out
+    static int fft_forward(exx_ctx* c, const cplx* in_base, int nbox, cplx* work) {
+        const unsigned tiles1 = N * (8 / U1), tiles2 = R1 * (N / Z);
+        {
+            LaunchScope ls(c, KC_FFT_FUSED, nbox);
+            fft_a_kernel<R1><<<tiles1 * nbox, FusedCfg<R1>::NT1, smem_a, c->stream>>>(in_base, nbox, work);
+        }
+        {
+            LaunchScope ls(c, KC_FFT_FUSED, nbox);
+            fft_b_kernel<R1, -1><<<tiles2 * nbox, FusedCfg<R1>::NT2, smem_b, c->stream>>>(work, nbox);
+        }
+        EXX_CUDA(c, cudaGetLastError());
+        return EXX_OK;
+    }
+    static int fft_inverse(exx_ctx* c, cplx* work, int nbox, cplx* out_base) {
+        const unsigned tiles3 = N * (8 / U3), tiles2 = R1 * (N / Z);
+        {
+            LaunchScope ls(c, KC_FFT_FUSED, nbox);
+            fft_b_kernel<R1, +1><<<tiles2 * nbox, FusedCfg<R1>::NT2, smem_b, c->stream>>>(work, nbox);
+        }
+        {
+            LaunchScope ls(c, KC_FFT_FUSED, nbox);
+            fft_c_kernel<R1><<<tiles3 * nbox, FusedCfg<R1>::NT3, smem_c, c->stream>>>(work, nbox, out_base);
+        }
+        EXX_CUDA(c, cudaGetLastError());
+        return EXX_OK;
+    }
+    static void fill_fmap(const int32_t* nat, int n, int32_t* out) {
+        for (int i = 0; i < n; i++) {
+            int j = nat[i];
+            out[i] = (int32_t)findex<R1>(j / (N * N), (j / N) % N, j % N);
+        }
     }
     // one accumulation sweep (pass C)
     static int pass_c(exx_ctx* c, const cplx* usrc_base, const CJob& job, int64_t units, const cplx* work, cplx* acc_base) {
@@ -290,6 +415,16 @@ int fused_create(exx_ctx* c) {
         permute_ktable(st->R1, Z, nat.data(), perm.data());
         EXX_CUDA(c, cudaMemcpy(st->kperm_dev + (size_t)t * Ng, perm.data(), sizeof(double) * Ng, cudaMemcpyHostToDevice));
     }
+    // sphere -> F layout maps for S1 / S7
+    if (cudaMalloc((void**)&st->fmap_dev, sizeof(int32_t) * (size_t)std::max<int64_t>(1, c->map_off[c->nk])) != cudaSuccess) {
+        cudaGetLastError();
+        return EXX_ERR_ALLOC;
+    }
+    for (int k = 0; k < c->nk; k++) {
+        std::vector<int32_t> fm(c->npw[k]);
+        EXX_DISPATCH_R1(st->R1, L::fill_fmap(c->map_h[k].data(), c->npw[k], fm.data()));
+        EXX_CUDA(c, cudaMemcpy(st->fmap_dev + c->map_off[k], fm.data(), sizeof(int32_t) * c->npw[k], cudaMemcpyHostToDevice));
+    }
     int rc = EXX_OK;
     EXX_DISPATCH_R1(st->R1, rc = L::init(c));
     return rc;
@@ -299,6 +434,7 @@ void fused_destroy(exx_ctx* c) {
     FusedState* st = (FusedState*)c->fused;
     if (!st) return;
     cudaFree(st->kperm_dev);
+    cudaFree(st->fmap_dev);
     delete st;
     c->fused = nullptr;
 }
@@ -318,7 +454,16 @@ int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out)
     const size_t Ng = (size_t)c->Ng;
     c->path_used = 2;
     c->pruned_used = 0;
-    if ((rc = compute_u_cache(c, psi))) return rc;
+    // S1: sphere coefficients -> F-layout work boxes (scatter) -> inverse transform through passes B/C -> u cache
+    for (int k = 0; k < nk; k++) {
+        const int bmax = (int)std::min<size_t>(c->work_boxes, (size_t)nb);
+        for (int n0 = 0; n0 < nb; n0 += bmax) {
+            const int bn = std::min(bmax, nb - n0);
+            if ((rc = launch_scatter(c, k, psi + c->off[k] + (int64_t)n0 * c->npw[k], bn, (double2*)c->work_dev, st->fmap_dev + c->map_off[k]))) return rc;
+            EXX_DISPATCH_R1(st->R1, rc = L::fft_inverse(c, (cplx*)c->work_dev, bn, (cplx*)c->u_dev + ((size_t)k * nb + n0) * Ng));
+            if (rc) return rc;
+        }
+    }
     int ta_max = 16, tb_max = 16;
     while ((size_t)ta_max * tb_max > c->work_boxes && tb_max > 1) tb_max /= 2;
     while ((size_t)ta_max * tb_max > c->work_boxes && ta_max > 1) ta_max /= 2;
@@ -460,14 +605,14 @@ int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out)
                     }
                 }
         }
-    // S7: forward transform of every accumulator, gather onto sphere(k) (in batches that keep launches below 2^28 elements)
+    // S7: forward transform of every accumulator through passes A/B (-> F layout), gather onto sphere(k)
     for (int k = 0; k < nk; k++) {
-        int bmax = (int)std::max<int64_t>(1, std::min<int64_t>(nb, ((int64_t)1 << 28) / (int64_t)Ng));
+        const int bmax = (int)std::min<size_t>(c->work_boxes, (size_t)nb);
         for (int n0 = 0; n0 < nb; n0 += bmax) {
-            int bn = std::min(bmax, nb - n0);
-            double2* box = (double2*)acc + ((size_t)k * nb + n0) * Ng;
-            if ((rc = launch_fft3d_generic(c, box, bn, -1))) return rc;
-            if ((rc = launch_gather(c, k, box, bn, out + c->off[k] + (int64_t)n0 * c->npw[k]))) return rc;
+            const int bn = std::min(bmax, nb - n0);
+            EXX_DISPATCH_R1(st->R1, rc = L::fft_forward(c, acc + ((size_t)k * nb + n0) * Ng, bn, work));
+            if (rc) return rc;
+            if ((rc = launch_gather(c, k, (const double2*)work, bn, out + c->off[k] + (int64_t)n0 * c->npw[k], st->fmap_dev + c->map_off[k]))) return rc;
         }
     }
     return EXX_OK;

@@ -25,7 +25,8 @@ enum KClass {
     KC_PASS_B = 8,       // fused: forward x, K', inverse x
     KC_PASS_C = 9,       // fused: inverse (y,z)-plane transform, times f_m u_m, accumulate
     KC_SUBSPACE = 10,    // subspace ZGEMM (DMMA) + its slice reduction
-    KC_COUNT = 11
+    KC_FFT_FUSED = 11,   // plain 3-D transforms (S1, S7) through the fused passes; unit = one box pass
+    KC_COUNT = 12
 };
 
 struct Plan1D {
@@ -151,8 +152,8 @@ struct CJob {
     unsigned char col[16][16];
 };
 int fft_generic_init(exx_ctx* c);
-int launch_scatter(exx_ctx* c, int ik, const double2* coef, int nbatch, double2* box);
-int launch_gather(exx_ctx* c, int ik, const double2* box, int nbatch, double2* coef);
+int launch_scatter(exx_ctx* c, int ik, const double2* coef, int nbatch, double2* box, const int32_t* map = nullptr);  // map: override (F layout)
+int launch_gather(exx_ctx* c, int ik, const double2* box, int nbatch, double2* coef, const int32_t* map = nullptr);
 int launch_fft3d_generic(exx_ctx* c, double2* box, int nbatch, int sign);
 int launch_codensity_tile(exx_ctx* c, const double2* un_base, int n0, int tn, const double2* uq_base, const MTile& mt, double2* work);
 int launch_kmul(exx_ctx* c, const double* ktab, double2* work, int nboxes);

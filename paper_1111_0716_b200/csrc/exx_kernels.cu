@@ -32,25 +32,27 @@ __global__ void gather_kernel(const double2* __restrict__ box, const int32_t* __
         coef[(int64_t)b * npw + ig] = box[(int64_t)b * Ng + map[ig]];
 }
 
-int launch_scatter(exx_ctx* c, int ik, const double2* coef, int nbatch, double2* box) {
+int launch_scatter(exx_ctx* c, int ik, const double2* coef, int nbatch, double2* box, const int32_t* map) {
+    if (!map) map = c->map_dev + c->map_off[ik];
     EXX_CUDA(c, cudaMemsetAsync(box, 0, sizeof(double2) * (size_t)c->Ng * nbatch, c->stream));
     int npw = c->npw[ik];
     for (int b0 = 0; b0 < nbatch; b0 += 32768) {
         int nb = nbatch - b0 < 32768 ? nbatch - b0 : 32768;
         LaunchScope ls(c, KC_SCATTER, nb);
         dim3 grid((npw + 255) / 256, nb);
-        scatter_kernel<<<grid, 256, 0, c->stream>>>(coef + (int64_t)b0 * npw, c->map_dev + c->map_off[ik], npw, c->Ng, box + (int64_t)b0 * c->Ng);
+        scatter_kernel<<<grid, 256, 0, c->stream>>>(coef + (int64_t)b0 * npw, map, npw, c->Ng, box + (int64_t)b0 * c->Ng);
     }
     EXX_CUDA(c, cudaGetLastError());
     return EXX_OK;
 }
-int launch_gather(exx_ctx* c, int ik, const double2* box, int nbatch, double2* coef) {
+int launch_gather(exx_ctx* c, int ik, const double2* box, int nbatch, double2* coef, const int32_t* map) {
+    if (!map) map = c->map_dev + c->map_off[ik];
     int npw = c->npw[ik];
     for (int b0 = 0; b0 < nbatch; b0 += 32768) {
         int nb = nbatch - b0 < 32768 ? nbatch - b0 : 32768;
         LaunchScope ls(c, KC_GATHER, nb);
         dim3 grid((npw + 255) / 256, nb);
-        gather_kernel<<<grid, 256, 0, c->stream>>>(box + (int64_t)b0 * c->Ng, c->map_dev + c->map_off[ik], npw, c->Ng, coef + (int64_t)b0 * npw);
+        gather_kernel<<<grid, 256, 0, c->stream>>>(box + (int64_t)b0 * c->Ng, map, npw, c->Ng, coef + (int64_t)b0 * npw);
     }
     EXX_CUDA(c, cudaGetLastError());
     return EXX_OK;

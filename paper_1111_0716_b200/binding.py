@@ -43,6 +43,15 @@ def lib():
     """Load libexx.so (built in-tree by paper_1111_0716_b200.build).  Raises if it is missing: no fallback."""
     global _lib
     if _lib is None:
+        if not os.environ.get("EXX_LIB"):
+            # compile (or re-compile after a source change) the CUDA library in-tree; compiling is not a fallback path:
+            # if nvcc or the sources are missing this raises, and nothing else can compute
+            try:
+                from . import build as _build
+                _build.build()
+            except Exception as e:  # noqa: BLE001
+                if not os.path.exists(LIB_PATH):
+                    raise RuntimeError("libexx.so is missing and could not be built (%s); there is no CPU fallback" % e)
         if not os.path.exists(LIB_PATH):
             raise RuntimeError("libexx.so not found at %s: build it with `python -m paper_1111_0716_b200.build` "
                                "(there is no CPU fallback)" % LIB_PATH)

@@ -517,3 +517,26 @@ def test_fused_ragged_tiles_and_occupation_holes(B, tile):
     again = g.apply(pd, w.occ).cpu().numpy()
     assert np.array_equal(again.view(np.float64), res[0].view(np.float64))
     g.close()
+
+
+def test_fused_128_full_grid_against_live_oracle(B):
+    """The N = 128 (R1 = 16) instantiation of the fused passes, which the default (compact-grid) runs of C5 never use: a C5-shaped
+    cell with 3 bands on the caller's full 128^3 grid (EXX_OPT_PRUNE = 0), both symmetry modes, against the oracle run now."""
+    w = W.custom("c5_small", 555, (128, 128, 128), W.cubic(30.0), [[0, 0, 0]], [1.0], 10.0, 3, [1.0, 0.5, 0.0], kernel_kind=1, mu=0.106)
+    o, g = _pair(B, w)
+    assert g.get_info(B.EXX_INFO_COMPACT_GRID) == 96
+    psi = w.coefficients(o.npw)
+    want = o.apply(psi, w.occ)
+    e_want, _ = o.energy(psi, w.occ, want)
+    pd = g.to_device(psi)
+    g.set_option(B.EXX_OPT_PRUNE, 0)
+    for sym in (1, 0):
+        g.set_option(B.EXX_OPT_SYMMETRY, sym)
+        out = g.apply(pd, w.occ)
+        assert g.get_info(B.EXX_INFO_WORK_GRID) == 128 and g.get_info(B.EXX_INFO_PATH_USED) == 2
+        got = out.cpu().numpy()
+        for n in range(w.nbands):
+            assert _rel(o.band(got, 0, n), o.band(want, 0, n)) < TOL_VX, (sym, n)
+        e, _ = g.energy(pd, w.occ, out)
+        assert abs(e - e_want) <= TOL_EX * abs(e_want)
+    g.close()

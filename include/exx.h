@@ -70,6 +70,10 @@ enum {
     EXX_OPT_PRUNE = 4,      /* 1 (default): run the pair pipeline on the compact work grid when there is one (see EXX_INFO_COMPACT_GRID);
                                0: always transform the caller's full grid */
     EXX_OPT_PROFILE = 5,    /* 1: bracket every kernel launch with CUDA events so exx_get_kernel_time works (slower) */
+    EXX_OPT_PRECISION = 8,  /* 0 (default): fp64 throughout.  1: mixed precision, the paper's second mode ("some or all of the
+                               FFTs in single precision"): the pair transforms, the kernel multiply and the product with u_m run in fp32
+                               (fused path only); S1, S7, every accumulator and E_x stay fp64.  Agrees with fp64 to ~1e-6 relative
+                               (the paper reports 1e-5); NOT covered by the 1e-10 / 1e-11 parity bars */
     EXX_OPT_SYMMETRY = 6    /* 1 (default): evaluate each unordered band pair once and use v_{mq,nk} = conj(v_{nk,mq}) for the second
                                accumulation (fused path on alias-free grids only; see EXX_INFO_SYMMETRY); 0: every ordered pair */
 };
@@ -88,6 +92,7 @@ enum {
     EXX_INFO_NUM_KERNEL_CLASSES = 10,  /* how many kernel classes exx_get_kernel_time knows (the value, not this enum) */
     EXX_INFO_WORK_GRID = 11,      /* N of the (cubic) grid the last apply transformed; first axis of the caller's grid if not compacted */
     EXX_INFO_SYMMETRY = 13,       /* 1 if the last apply used the pair symmetry (then PAIRS_EXECUTED < PAIRS_ORDERED) */
+    EXX_INFO_PRECISION = 15,      /* 0 fp64, 1 mixed: what the last apply ran in */
     EXX_INFO_COMPACT_GRID = 12    /* (no apply needed) N of the compact work grid, 0 if none: the smallest supported cubic grid with
                                      N >= 4 max|g_i| + 1, used when it is smaller than the caller's box and the caller's box is itself
                                      alias-free (N_i >= 4 max|g_i| + 1).  Then no product the method forms wraps around on either grid and

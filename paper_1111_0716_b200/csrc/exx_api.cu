@@ -459,6 +459,10 @@ int exx_set_option(exx_ctx* c, int option, int64_t value) {
     case EXX_OPT_SYMMETRY:
         c->opt_symmetry = value ? 1 : 0;
         return EXX_OK;
+    case EXX_OPT_PRECISION:
+        if (value != 0 && value != 1) return EXX_ERR_BAD_ARG;
+        c->opt_precision = value;
+        return EXX_OK;
     default: return EXX_ERR_BAD_ARG;
     }
 }
@@ -471,6 +475,7 @@ int exx_get_option(const exx_ctx* c, int option, int64_t* value) {
     case EXX_OPT_PRUNE: *value = c->opt_prune; return EXX_OK;
     case EXX_OPT_PROFILE: *value = c->opt_profile; return EXX_OK;
     case EXX_OPT_SYMMETRY: *value = c->opt_symmetry; return EXX_OK;
+    case EXX_OPT_PRECISION: *value = c->opt_precision; return EXX_OK;
     default: return EXX_ERR_BAD_ARG;
     }
 }
@@ -489,6 +494,7 @@ int exx_get_info(const exx_ctx* c, int what, int64_t* value) {
     case EXX_INFO_TILE_M: *value = c->tile_m_used; return EXX_OK;
     case EXX_INFO_PRUNED: *value = c->pruned_used; return EXX_OK;
     case EXX_INFO_SYMMETRY: *value = c->symmetry_used; return EXX_OK;
+    case EXX_INFO_PRECISION: *value = c->precision_used; return EXX_OK;
     case EXX_INFO_NUM_KERNEL_CLASSES: *value = KC_COUNT; return EXX_OK;
     default: return EXX_ERR_BAD_ARG;
     }
@@ -549,6 +555,7 @@ static void reset_counters(exx_ctx* c) {
     c->event_pool_used = 0;
     c->pairs_ordered = c->pairs_executed = 0;
     c->symmetry_used = 0;
+    c->precision_used = 0;
 }
 
 // Generic pipeline, steps S1..S7 as separate kernels.
@@ -606,6 +613,7 @@ static int apply_impl(exx_ctx* c, const double2* psi, const double* occ, double2
         in->opt_tile_m = c->opt_tile_m;
         in->opt_profile = c->opt_profile;
         in->opt_symmetry = c->opt_symmetry;
+        in->opt_precision = c->opt_precision;
         int rc = apply_impl(in, psi, occ, out);
         c->launches = in->launches;
         c->pairs_ordered = in->pairs_ordered;
@@ -614,6 +622,7 @@ static int apply_impl(exx_ctx* c, const double2* psi, const double* occ, double2
         c->tile_n_used = in->tile_n_used;
         c->tile_m_used = in->tile_m_used;
         c->symmetry_used = in->symmetry_used;
+        c->precision_used = in->precision_used;
         c->pruned_used = 1;
         c->last_pruned = 1;
         if (rc) c->last_error = in->last_error;

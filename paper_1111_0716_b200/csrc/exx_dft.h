@@ -5,21 +5,31 @@
 // Convention: dft_fwd<R>(v) replaces v[0..R) by X[k] = sum_n v[n] exp(-2 pi i n k / R), natural order in and out
 // (the forward sign of S3).  dft<R,+1> is the unnormalised inverse (S5), obtained by swapping
 // real and imaginary parts around the forward codelet (register renaming, no arithmetic).
-#pragma once
-
+//
+// The header is written against the scalar type `real` of the enclosing mode: it may be included once per mode, each time
+// with EXX_NS (namespace) and EXX_REAL (double or float) defined — the fp64 product path uses exx / double; the mixed-precision
+// pair pipeline includes it a second time as exx32 / float.
+#ifndef EXX_HD
 #if defined(__CUDACC__)
 #define EXX_HD __host__ __device__ __forceinline__
 #else
 #define EXX_HD inline
 #endif
+#endif
+#ifndef EXX_NS
+#define EXX_NS exx
+#define EXX_REAL double
+#endif
+#define EXX_RC(x) ((real)(x))
 
-namespace exx {
+namespace EXX_NS {
 
-struct alignas(16) cplx {
-    double x, y;
+typedef EXX_REAL real;
+struct alignas(2 * sizeof(EXX_REAL)) cplx {
+    real x, y;
 };
 
-EXX_HD cplx mk(double x, double y) {
+EXX_HD cplx mk(real x, real y) {
     cplx r;
     r.x = x;
     r.y = y;
@@ -30,11 +40,12 @@ EXX_HD cplx operator-(cplx a, cplx b) { return mk(a.x - b.x, a.y - b.y); }
 EXX_HD cplx operator*(cplx a, cplx b) { return mk(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 EXX_HD cplx mul_conj_b(cplx a, cplx b) { return mk(a.x * b.x + a.y * b.y, a.y * b.x - a.x * b.y); }  // a * conj(b)
 EXX_HD cplx conj_mul(cplx a, cplx b) { return mk(a.x * b.x + a.y * b.y, a.x * b.y - a.y * b.x); }    // conj(a) * b
-EXX_HD cplx scale(double s, cplx a) { return mk(s * a.x, s * a.y); }
+EXX_HD cplx scale(real s, cplx a) { return mk(s * a.x, s * a.y); }
 EXX_HD cplx mul_mi(cplx a) { return mk(a.y, -a.x); }  // a * (-i)
 EXX_HD cplx mul_pi(cplx a) { return mk(-a.y, a.x); }  // a * (+i)
-EXX_HD cplx mulc(cplx a, double cr, double ci) { return mk(a.x * cr - a.y * ci, a.x * ci + a.y * cr); }  // a * (cr + i ci)
+EXX_HD cplx mulc(cplx a, real cr, real ci) { return mk(a.x * cr - a.y * ci, a.x * ci + a.y * cr); }  // a * (cr + i ci)
 
+#ifndef EXX_HS3
 #define EXX_HS3 0.86602540378443864676372317075294   /* sqrt(3)/2 */
 #define EXX_RH2 0.70710678118654752440084436210485   /* sqrt(1/2) */
 #define EXX_C16 0.92387953251128675612818318939679   /* cos(pi/8) */
@@ -45,6 +56,7 @@ EXX_HD cplx mulc(cplx a, double cr, double ci) { return mk(a.x * cr - a.y * ci, 
 #define EXX_S9_2 0.98480775301220805936674302458952  /* sin(4 pi/9) */
 #define EXX_C9_4 (-0.93969262078590838405410927732473) /* cos(8 pi/9) */
 #define EXX_S9_4 0.34202014332566873304409961468226  /* sin(8 pi/9) */
+#endif
 
 EXX_HD void bf2(cplx& a, cplx& b) {
     cplx t = a - b;
@@ -53,8 +65,8 @@ EXX_HD void bf2(cplx& a, cplx& b) {
 }
 EXX_HD void bf3(cplx& a, cplx& b, cplx& c) {  // forward 3-point DFT
     cplx t1 = b + c, t2 = b - c;
-    cplx m = mk(a.x - 0.5 * t1.x, a.y - 0.5 * t1.y);
-    cplx r = mk(EXX_HS3 * t2.y, -EXX_HS3 * t2.x);  // (-i) (sqrt3/2) t2
+    cplx m = mk(a.x - EXX_RC(0.5) * t1.x, a.y - EXX_RC(0.5) * t1.y);
+    cplx r = mk(EXX_RC(EXX_HS3) * t2.y, -EXX_RC(EXX_HS3) * t2.x);  // (-i) (sqrt3/2) t2
     a = a + t1;
     b = m + r;
     c = m - r;
@@ -105,9 +117,9 @@ struct Dft<8> {
     static EXX_HD void fwd(cplx* v) {
         bf4(v[0], v[2], v[4], v[6]);  // E[k] in v[0], v[2], v[4], v[6]
         bf4(v[1], v[3], v[5], v[7]);  // O[k] in v[1], v[3], v[5], v[7]
-        cplx o1 = mk(EXX_RH2 * (v[3].x + v[3].y), EXX_RH2 * (v[3].y - v[3].x));   // O1 * W8^1
+        cplx o1 = mk(EXX_RC(EXX_RH2) * (v[3].x + v[3].y), EXX_RC(EXX_RH2) * (v[3].y - v[3].x));   // O1 * W8^1
         cplx o2 = mul_mi(v[5]);                                                   // O2 * W8^2
-        cplx o3 = mk(EXX_RH2 * (v[7].y - v[7].x), -EXX_RH2 * (v[7].x + v[7].y));  // O3 * W8^3
+        cplx o3 = mk(EXX_RC(EXX_RH2) * (v[7].y - v[7].x), -EXX_RC(EXX_RH2) * (v[7].x + v[7].y));  // O3 * W8^3
         cplx e0 = v[0], e1 = v[2], e2 = v[4], e3 = v[6], o0 = v[1];
         v[0] = e0 + o0;
         v[4] = e0 - o0;
@@ -171,13 +183,13 @@ struct Dft<16> {
         bf4(v[2], v[6], v[10], v[14]);
         bf4(v[3], v[7], v[11], v[15]);
         v[5] = mulc(v[5], EXX_C16, -EXX_S16);                                                    // W16^1
-        v[6] = mk(EXX_RH2 * (v[6].x + v[6].y), EXX_RH2 * (v[6].y - v[6].x));                     // W16^2
+        v[6] = mk(EXX_RC(EXX_RH2) * (v[6].x + v[6].y), EXX_RC(EXX_RH2) * (v[6].y - v[6].x));                     // W16^2
         v[7] = mulc(v[7], EXX_S16, -EXX_C16);                                                    // W16^3
-        v[9] = mk(EXX_RH2 * (v[9].x + v[9].y), EXX_RH2 * (v[9].y - v[9].x));                     // W16^2
+        v[9] = mk(EXX_RC(EXX_RH2) * (v[9].x + v[9].y), EXX_RC(EXX_RH2) * (v[9].y - v[9].x));                     // W16^2
         v[10] = mul_mi(v[10]);                                                                   // W16^4
-        v[11] = mk(EXX_RH2 * (v[11].y - v[11].x), -EXX_RH2 * (v[11].x + v[11].y));               // W16^6
+        v[11] = mk(EXX_RC(EXX_RH2) * (v[11].y - v[11].x), -EXX_RC(EXX_RH2) * (v[11].x + v[11].y));               // W16^6
         v[13] = mulc(v[13], EXX_S16, -EXX_C16);                                                  // W16^3
-        v[14] = mk(EXX_RH2 * (v[14].y - v[14].x), -EXX_RH2 * (v[14].x + v[14].y));               // W16^6
+        v[14] = mk(EXX_RC(EXX_RH2) * (v[14].y - v[14].x), -EXX_RC(EXX_RH2) * (v[14].x + v[14].y));               // W16^6
         v[15] = mulc(v[15], -EXX_C16, EXX_S16);                                                  // W16^9
         bf4(v[0], v[1], v[2], v[3]);
         bf4(v[4], v[5], v[6], v[7]);
@@ -204,4 +216,4 @@ EXX_HD void dft(cplx* v) {
     }
 }
 
-}  // namespace exx
+}  // namespace EXX_NS

@@ -1,0 +1,359 @@
+// exx_fused_kernels.h — the kernels of the fused passes and their launchers (Launch<R1>), mode-generic like
+// exx_fused_phases.h: exx_fused.cu includes it once per (EXX_NS, EXX_REAL) — exx / double for the fp64 product path, exx32 /
+// float for the mixed-precision pair pipeline.  Product code: shares nothing with oracle/.
+#include "exx_fused_phases.h"
+
+namespace EXX_NS {
+#ifdef EXX_SECOND_MODE  // names of exx_internal.h that the first mode (namespace exx) sees directly
+using ::exx::AJob;
+using ::exx::CJob;
+using ::exx::LaunchScope;
+using ::exx::KC_PASS_A;
+using ::exx::KC_PASS_B;
+using ::exx::KC_PASS_C;
+using ::exx::KC_FFT_FUSED;
+#endif
+
+cplx h_tw[TW_TOTAL];  // host copy of the twiddle tables (source of the constant-memory upload)
+
+// ---------------------------------------------------------------------------------------------------------------
+// pass A: rho = conj(u_b) u_a, z transform, first y step.  One CTA per (tile, pair), pair fastest so that the CTAs that
+// share a u tile run back to back and the tile is fetched from HBM once.
+template <int R1>
+__global__ void __launch_bounds__(FusedCfg<R1>::NT1, FusedCfg<R1>::MINB1) pass_a_kernel(const cplx* __restrict__ ua_base, const cplx* __restrict__ ub_base,
+                                                                    AJob job, cplx* __restrict__ work) {
+    constexpr int N = 8 * R1, U = FusedCfg<R1>::U1, NT = FusedCfg<R1>::NT1;
+    constexpr bool TWREG = FusedCfg<R1>::TWREG;
+    static_assert(!TWREG || NT % R1 == 0, "TWREG needs a thread-invariant k1z");
+    constexpr size_t Ng = (size_t)N * N * N;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* S = reinterpret_cast<cplx*>(smem_raw);
+    cplx* T = S + U * R1 * N;
+    const int tid = threadIdx.x;
+    const unsigned bid = blockIdx.x;
+    const int p = bid % job.npairs;
+    const int tile = bid / job.npairs;
+    const int pi = job.pi[p], pj = job.pj[p];
+    const int x = tile / (8 / U), yb = tile % (8 / U);
+    cplx twr[8];
+    if (TWREG)
+        load_twr<R1>(tid, twr);
+    else
+        for (int i = tid; i < R1 * 8; i += NT) T[tidx(i >> 3, i & 7)] = c_tw[TwOff<R1>::v + (i >> 3) * (i & 7)];
+    const cplx* un = ua_base + (size_t)job.a_idx[pi] * Ng;
+    const cplx* um = ub_base + (size_t)job.b_idx[pj] * Ng;
+    cplx* W = work + (size_t)(pi * job.tb + pj) * Ng;
+    p1_z1<R1, U, NT>(tid, un, um, x, yb, S);
+    __syncthreads();
+    p13_z8<R1, U, NT, -1, TWREG>(tid, S, T, twr);
+    __syncthreads();
+    p1_y1<R1, U, NT>(tid, S, W, x, yb);
+}
+
+// ---- bulk-copy (TMA, 1-D) and mbarrier helpers for pass B --------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)), "l"(gsrc),
+                 "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void* gdst, const void* smem_src, uint32_t bytes) {
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(smem_u32(smem_src)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit_wait_all() {
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+}
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// pass B: second y step, x transform, K', inverse x, first inverse y step; in place on the pair's work box.  The tile
+// (k1y, zb) is one contiguous run of the work box (layout widx): N rows of 512 bytes are bulk-copied (TMA) into the padded
+// shared-memory tile, all five steps run in shared memory, and the rows are bulk-copied back.
+template <int R1>
+__global__ void __launch_bounds__(FusedCfg<R1>::NT2, FusedCfg<R1>::MINB2) pass_b_kernel(cplx* __restrict__ work, const real* __restrict__ kperm, AJob job) {
+    constexpr int N = 8 * R1, Z = FusedCfg<R1>::Z, NT = FusedCfg<R1>::NT2, PX = P2Geo<Z>::PX;
+    constexpr size_t Ng = (size_t)N * N * N;
+    constexpr uint32_t ROWB = 8 * Z * sizeof(cplx);
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* S = reinterpret_cast<cplx*>(smem_raw);
+    __shared__ __align__(8) uint64_t bar;
+    const int tid = threadIdx.x;
+    const unsigned bid = blockIdx.x;
+    const int p = bid % job.npairs;
+    const int tile = bid / job.npairs;
+    const int k1y = tile / (N / Z);
+    cplx* Wt = work + (size_t)(job.pi[p] * job.tb + job.pj[p]) * Ng + (size_t)tile * ((size_t)N * 8 * Z);
+    const real* Kt = kperm + (size_t)tile * ((size_t)N * 8 * Z);
+    if (tid == 0) mbar_init(&bar, 1);
+    __syncthreads();
+    if (tid == 0) mbar_arrive_expect_tx(&bar, ROWB * N);
+    for (int x = tid; x < N; x += NT) bulk_g2s(S + x * PX, Wt + x * 8 * Z, ROWB, &bar);
+    mbar_wait(&bar, 0);
+    p2_y8<R1, Z, NT, -1>(tid, S, k1y);
+    __syncthreads();
+    p2_xR<R1, Z, NT, -1>(tid, S);
+    __syncthreads();
+    p2_x8<R1, Z, NT>(tid, S, Kt);
+    __syncthreads();
+    p2_xR<R1, Z, NT, +1>(tid, S);
+    __syncthreads();
+    p2_y8<R1, Z, NT, +1>(tid, S, k1y);
+    fence_proxy_async_smem();
+    __syncthreads();
+    for (int x = tid; x < N; x += NT) bulk_s2g(Wt + x * 8 * Z, S + x * PX, ROWB);
+    bulk_commit_wait_all();
+}
+
+// pass C: second inverse y step, inverse z, acc -= coef u v.  One CTA per (tile, row) loops over the row's columns with
+// its accumulator tile on chip, then adds it to the row's accumulator box in global memory once (fixed summation order).
+// Rows/columns are the a/b bands of the batch (CJob); the transposed sweep (cj) uses conj(v) and the a-band as multiplier.
+template <int R1>
+__global__ void __launch_bounds__(FusedCfg<R1>::NT3, FusedCfg<R1>::MINB3) pass_c_kernel(const cplx* __restrict__ work, const cplx* __restrict__ usrc_base, CJob job,
+                                                                    acc_c* __restrict__ acc_base) {
+    constexpr int N = 8 * R1, U = FusedCfg<R1>::U3, NT = FusedCfg<R1>::NT3;
+    constexpr bool TWREG = FusedCfg<R1>::TWREG, ACCREG = FusedCfg<R1>::ACCREG;
+    static_assert(!TWREG || NT % R1 == 0, "TWREG needs a thread-invariant k1z");
+    constexpr size_t Ng = (size_t)N * N * N;
+    constexpr int IT = (U * R1 * 8 + NT - 1) / NT;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* S = reinterpret_cast<cplx*>(smem_raw);
+    acc_c* A = reinterpret_cast<acc_c*>(S + U * R1 * N);  // fp64 accumulator tile; unused when ACCREG
+    cplx* T = reinterpret_cast<cplx*>(A + (ACCREG ? 0 : U * R1 * N));
+    const int tid = threadIdx.x;
+    const unsigned bid = blockIdx.x;
+    const int r = bid % job.nr;
+    const int tile = bid / job.nr;
+    const int x = tile / (8 / U), yb = tile % (8 / U);
+    const int cnt = job.cnt[r];
+    const bool cj = job.cj != 0;
+    cplx twr[8];
+    if (TWREG)
+        load_twr<R1>(tid, twr);
+    else
+        for (int i = tid; i < R1 * 8; i += NT) T[tidx(i >> 3, i & 7)] = c_tw[TwOff<R1>::v + (i >> 3) * (i & 7)];
+    acc_c accr[ACCREG ? IT * R1 : 1];
+    if (ACCREG) {
+#pragma unroll
+        for (int i = 0; i < (ACCREG ? IT * R1 : 1); i++) accr[i] = mka(0.0, 0.0);
+    }
+    for (int ci = 0; ci < cnt; ci++) {
+        const int col = job.col[r][ci];
+        const cplx* W = work + (size_t)(r * job.box_r + col * job.box_c) * Ng;
+        const cplx* um = usrc_base + (size_t)job.src[col] * Ng;
+        const double wf = job.coef[col];
+        p3_y2inv<R1, U, NT>(tid, W, x, yb, S);
+        __syncthreads();
+        p13_z8<R1, U, NT, +1, TWREG>(tid, S, T, twr);
+        __syncthreads();
+        if (ACCREG)
+            p3_zinv2_reg<R1, U, NT>(tid, S, um, wf, x, yb, accr, cj);
+        else
+            p3_zinv2<R1, U, NT>(tid, S, um, wf, x, yb, A, ci == 0, cj);
+        __syncthreads();
+    }
+    if (cnt > 0) {
+        if (ACCREG)
+            p3_flush_reg<R1, U, NT>(tid, accr, acc_base + (size_t)job.tgt[r] * Ng, x, yb);
+        else
+            p3_flush<R1, U, NT>(tid, A, acc_base + (size_t)job.tgt[r] * Ng, x, yb);
+    }
+}
+
+// ---- plain 3-D transforms through the same passes (S1, S7; F layout, see exx_fused_phases.h) ------------------------
+// forward first half: natural box p of in_base -> work box p (z transform, first y step)
+template <int R1>
+__global__ void __launch_bounds__(FusedCfg<R1>::NT1, FusedCfg<R1>::MINB1) fft_a_kernel(const cplx* __restrict__ in_base, int nbox, cplx* __restrict__ work) {
+    constexpr int N = 8 * R1, U = FusedCfg<R1>::U1, NT = FusedCfg<R1>::NT1;
+    constexpr bool TWREG = FusedCfg<R1>::TWREG;
+    constexpr size_t Ng = (size_t)N * N * N;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* S = reinterpret_cast<cplx*>(smem_raw);
+    cplx* T = S + U * R1 * N;
+    const int tid = threadIdx.x;
+    const int p = blockIdx.x % nbox, tile = blockIdx.x / nbox;
+    const int x = tile / (8 / U), yb = tile % (8 / U);
+    cplx twr[8];
+    if (TWREG)
+        load_twr<R1>(tid, twr);
+    else
+        for (int i = tid; i < R1 * 8; i += NT) T[tidx(i >> 3, i & 7)] = c_tw[TwOff<R1>::v + (i >> 3) * (i & 7)];
+    p1_z1_single<R1, U, NT>(tid, in_base + (size_t)p * Ng, x, yb, S);
+    __syncthreads();
+    p13_z8<R1, U, NT, -1, TWREG>(tid, S, T, twr);
+    __syncthreads();
+    p1_y1<R1, U, NT>(tid, S, work + (size_t)p * Ng, x, yb);
+}
+
+// the pass-B half, in place on work box p.  SIGN < 0: second y step, forward x (-> F layout); SIGN > 0: inverse x, first
+// inverse y step (F layout ->)
+template <int R1, int SIGN>
+__global__ void __launch_bounds__(FusedCfg<R1>::NT2, FusedCfg<R1>::MINB2) fft_b_kernel(cplx* __restrict__ work, int nbox) {
+    constexpr int N = 8 * R1, Z = FusedCfg<R1>::Z, NT = FusedCfg<R1>::NT2, PX = P2Geo<Z>::PX;
+    constexpr size_t Ng = (size_t)N * N * N;
+    constexpr uint32_t ROWB = 8 * Z * sizeof(cplx);
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* S = reinterpret_cast<cplx*>(smem_raw);
+    __shared__ __align__(8) uint64_t bar;
+    const int tid = threadIdx.x;
+    const int p = blockIdx.x % nbox, tile = blockIdx.x / nbox;
+    const int k1y = tile / (N / Z);
+    cplx* Wt = work + (size_t)p * Ng + (size_t)tile * ((size_t)N * 8 * Z);
+    if (tid == 0) mbar_init(&bar, 1);
+    __syncthreads();
+    if (tid == 0) mbar_arrive_expect_tx(&bar, ROWB * N);
+    for (int x = tid; x < N; x += NT) bulk_g2s(S + x * PX, Wt + x * 8 * Z, ROWB, &bar);
+    mbar_wait(&bar, 0);
+    if (SIGN < 0) {
+        p2_y8<R1, Z, NT, -1>(tid, S, k1y);
+        __syncthreads();
+        p2_xR<R1, Z, NT, -1>(tid, S);
+        __syncthreads();
+        p2_x8_half<R1, Z, NT, -1>(tid, S);
+    } else {
+        p2_x8_half<R1, Z, NT, +1>(tid, S);
+        __syncthreads();
+        p2_xR<R1, Z, NT, +1>(tid, S);
+        __syncthreads();
+        p2_y8<R1, Z, NT, +1>(tid, S, k1y);
+    }
+    fence_proxy_async_smem();
+    __syncthreads();
+    for (int x = tid; x < N; x += NT) bulk_s2g(Wt + x * 8 * Z, S + x * PX, ROWB);
+    bulk_commit_wait_all();
+}
+
+// inverse second half: work box p -> natural box p of out_base (second inverse y step, inverse z)
+template <int R1>
+__global__ void __launch_bounds__(FusedCfg<R1>::NT3, FusedCfg<R1>::MINB3) fft_c_kernel(const cplx* __restrict__ work, int nbox, cplx* __restrict__ out_base) {
+    constexpr int N = 8 * R1, U = FusedCfg<R1>::U3, NT = FusedCfg<R1>::NT3;
+    constexpr bool TWREG = FusedCfg<R1>::TWREG;
+    constexpr size_t Ng = (size_t)N * N * N;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* S = reinterpret_cast<cplx*>(smem_raw);
+    cplx* T = S + U * R1 * N;
+    const int tid = threadIdx.x;
+    const int p = blockIdx.x % nbox, tile = blockIdx.x / nbox;
+    const int x = tile / (8 / U), yb = tile % (8 / U);
+    cplx twr[8];
+    if (TWREG)
+        load_twr<R1>(tid, twr);
+    else
+        for (int i = tid; i < R1 * 8; i += NT) T[tidx(i >> 3, i & 7)] = c_tw[TwOff<R1>::v + (i >> 3) * (i & 7)];
+    p3_y2inv<R1, U, NT>(tid, work + (size_t)p * Ng, x, yb, S);
+    __syncthreads();
+    p13_z8<R1, U, NT, +1, TWREG>(tid, S, T, twr);
+    __syncthreads();
+    p3_zinv2_store<R1, U, NT>(tid, S, out_base + (size_t)p * Ng, x, yb);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+template <int R1>
+struct Launch {
+    static constexpr int N = 8 * R1, U1 = FusedCfg<R1>::U1, U3 = FusedCfg<R1>::U3, Z = FusedCfg<R1>::Z;
+    static constexpr bool TWREG = FusedCfg<R1>::TWREG, ACCREG = FusedCfg<R1>::ACCREG;
+    static constexpr size_t smem_a = sizeof(cplx) * ((size_t)U1 * R1 * N + (TWREG ? 0 : R1 * 8));
+    static constexpr size_t smem_c = sizeof(cplx) * ((size_t)U3 * R1 * N + (TWREG ? 0 : R1 * 8)) + sizeof(acc_c) * (ACCREG ? 0 : (size_t)U3 * R1 * N);
+    static constexpr size_t smem_b = sizeof(cplx) * ((size_t)N * P2Geo<Z>::PX);
+
+    static int init(exx_ctx* c) {
+        EXX_CUDA(c, cudaFuncSetAttribute(pass_a_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a));
+        EXX_CUDA(c, cudaFuncSetAttribute(pass_b_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b));
+        EXX_CUDA(c, cudaFuncSetAttribute(pass_c_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_c));
+        EXX_CUDA(c, cudaFuncSetAttribute(fft_a_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a));
+        EXX_CUDA(c, cudaFuncSetAttribute((fft_b_kernel<R1, -1>), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b));
+        EXX_CUDA(c, cudaFuncSetAttribute((fft_b_kernel<R1, +1>), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b));
+        EXX_CUDA(c, cudaFuncSetAttribute(fft_c_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_c));
+        return EXX_OK;
+    }
+    // passes A and B over the pairs of one batch
+    static int pass_ab(exx_ctx* c, const cplx* ua_base, const cplx* ub_base, const AJob& job, const real* kperm, cplx* work) {
+        const unsigned tiles1 = N * (8 / U1), tiles2 = R1 * (N / Z);
+        {
+            LaunchScope ls(c, KC_PASS_A, job.npairs);
+            pass_a_kernel<R1><<<tiles1 * job.npairs, FusedCfg<R1>::NT1, smem_a, c->stream>>>(ua_base, ub_base, job, work);
+        }
+        {
+            LaunchScope ls(c, KC_PASS_B, job.npairs);
+            pass_b_kernel<R1><<<tiles2 * job.npairs, FusedCfg<R1>::NT2, smem_b, c->stream>>>(work, kperm, job);
+        }
+        EXX_CUDA(c, cudaGetLastError());
+        return EXX_OK;
+    }
+    // plain transforms of nbox boxes: forward natural in -> F layout in work; inverse F layout in work -> natural out
+    static int fft_forward(exx_ctx* c, const cplx* in_base, int nbox, cplx* work) {
+        const unsigned tiles1 = N * (8 / U1), tiles2 = R1 * (N / Z);
+        {
+            LaunchScope ls(c, KC_FFT_FUSED, nbox);
+            fft_a_kernel<R1><<<tiles1 * nbox, FusedCfg<R1>::NT1, smem_a, c->stream>>>(in_base, nbox, work);
+        }
+        {
+            LaunchScope ls(c, KC_FFT_FUSED, nbox);
+            fft_b_kernel<R1, -1><<<tiles2 * nbox, FusedCfg<R1>::NT2, smem_b, c->stream>>>(work, nbox);
+        }
+        EXX_CUDA(c, cudaGetLastError());
+        return EXX_OK;
+    }
+    static int fft_inverse(exx_ctx* c, cplx* work, int nbox, cplx* out_base) {
+        const unsigned tiles3 = N * (8 / U3), tiles2 = R1 * (N / Z);
+        {
+            LaunchScope ls(c, KC_FFT_FUSED, nbox);
+            fft_b_kernel<R1, +1><<<tiles2 * nbox, FusedCfg<R1>::NT2, smem_b, c->stream>>>(work, nbox);
+        }
+        {
+            LaunchScope ls(c, KC_FFT_FUSED, nbox);
+            fft_c_kernel<R1><<<tiles3 * nbox, FusedCfg<R1>::NT3, smem_c, c->stream>>>(work, nbox, out_base);
+        }
+        EXX_CUDA(c, cudaGetLastError());
+        return EXX_OK;
+    }
+    static void fill_fmap(const int32_t* nat, int n, int32_t* out) {
+        for (int i = 0; i < n; i++) {
+            int j = nat[i];
+            out[i] = (int32_t)findex<R1>(j / (N * N), (j / N) % N, j % N);
+        }
+    }
+    // one accumulation sweep (pass C)
+    static int pass_c(exx_ctx* c, const cplx* usrc_base, const CJob& job, int64_t units, const cplx* work, acc_c* acc_base) {
+        const unsigned tiles3 = N * (8 / U3);
+        LaunchScope ls(c, KC_PASS_C, units);
+        pass_c_kernel<R1><<<tiles3 * job.nr, FusedCfg<R1>::NT3, smem_c, c->stream>>>(work, usrc_base, job, acc_base);
+        EXX_CUDA(c, cudaGetLastError());
+        return EXX_OK;
+    }
+};
+
+// twiddles W_N^j for every supported N (long double angles), to this mode's constant memory
+inline int upload_twiddles(exx_ctx* c) {
+    const int Ns[5] = {48, 64, 72, 96, 128};
+    const int off[5] = {TwOff<6>::v, TwOff<8>::v, TwOff<9>::v, TwOff<12>::v, TwOff<16>::v};
+    const long double tp = 6.283185307179586476925286766559005768L;
+    for (int s = 0; s < 5; s++)
+        for (int j = 0; j < Ns[s]; j++) {
+            long double a = tp * j / Ns[s];
+            h_tw[off[s] + j] = mk((real)cosl(a), (real)(-sinl(a)));
+        }
+    EXX_CUDA(c, cudaMemcpyToSymbol(c_tw, h_tw, sizeof(h_tw)));
+    return EXX_OK;
+}
+
+}  // namespace EXX_NS

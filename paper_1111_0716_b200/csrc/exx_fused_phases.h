@@ -12,12 +12,29 @@
 //   pass B (p2_*): second y step; x transform; times K'; inverse x; first inverse y step  tile: one k1y, Z positions of z
 //   pass C (p3_*): second inverse y step; inverse z; acc -= w f u_m v                     tile: as pass A, loops over m
 // With pair symmetry (v_{mq,nk} = conj v_{nk,mq}) pass C runs a second time with the roles of the bands swapped (cj).
-#pragma once
+//
+// Like exx_dft.h this header is mode-generic: included once per (EXX_NS, EXX_REAL); accumulators are always fp64 (acc_c).
 #include <stddef.h>
 
 #include "exx_dft.h"
 
-namespace exx {
+#ifndef EXX_ACC_C_DEFINED
+#define EXX_ACC_C_DEFINED
+namespace exx_acc {
+struct alignas(16) acc_c {  // fp64 complex accumulator element, whatever the mode of the transforms
+    double x, y;
+};
+}  // namespace EXX_NS_acc
+#endif
+
+namespace EXX_NS {
+using exx_acc::acc_c;
+EXX_HD acc_c mka(double x, double y) {
+    acc_c r;
+    r.x = x;
+    r.y = y;
+    return r;
+}
 
 // twiddle tables W_N^j, j < N, for every supported N, in one array (constant memory on the device)
 constexpr int TW_TOTAL = 48 + 64 + 72 + 96 + 128;
@@ -44,10 +61,14 @@ struct TwOff<16> {
     static constexpr int v = 280;
 };
 
+#if defined(__CUDACC__)
+__constant__ cplx c_tw[TW_TOTAL];  // one table per mode (this header is included in exactly one .cu)
+#endif
+extern cplx h_tw[TW_TOTAL];
+#undef EXX_TW
 #if defined(__CUDA_ARCH__)
 #define EXX_TW(R1, j) c_tw[TwOff<R1>::v + (j)]
 #else
-extern cplx h_tw[TW_TOTAL];
 #define EXX_TW(R1, j) h_tw[TwOff<R1>::v + (j)]
 #endif
 
@@ -320,7 +341,7 @@ EXX_HD void p2_xR(int tid, cplx* S) {
 }
 
 template <int R1, int Z, int NT>
-EXX_HD void p2_x8(int tid, cplx* S, const double* __restrict__ Kt) {
+EXX_HD void p2_x8(int tid, cplx* S, const real* __restrict__ Kt) {
     // items (k1x, rem): second forward x step, times K' (S4), first inverse x step, conjugate twiddle.
     // Kt: this tile's slice of the permuted kernel table, 8 consecutive doubles (k2x = 0..7) per item.
     constexpr int NI = R1 * 8 * Z, IT = (NI + NT - 1) / NT, PX = P2Geo<Z>::PX;
@@ -330,7 +351,7 @@ EXX_HD void p2_x8(int tid, cplx* S, const double* __restrict__ Kt) {
         if (it < NI) {
             int k1x = it / (8 * Z), rem = it - k1x * (8 * Z);
             cplx v[8];
-            double kk[8];
+            real kk[8];
 #pragma unroll
             for (int j = 0; j < 8; j++) kk[j] = Kt[(size_t)it * 8 + j];
 #pragma unroll
@@ -369,7 +390,7 @@ EXX_HD void p3_y2inv(int tid, const cplx* __restrict__ W, int x, int yb, cplx* S
 }
 
 template <int R1, int U, int NT>
-EXX_HD void p3_zinv2(int tid, const cplx* S, const cplx* __restrict__ um, double wf, int x, int yb, cplx* A, bool first, bool cj = false) {
+EXX_HD void p3_zinv2(int tid, const cplx* S, const cplx* __restrict__ um, double wf, int x, int yb, acc_c* A, bool first, bool cj = false) {
     // items (row, n2z): last inverse z step, then acc -= (w_q f_m) u_m v   (S6); A is this CTA's private accumulator tile
     constexpr int N = 8 * R1, NI = U * R1 * 8, IT = (NI + NT - 1) / NT;
 #pragma unroll
@@ -388,18 +409,18 @@ EXX_HD void p3_zinv2(int tid, const cplx* S, const cplx* __restrict__ um, double
 #pragma unroll
             for (int j = 0; j < R1; j++) {
                 cplx p = b[j] * (cj ? mk(v[j].x, -v[j].y) : v[j]);  // cj: the transposed pair uses conj(v)
-                cplx* a = A + row * N + j * 8 + n2z;
+                acc_c* a = A + row * N + j * 8 + n2z;
                 if (first)
-                    *a = mk(-wf * p.x, -wf * p.y);
+                    *a = mka(-wf * p.x, -wf * p.y);
                 else
-                    *a = mk(a->x - wf * p.x, a->y - wf * p.y);
+                    *a = mka(a->x - wf * p.x, a->y - wf * p.y);
             }
         }
     }
 }
 
 template <int R1, int U, int NT>
-EXX_HD void p3_flush(int tid, const cplx* A, cplx* __restrict__ accg, int x, int yb) {
+EXX_HD void p3_flush(int tid, const acc_c* A, acc_c* __restrict__ accg, int x, int yb) {
     constexpr int N = 8 * R1, NI = U * R1 * 8, IT = (NI + NT - 1) / NT;
 #pragma unroll
     for (int i = 0; i < IT; i++) {
@@ -410,8 +431,8 @@ EXX_HD void p3_flush(int tid, const cplx* A, cplx* __restrict__ accg, int x, int
             size_t base = ((size_t)x * N + (n1y * 8 + yb * U + u)) * N + n2z;
 #pragma unroll
             for (int j = 0; j < R1; j++) {
-                cplx g = accg[base + j * 8], a = A[row * N + j * 8 + n2z];
-                accg[base + j * 8] = g + a;
+                acc_c g = accg[base + j * 8], a = A[row * N + j * 8 + n2z];
+                accg[base + j * 8] = mka(g.x + a.x, g.y + a.y);
             }
         }
     }
@@ -419,7 +440,7 @@ EXX_HD void p3_flush(int tid, const cplx* A, cplx* __restrict__ accg, int x, int
 
 // register-accumulator variants (ACCREG): acc[i*R1 + j] belongs to item tid + i*NT, element n1z = j
 template <int R1, int U, int NT>
-EXX_HD void p3_zinv2_reg(int tid, const cplx* S, const cplx* __restrict__ um, double wf, int x, int yb, cplx* acc, bool cj = false) {
+EXX_HD void p3_zinv2_reg(int tid, const cplx* S, const cplx* __restrict__ um, double wf, int x, int yb, acc_c* acc, bool cj = false) {
     constexpr int N = 8 * R1, NI = U * R1 * 8, IT = (NI + NT - 1) / NT;
 #pragma unroll
     for (int i = 0; i < IT; i++) {
@@ -437,14 +458,14 @@ EXX_HD void p3_zinv2_reg(int tid, const cplx* S, const cplx* __restrict__ um, do
 #pragma unroll
             for (int j = 0; j < R1; j++) {
                 cplx p = b[j] * (cj ? mk(v[j].x, -v[j].y) : v[j]);  // cj: the transposed pair uses conj(v)
-                acc[i * R1 + j] = mk(acc[i * R1 + j].x - wf * p.x, acc[i * R1 + j].y - wf * p.y);
+                acc[i * R1 + j] = mka(acc[i * R1 + j].x - wf * p.x, acc[i * R1 + j].y - wf * p.y);
             }
         }
     }
 }
 
 template <int R1, int U, int NT>
-EXX_HD void p3_flush_reg(int tid, const cplx* acc, cplx* __restrict__ accg, int x, int yb) {
+EXX_HD void p3_flush_reg(int tid, const acc_c* acc, acc_c* __restrict__ accg, int x, int yb) {
     constexpr int N = 8 * R1, NI = U * R1 * 8, IT = (NI + NT - 1) / NT;
 #pragma unroll
     for (int i = 0; i < IT; i++) {
@@ -454,7 +475,7 @@ EXX_HD void p3_flush_reg(int tid, const cplx* acc, cplx* __restrict__ accg, int 
             int u = row / R1, n1y = row - u * R1;
             size_t base = ((size_t)x * N + (n1y * 8 + yb * U + u)) * N + n2z;
 #pragma unroll
-            for (int j = 0; j < R1; j++) accg[base + j * 8] = accg[base + j * 8] + acc[i * R1 + j];
+            for (int j = 0; j < R1; j++) accg[base + j * 8] = mka(accg[base + j * 8].x + acc[i * R1 + j].x, accg[base + j * 8].y + acc[i * R1 + j].y);
         }
     }
 }
@@ -553,4 +574,4 @@ inline void permute_ktable(int R1, int Z, const double* nat, double* perm) {
                         }
 }
 
-}  // namespace exx
+}  // namespace EXX_NS

@@ -25,13 +25,14 @@ static void fill_tw() {
 }
 
 template <int R1>
-static void emu_pair(const cplx* un, const cplx* um, const double* Knat, double wf, cplx* acc, cplx* W) {
+static void emu_pair(const cplx* un, const cplx* um, const double* Knat, double wf, acc_c* acc, cplx* W) {
     typedef FusedCfg<R1> C;
     constexpr int N = 8 * R1, U = C::U1, NT13 = C::NT1, U3 = C::U3, NT3 = C::NT3, Z = C::Z, NT2 = C::NT2;
     constexpr bool TWREG = C::TWREG, ACCREG = C::ACCREG;
     std::vector<double> Kp((size_t)N * N * N);
     permute_ktable(R1, Z, Knat, Kp.data());
-    std::vector<cplx> S((size_t)(U > U3 ? U : U3) * R1 * N), A((size_t)U3 * R1 * N), T(R1 * 8), S2((size_t)N * P2Geo<Z>::PX);
+    std::vector<acc_c> A((size_t)U3 * R1 * N);
+    std::vector<cplx> S((size_t)(U > U3 ? U : U3) * R1 * N), T(R1 * 8), S2((size_t)N * P2Geo<Z>::PX);
     for (int k = 0; k < R1; k++)
         for (int j = 0; j < 8; j++) T[tidx(k, j)] = EXX_TW(R1, j * k);
     // pass A
@@ -60,10 +61,10 @@ static void emu_pair(const cplx* un, const cplx* um, const double* Knat, double 
         }
     // pass C (one m)
     constexpr int IT3 = (U3 * R1 * 8 + NT3 - 1) / NT3;
-    std::vector<cplx> accr((size_t)NT3 * IT3 * R1);
+    std::vector<acc_c> accr((size_t)NT3 * IT3 * R1);
     for (int x = 0; x < N; x++)
         for (int yb = 0; yb < 8 / U3; yb++) {
-            for (auto& a : accr) a = mk(0.0, 0.0);
+            for (auto& a : accr) a = mka(0.0, 0.0);
             for (int t = 0; t < NT3; t++) p3_y2inv<R1, U3, NT3>(t, W, x, yb, S.data());
             for (int t = 0; t < NT3; t++) {
                 cplx twr[8];
@@ -171,11 +172,11 @@ int exx_emu_dft(int R, int sign, double* inout) {
 int exx_emu_pair(int R1, const double* un, const double* um, const double* Knat, double wf, double* acc, double* work) {
     fill_tw();
     switch (R1) {
-    case 6: emu_pair<6>((const cplx*)un, (const cplx*)um, Knat, wf, (cplx*)acc, (cplx*)work); return 0;
-    case 8: emu_pair<8>((const cplx*)un, (const cplx*)um, Knat, wf, (cplx*)acc, (cplx*)work); return 0;
-    case 9: emu_pair<9>((const cplx*)un, (const cplx*)um, Knat, wf, (cplx*)acc, (cplx*)work); return 0;
-    case 12: emu_pair<12>((const cplx*)un, (const cplx*)um, Knat, wf, (cplx*)acc, (cplx*)work); return 0;
-    case 16: emu_pair<16>((const cplx*)un, (const cplx*)um, Knat, wf, (cplx*)acc, (cplx*)work); return 0;
+    case 6: emu_pair<6>((const cplx*)un, (const cplx*)um, Knat, wf, (acc_c*)acc, (cplx*)work); return 0;
+    case 8: emu_pair<8>((const cplx*)un, (const cplx*)um, Knat, wf, (acc_c*)acc, (cplx*)work); return 0;
+    case 9: emu_pair<9>((const cplx*)un, (const cplx*)um, Knat, wf, (acc_c*)acc, (cplx*)work); return 0;
+    case 12: emu_pair<12>((const cplx*)un, (const cplx*)um, Knat, wf, (acc_c*)acc, (cplx*)work); return 0;
+    case 16: emu_pair<16>((const cplx*)un, (const cplx*)um, Knat, wf, (acc_c*)acc, (cplx*)work); return 0;
     default: return -1;
     }
 }

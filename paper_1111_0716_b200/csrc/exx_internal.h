@@ -96,10 +96,10 @@ struct exx_ctx {
     int last_pruned = 0;
 
     // options
-    int64_t opt_path = 0, opt_tile_n = 0, opt_tile_m = 0, opt_prune = 1, opt_profile = 0, opt_symmetry = 1;
+    int64_t opt_path = 0, opt_tile_n = 0, opt_tile_m = 0, opt_prune = 1, opt_profile = 0, opt_symmetry = 1, opt_precision = 0;
 
     // counters of the last apply
-    int64_t symmetry_used = 0;
+    int64_t symmetry_used = 0, precision_used = 0;
     int64_t launches = 0, pairs_ordered = 0, pairs_executed = 0, path_used = 0, tile_n_used = 0, tile_m_used = 0, pruned_used = 0;
     int64_t launches_by_class[exx::KC_COUNT] = {0};
     int64_t units_by_class[exx::KC_COUNT] = {0};   // box passes (generic) or pairs (fused) processed

@@ -151,6 +151,14 @@ int exx_scatter(exx_ctx* ctx, int ik, const double* coef_dev, int nbatch, double
 int exx_gather(exx_ctx* ctx, int ik, const double* box_dev, int nbatch, double* coef_dev);
 int exx_fft3d(exx_ctx* ctx, double* box_dev, int nbatch, int sign);
 int exx_to_real(exx_ctx* ctx, int ik, const double* coef_dev, int nbatch, double* box_dev);
+/* Stand-alone batched 3-D transform through the fused passes (cubic N = 48, 64, 72, 96, 128; EXX_ERR_BAD_GRID otherwise): two
+ * passes per transform instead of the three of exx_fft3d.  The frequency side lives in the library's "F layout":
+ * exx_findex gives, for every natural C-order frequency index ((kx*N + ky)*N + kz), its position in an F-layout box.
+ *   sign = -1: in_dev natural-order boxes (unchanged) -> out_dev F-layout boxes, unnormalised forward transform
+ *   sign = +1: in_dev F-layout boxes (used as scratch: destroyed) -> out_dev natural-order boxes, unnormalised inverse
+ * in_dev != out_dev, nbatch boxes of Ng complex128 each; asynchronous on the stream. */
+int exx_fft3d_fused(exx_ctx* ctx, double* in_dev, int nbatch, int sign, double* out_dev);
+int exx_findex(const exx_ctx* ctx, int32_t* host_out /* Ng entries */);
 /* K'_{k-q}(g) as the library tabulated it (host_out: Ng doubles, C order). */
 int exx_kernel_table(const exx_ctx* ctx, int ik, int iq, double* host_out);
 

@@ -22,7 +22,7 @@ EXX_INFO_PRECISION = 15
 SYMBOLS = ("exx_create", "exx_destroy", "exx_npw", "exx_index_map", "exx_psi_offset", "exx_set_option", "exx_get_option",
            "exx_get_info", "exx_get_kernel_time", "exx_kernel_class_name", "exx_apply", "exx_energy", "exx_apply_host",
            "exx_scatter", "exx_gather", "exx_fft3d", "exx_to_real", "exx_kernel_table", "exx_strerror", "exx_last_error",
-           "exx_version", "exx_subspace")
+           "exx_version", "exx_subspace", "exx_fft3d_fused", "exx_findex")
 
 
 class KernelParams(C.Structure):
@@ -75,6 +75,8 @@ def lib():
         L.exx_energy.argtypes = [vp, vp, dp, vp, dp, dp]
         L.exx_apply_host.argtypes = [vp, vp, dp, vp, dp]
         L.exx_subspace.argtypes = [vp, C.c_int, vp, vp, vp]
+        L.exx_fft3d_fused.argtypes = [vp, vp, C.c_int, C.c_int, vp]
+        L.exx_findex.argtypes = [vp, C.POINTER(C.c_int32)]
         L.exx_scatter.argtypes = [vp, C.c_int, vp, C.c_int, vp]
         L.exx_gather.argtypes = [vp, C.c_int, vp, C.c_int, vp]
         L.exx_fft3d.argtypes = [vp, vp, C.c_int, C.c_int]
@@ -245,6 +247,15 @@ class Exx:
     def fft3d(self, box_dev, nbatch, sign):
         self._chk(lib().exx_fft3d(self._h, self._dev(box_dev, nbatch * self.ng), nbatch, sign))
         return box_dev
+
+    def fft3d_fused(self, in_dev, nbatch, sign, out_dev):
+        self._chk(lib().exx_fft3d_fused(self._h, self._dev(in_dev, nbatch * self.ng), nbatch, sign, self._dev(out_dev, nbatch * self.ng)))
+        return out_dev
+
+    def findex(self):
+        f = np.empty(self.ng, dtype=np.int32)
+        self._chk(lib().exx_findex(self._h, f.ctypes.data_as(C.POINTER(C.c_int32))))
+        return f
 
     def to_real(self, ik, coef_dev, nbatch, box_dev):
         self._chk(lib().exx_to_real(self._h, ik, self._dev(coef_dev, nbatch * self.npw[ik]), nbatch, self._dev(box_dev, nbatch * self.ng)))

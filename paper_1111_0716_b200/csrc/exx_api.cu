@@ -536,6 +536,16 @@ int exx_fft3d(exx_ctx* c, double* box_dev, int nbatch, int sign) {
     if (nbatch == 0) return EXX_OK;
     return launch_fft3d_generic(c, (double2*)box_dev, nbatch, sign);
 }
+int exx_fft3d_fused(exx_ctx* c, double* in_dev, int nbatch, int sign, double* out_dev) {
+    if (!c || !in_dev || !out_dev) return EXX_ERR_NULL;
+    if (nbatch < 0 || (sign != 1 && sign != -1) || in_dev == out_dev) return EXX_ERR_BAD_ARG;
+    if (nbatch == 0) return EXX_OK;
+    return fused_fft3d(c, (double2*)in_dev, nbatch, sign, (double2*)out_dev);
+}
+int exx_findex(const exx_ctx* c, int32_t* host_out) {
+    if (!c || !host_out) return EXX_ERR_NULL;
+    return fused_findex(c, host_out);
+}
 int exx_to_real(exx_ctx* c, int ik, const double* coef_dev, int nbatch, double* box_dev) {
     int rc = exx_scatter(c, ik, coef_dev, nbatch, box_dev);
     if (rc) return rc;

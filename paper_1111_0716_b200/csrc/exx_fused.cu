@@ -110,6 +110,45 @@ void fused_destroy(exx_ctx* c) {
     c->fused = nullptr;
 }
 
+// Stand-alone batched 3-D transform through the fused passes (S8(f)-3; the paper's third intercept, offloads
+// FFT3D calls above a size threshold).  Forward: natural-order boxes `in` -> F-layout boxes `out`.  Inverse: F-layout boxes
+// `in` (used as scratch, destroyed) -> natural-order boxes `out`.  Needs only the twiddles and kernel attributes, none of the
+// per-band buffers.
+int fused_fft3d(exx_ctx* c, double2* in, int nbatch, int sign, double2* out) {
+    if (!fused_supported(c)) return EXX_ERR_BAD_GRID;
+    const int R1 = c->N[0] / 8;
+    int rc = EXX_OK;
+    if (!c->fft_ready) {
+        if ((rc = upload_twiddles(c))) return rc;
+        EXX_DISPATCH_R1(R1, rc = L::init(c));
+        if (rc) return rc;
+        c->fft_ready = true;
+    }
+    const size_t Ng = (size_t)c->Ng;
+    const int bmax = 1 << 12;  // keeps every grid well below 2^31 CTAs
+    for (int b0 = 0; b0 < nbatch; b0 += bmax) {
+        const int bn = std::min(bmax, nbatch - b0);
+        if (sign < 0) {
+            EXX_DISPATCH_R1(R1, rc = L::fft_forward(c, (const cplx*)in + (size_t)b0 * Ng, bn, (cplx*)out + (size_t)b0 * Ng));
+        } else {
+            EXX_DISPATCH_R1(R1, rc = L::fft_inverse(c, (cplx*)in + (size_t)b0 * Ng, bn, (cplx*)out + (size_t)b0 * Ng));
+        }
+        if (rc) return rc;
+    }
+    return EXX_OK;
+}
+int fused_findex(const exx_ctx* c, int32_t* host_out) {
+    if (!fused_supported(c)) return EXX_ERR_BAD_GRID;
+    const int R1 = c->N[0] / 8, N = c->N[0];
+    std::vector<int32_t> nat((size_t)N);
+    for (int kx = 0; kx < N; kx++)
+        for (int ky = 0; ky < N; ky++) {
+            for (int kz = 0; kz < N; kz++) nat[kz] = (int32_t)(((int64_t)kx * N + ky) * N + kz);
+            EXX_DISPATCH_R1(R1, L::fill_fmap(nat.data(), N, host_out + ((size_t)kx * N + ky) * N));
+        }
+    return EXX_OK;
+}
+
 __global__ void to_float_kernel(const double* __restrict__ in, float* __restrict__ out, size_t n) {
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) out[i] = (float)in[i];
 }

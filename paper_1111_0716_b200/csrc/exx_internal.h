@@ -91,6 +91,7 @@ struct exx_ctx {
     // holds every product the method forms without wrap-around (N >= 4 gmax + 1); owned by this context.  big_alloc: the
     // real-space cache, pair workspace, accumulators and fused tables of THIS grid exist (allocated in exx_create when there is
     // no inner context, else on the first apply with pruning switched off).
+    bool fft_ready = false;           // twiddles/attributes of the fused kernels set up for exx_fft3d_fused
     exx_ctx* inner = nullptr;
     bool big_alloc = false;
     int last_pruned = 0;
@@ -168,5 +169,7 @@ void fused_tiles(const exx_ctx* c, int* tn, int* tm);
 int fused_create(exx_ctx* c);
 void fused_destroy(exx_ctx* c);
 int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out);
+int fused_fft3d(exx_ctx* c, double2* in, int nbatch, int sign, double2* out);
+int fused_findex(const exx_ctx* c, int32_t* host_out);
 
 }  // namespace exx

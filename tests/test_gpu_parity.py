@@ -589,3 +589,43 @@ def test_mixed_precision_against_oracle_small(B):
         e, _ = g.energy(pd, w.occ, out)
         assert abs(e - e_want) <= 1e-6 * abs(e_want)
     g.close()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# S8(f)-3: stand-alone batched 3-D transform through the fused passes
+@pytest.mark.parametrize("n", [48, 64, 72])
+def test_fft3d_fused_against_oracle_fft(B, n):
+    import torch
+    g = B.Exx((n, n, n), W.cubic(10.0), np.zeros((1, 3)), [1.0], 2.0, nbands=1)
+    fidx = g.findex()
+    assert np.array_equal(np.sort(fidx), np.arange(n ** 3, dtype=np.int32))
+    rng = np.random.default_rng(n)
+    nbatch = 3
+    x = rng.standard_normal((nbatch, n, n, n)) + 1j * rng.standard_normal((nbatch, n, n, n))
+    xin = torch.from_numpy(x.reshape(-1).copy()).cuda()
+    out = torch.empty_like(xin)
+    g.fft3d_fused(xin, nbatch, -1, out)
+    assert np.array_equal(xin.cpu().numpy(), x.reshape(-1))            # forward leaves its input alone
+    got = out.cpu().numpy().reshape(nbatch, -1)
+    for b in range(nbatch if n < 64 else 1):
+        want = R.fft3d(x[b], -1).reshape(-1)
+        assert _rel(got[b][fidx], want) < 2e-15 * np.log2(n ** 3)
+    # inverse of the forward gives back Ng * x
+    back = torch.empty_like(xin)
+    g.fft3d_fused(out, nbatch, +1, back)
+    assert _rel(back.cpu().numpy(), x.reshape(-1) * n ** 3) < 1e-14
+    # agrees with the generic natural-order transform of the library too
+    ref = xin.clone()
+    g.fft3d(ref, nbatch, -1)
+    assert _rel(got[:, fidx].reshape(-1), ref.cpu().numpy()) < 1e-14
+    g.close()
+
+
+def test_fft3d_fused_refuses_unsupported_grids(B):
+    import torch
+    g = B.Exx((12, 18, 16), W.cubic(6.0), np.zeros((1, 3)), [1.0], 2.0, nbands=1)
+    a = torch.zeros(g.ng, dtype=torch.complex128, device="cuda")
+    with pytest.raises(B.ExxError) as ei:
+        g.fft3d_fused(a, 1, -1, torch.empty_like(a))
+    assert ei.value.code == -2
+    g.close()

@@ -134,6 +134,8 @@ def run_ours(args, rank, world, local):
     g = B.Exx.from_workload(w)
     if args.path is not None:
         g.set_option(B.EXX_OPT_PATH, args.path)
+    if args.precision == "mixed":   # the paper's second mode; NOT the graded fp64 configuration
+        g.set_option(B.EXX_OPT_PRECISION, 1)
     psi = w.coefficients(g.npw)
     occ = w.occ
     pd = g.to_device(psi)
@@ -239,7 +241,7 @@ def run_ours(args, rank, world, local):
         full = {"grid": list(w.grid), "ms_per_step": ms_f, "value": world * pairs_ord / (ms_f * 1e-3), "unit": UNIT,
                 "us_per_executed_pair": 1e3 * ms_f / max(1, pe_f), "us_per_ordered_pair": 1e3 * ms_f / max(1, pairs_ord),
                 "bytes_per_pass_execution": 32 * w.ng, "pipeline_achieved_GBs": pipe_f, "pipeline_frac": pipe_f / peak, "E_x": ex_f}
-        assert abs(ex_f - ex) <= 1e-11 * abs(ex)
+        assert abs(ex_f - ex) <= (1e-11 if args.precision == "fp64" else 1e-5) * abs(ex)
         g.set_option(B.EXX_OPT_PRUNE, 1)
 
     # ---- timed region 3: end to end through exx_apply_host, pinned host buffers, copies inside the timed region
@@ -253,11 +255,13 @@ def run_ours(args, rank, world, local):
     h1.record()
     sync_all()
     ms_e2e = max_over_ranks(h0.elapsed_time(h1), world, dev) / args.steps
-    assert ex_h == ex or abs(ex_h - ex) <= 1e-12 * abs(ex)
+    assert ex_h == ex or abs(ex_h - ex) <= (1e-12 if args.precision == "fp64" else 1e-5) * abs(ex)
 
     value = world * pairs_ord / (ms * 1e-3)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64" if args.precision == "fp64" else "f32 transforms + f64 accumulation (mixed; outside the fp64 parity contract)",
+            "data": "synthetic",
             "config": {"workload": w.name, "description": w.description, "grid": list(w.grid), "nk": w.nk, "nbands": w.nbands,
                        "pairs_per_step": pairs_ord, "parallelism": "replicas x%d" % world,
                        "path": {1: "generic", 2: "fused"}.get(g.get_info(B.EXX_INFO_PATH_USED)),
@@ -300,6 +304,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C4a", choices=list(W.ALL))
     ap.add_argument("--path", type=int, default=None, help="EXX_OPT_PATH override: 1 generic, 2 fused")
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "mixed"],
+                    help="mixed = EXX_OPT_PRECISION 1 (fp32 pair transforms); for information only, the default fp64 run is the benchmark")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-full-grid", action="store_true", help="skip the extra full-grid (EXX_OPT_PRUNE = 0) timing")
     args = ap.parse_args()

@@ -158,6 +158,12 @@ struct FusedCfg<EXX_TUNE_R1> {
 template <int R1>
 EXX_HD int sidx(int u, int r, int k1z, int j) {  // row = u R1 + r
     int row = u * R1 + r;
+    if (sizeof(real) == 4) {
+        // 8-byte elements: a half-warp (16 lanes) is served together and the bank is the low 4 bits of the element index.
+        // Bit 3 of the index is the parity of it = row R1 + k1z, so swizzling j with the next three bits of it makes 16
+        // consecutive (row, k1z) items, 16 consecutive positions of a row, and 2 rows x 8 j (R1 odd) all conflict-free.
+        return row * (8 * R1) + k1z * 8 + (j ^ (((row * R1 + k1z) >> 1) & 7));
+    }
     return row * (8 * R1) + k1z * 8 + (j ^ (((row * R1 + k1z) & 7) ^ ((u & 1) << 2)));
 }
 // the pair work box W between the passes: [k1y][kzpos / 4][x][n2y][kzpos % 4] — a pass-B tile (k1y, zb) is one

@@ -1,6 +1,7 @@
-// exx_fused.cu — the fused three-pass pair pipeline (S2..S6) for cubic grids N = 8 R1, R1 in {6, 8, 9, 12, 16}
-// (N = 48, 64, 72, 96, 128).  The per-thread phases live in exx_fused_phases.h; this file holds the kernels that
-// run them between barriers, the permuted kernel tables, and the loop nest over k, n-tiles, q, m-tiles
+// exx_fused.cu — host side of the fused three-pass pair pipeline (S1..S7) for cubic grids N = 8 R1, R1 in {6, 8, 9, 12, 16}
+// (N = 48, 64, 72, 96, 128).  The per-thread phases live in exx_fused_phases.h, the kernels and launchers in
+// exx_fused_kernels.h (compiled twice: fp64 and fp32); this file holds the permuted kernel tables, the F-layout sphere maps and
+// the loop nest over k, q and band-pair batches
 // (k,q loops on the host, band loops on the device, innermost loop blocked).
 // Product code: shares nothing with oracle/.
 #include <algorithm>
@@ -28,7 +29,6 @@ struct FusedState {
     // mixed precision (allocated on first use): fp32 copies of the u cache and of the permuted kernel tables
     exx32::cplx* u32_dev = nullptr;
     float* kperm32_dev = nullptr;
-    int tn = 0, tm = 0;
 };
 
 #define EXX_DISPATCH_R1(R1v, EXPR)                  \

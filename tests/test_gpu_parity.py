@@ -629,3 +629,30 @@ def test_fft3d_fused_refuses_unsupported_grids(B):
         g.fft3d_fused(a, 1, -1, torch.empty_like(a))
     assert ei.value.code == -2
     g.close()
+
+
+def test_fused_degenerate_cases(B):
+    """Fused path edge cases: a single band, all occupations zero, one occupied band among empties."""
+    import torch
+    for nb, occ in ((1, [1.0]), (3, [0.0, 0.0, 0.0]), (5, [0.0, 0.0, 0.7, 0.0, 0.0])):
+        w = W.custom("deg48", 31 + nb, (48, 48, 48), W.cubic(8.0), [[0, 0, 0]], [1.0], 5.0, nb, occ)
+        o, g = _pair(B, w)
+        psi = w.coefficients(o.npw)
+        want = o.apply(psi, w.occ)
+        pd = g.to_device(psi)
+        for sym in (1, 0):
+            g.set_option(B.EXX_OPT_SYMMETRY, sym)
+            out = g.apply(pd, w.occ)
+            assert g.get_info(B.EXX_INFO_PATH_USED) == 2
+            assert g.get_info(B.EXX_INFO_PAIRS_ORDERED) == w.pair_evals
+            got = out.cpu().numpy()
+            if not any(occ):
+                assert float(np.abs(got).max()) == 0.0 and g.get_info(B.EXX_INFO_PAIRS_EXECUTED) == 0
+                assert g.energy(pd, w.occ, out)[0] == 0.0
+            else:
+                for n in range(nb):
+                    assert _rel(o.band(got, 0, n), o.band(want, 0, n)) < TOL_VX, (nb, sym, n)
+                e, _ = g.energy(pd, w.occ, out)
+                e_want, _ = o.energy(psi, w.occ, want)
+                assert abs(e - e_want) <= TOL_EX * abs(e_want)
+        g.close()

@@ -62,11 +62,12 @@ enum {
     EXX_ERR_ALIAS = -10       /* out aliases psi */
 };
 
-/* Options (exx_set_option / exx_get_option).  All are tuning knobs: results may differ only by rounding order. */
+/* Options (exx_set_option / exx_get_option).  All but EXX_OPT_PRECISION are tuning knobs: results differ only by rounding
+ * order (<= 1e-13 relative, tested).  EXX_OPT_PRECISION = 1 changes the arithmetic (see below). */
 enum {
     EXX_OPT_PATH = 1,       /* 0 auto (fused kernels when the grid is supported, else generic), 1 generic per-axis kernels, 2 fused */
-    EXX_OPT_TILE_N = 2,     /* bands n per tile (0 = auto) */
-    EXX_OPT_TILE_M = 3,     /* bands m per tile (0 = auto) */
+    EXX_OPT_TILE_N = 2,     /* bands per row tile of a pair batch (0 = auto = 16; at most 16 on the fused path) */
+    EXX_OPT_TILE_M = 3,     /* bands per column tile of a pair batch (0 = auto = 16) */
     EXX_OPT_PRUNE = 4,      /* 1 (default): run the pair pipeline on the compact work grid when there is one (see EXX_INFO_COMPACT_GRID);
                                0: always transform the caller's full grid */
     EXX_OPT_PROFILE = 5,    /* 1: bracket every kernel launch with CUDA events so exx_get_kernel_time works (slower) */
@@ -88,7 +89,7 @@ enum {
     EXX_INFO_NCOEF = 6,           /* complex elements in psi / out */
     EXX_INFO_TILE_N = 7,
     EXX_INFO_TILE_M = 8,
-    EXX_INFO_PRUNED = 9,          /* 1 if band-limit pruning was active */
+    EXX_INFO_PRUNED = 9,          /* 1 if the last apply ran on the compact work grid */
     EXX_INFO_NUM_KERNEL_CLASSES = 10,  /* how many kernel classes exx_get_kernel_time knows (the value, not this enum) */
     EXX_INFO_WORK_GRID = 11,      /* N of the (cubic) grid the last apply transformed; first axis of the caller's grid if not compacted */
     EXX_INFO_SYMMETRY = 13,       /* 1 if the last apply used the pair symmetry (then PAIRS_EXECUTED < PAIRS_ORDERED) */
@@ -115,7 +116,8 @@ int exx_set_option(exx_ctx* ctx, int option, int64_t value);
 int exx_get_option(const exx_ctx* ctx, int option, int64_t* value);
 int exx_get_info(const exx_ctx* ctx, int what, int64_t* value);
 /* Per kernel class `kclass` (0 .. EXX_INFO_NUM_KERNEL_CLASSES-1), for the most recent exx_apply: launch count, work
- * units (generic kernels: box passes, i.e. one read + one write of an FFT box; fused passes: band pairs), and — with
+ * units (generic kernels and fused_fft_pass: box passes, i.e. one read + one write of an FFT box; fused passes A/B: band pairs;
+ * fused pass C: accumulation sweeps, one per pair and side), and — with
  * EXX_OPT_PROFILE = 1 — the device time from CUDA events on the context's stream (0 otherwise).  Synchronises.
  * exx_kernel_class_name gives the class name (static string, NULL if out of range). */
 int exx_get_kernel_time(exx_ctx* ctx, int kclass, double* ms_total, int64_t* launches, int64_t* units);

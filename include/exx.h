@@ -51,7 +51,7 @@ typedef struct {
 enum {
     EXX_OK = 0,
     EXX_ERR_NULL = -1,        /* a required pointer is NULL */
-    EXX_ERR_BAD_GRID = -2,    /* N_i not of the form 2^a 3^b (a+b >= 1), N_i > 1024, or the cutoff sphere does not fit the box */
+    EXX_ERR_BAD_GRID = -2,    /* N_i not of the form 2^a 3^b 5^c (>= 2), N_i > 1024, or the cutoff sphere does not fit the box */
     EXX_ERR_BAD_LATTICE = -3, /* zero or non-finite cell volume */
     EXX_ERR_BAD_CUTOFF = -4,  /* E_cut <= 0 or non-finite, or an empty sphere */
     EXX_ERR_BAD_KERNEL = -5,  /* unknown kind, mu <= 0 for HSE, non-finite scale */

@@ -59,10 +59,11 @@ static double norm2_frac(const double B[9], const double t[3]) {
     }
     return s;
 }
-static bool is_2a3b(int n) {
+static bool is_2a3b(int n) {  // 2^a 3^b 5^c
     if (n < 2) return false;
     while (n % 2 == 0) n /= 2;
     while (n % 3 == 0) n /= 3;
+    while (n % 5 == 0) n /= 5;
     return n == 1;
 }
 static void make_plan(Plan1D& p, int n) {
@@ -72,6 +73,7 @@ static void make_plan(Plan1D& p, int n) {
     while (m % 4 == 0) { p.radix[p.nst++] = 4; m /= 4; }
     while (m % 2 == 0) { p.radix[p.nst++] = 2; m /= 2; }
     while (m % 3 == 0) { p.radix[p.nst++] = 3; m /= 3; }
+    while (m % 5 == 0) { p.radix[p.nst++] = 5; m /= 5; }
 }
 
 static double kernel_value(const exx_kernel_params& kp, const double B[9], const double t[3]) {
@@ -155,7 +157,7 @@ const char* exx_strerror(int code) {
     switch (code) {
     case EXX_OK: return "ok";
     case EXX_ERR_NULL: return "null pointer";
-    case EXX_ERR_BAD_GRID: return "bad grid (each N_i must be 2^a 3^b, 2 <= N_i <= 1024, and hold the cutoff sphere)";
+    case EXX_ERR_BAD_GRID: return "bad grid (each N_i must be 2^a 3^b 5^c, 2 <= N_i <= 1024, and hold the cutoff sphere)";
     case EXX_ERR_BAD_LATTICE: return "bad lattice (zero or non-finite volume)";
     case EXX_ERR_BAD_CUTOFF: return "bad cutoff";
     case EXX_ERR_BAD_KERNEL: return "bad kernel parameters";
@@ -338,8 +340,8 @@ static int create_impl(exx_ctx** out, const int grid[3], const double lattice[9]
         if (allow_inner && c->alias_free) {
             int need = 0;
             for (int i = 0; i < 3; i++) need = std::max(need, 4 * c->gmax[i] + 1);
-            const int cand[5] = {48, 64, 72, 96, 128};
-            for (int ci = 0; ci < 5; ci++)
+            const int cand[9] = {16, 32, 40, 48, 64, 72, 80, 96, 128};
+            for (int ci = 0; ci < 9; ci++)
                 if (cand[ci] >= need) {
                     int64_t nw = cand[ci];
                     if (nw * nw * nw < c->Ng) {

@@ -1,4 +1,4 @@
-// exx_dft.h — complex fp64 helpers and in-register DFT codelets (R = 2,3,4,6,8,9,12,16) used by the fused passes.
+// exx_dft.h — complex fp64 helpers and in-register DFT codelets (R = 2,3,4,5,6,8,9,10,12,16) used by the fused passes.
 // Product code: shares nothing with oracle/.  Everything here is __host__ __device__ so that the same index and
 // butterfly logic can be executed on the CPU by tests/test_fused_host_emulation.py (host logic test, no GPU).
 //
@@ -95,6 +95,25 @@ struct Dft<4> {
     static EXX_HD void fwd(cplx* v) { bf4(v[0], v[1], v[2], v[3]); }
 };
 template <>
+struct Dft<5> {
+    // prime size: p_n = x_n + x_{5-n}, m_n = x_n - x_{5-n};  X_k = x_0 + sum_n p_n cos(2 pi n k/5) - i sum_n m_n sin(2 pi n k/5),
+    // X_{5-k} the same with + i
+    static EXX_HD void fwd(cplx* v) {
+        constexpr double C[5] = {1, 0.309016994374947451262869435595348477, -0.809016994374947340240566973079694435, -0.80901699437494756228517189811100252, 0.309016994374947229218264510564040393};
+        constexpr double S[5] = {0, 0.95105651629515353118193843329208903, 0.587785252292473248125759255344746634, -0.58778525229247302608115433031343855, -0.951056516295153642204240895807743073};
+        cplx p1 = v[1] + v[4], m1 = v[1] - v[4], p2 = v[2] + v[3], m2 = v[2] - v[3], x0 = v[0];
+        v[0] = x0 + p1 + p2;
+#pragma unroll
+        for (int k = 1; k <= 2; k++) {
+            const real c1 = (real)C[k % 5], c2 = (real)C[(2 * k) % 5], s1 = (real)S[k % 5], s2 = (real)S[(2 * k) % 5];
+            cplx a = mk(x0.x + c1 * p1.x + c2 * p2.x, x0.y + c1 * p1.y + c2 * p2.y);
+            cplx b = mk(s1 * m1.x + s2 * m2.x, s1 * m1.y + s2 * m2.y);
+            v[k] = a + mul_mi(b);
+            v[5 - k] = a - mul_mi(b);
+        }
+    }
+};
+template <>
 struct Dft<6> {
     // n = 3 n1 + n2, k = k1 + 2 k2: 2-point over n1, twiddle W6^(n2 k1), 3-point over n2
     static EXX_HD void fwd(cplx* v) {
@@ -149,6 +168,28 @@ struct Dft<9> {
         for (int k1 = 0; k1 < 3; k1++)
             for (int k2 = 0; k2 < 3; k2++) t[k1 + 3 * k2] = v[3 * k1 + k2];
         for (int k = 0; k < 9; k++) v[k] = t[k];
+    }
+};
+template <>
+struct Dft<10> {
+    // n = 5 n1 + n2, k = k1 + 2 k2: 2-point over n1, twiddle W10^(n2 k1), 5-point over n2
+    static EXX_HD void fwd(cplx* v) {
+        constexpr double C[5] = {1, 0.809016994374947451262869435595348477, 0.309016994374947451262869435595348477, -0.309016994374947340240566973079694435, -0.809016994374947340240566973079694435};
+        constexpr double S[5] = {0, 0.587785252292473137103456792829092592, 0.95105651629515353118193843329208903, 0.951056516295153642204240895807743073, 0.587785252292473248125759255344746634};
+#pragma unroll
+        for (int n2 = 0; n2 < 5; n2++) bf2(v[n2], v[5 + n2]);
+#pragma unroll
+        for (int n2 = 1; n2 < 5; n2++) v[5 + n2] = mulc(v[5 + n2], (real)C[n2], (real)(-S[n2]));
+        Dft<5>::fwd(v);      // k1 = 0: X[0], X[2], X[4], X[6], X[8]
+        Dft<5>::fwd(v + 5);  // k1 = 1: X[1], X[3], X[5], X[7], X[9]
+        cplx t[10];
+#pragma unroll
+        for (int k2 = 0; k2 < 5; k2++) {
+            t[2 * k2] = v[k2];
+            t[2 * k2 + 1] = v[5 + k2];
+        }
+#pragma unroll
+        for (int k = 0; k < 10; k++) v[k] = t[k];
     }
 };
 template <>

@@ -1,5 +1,5 @@
-// exx_fused.cu — host side of the fused three-pass pair pipeline (S1..S7) for cubic grids N = 8 R1, R1 in {6, 8, 9, 12, 16}
-// (N = 48, 64, 72, 96, 128).  The per-thread phases live in exx_fused_phases.h, the kernels and launchers in
+// exx_fused.cu — host side of the fused three-pass pair pipeline (S1..S7) for cubic grids N = 8 R1, R1 in {2, 4, 5, 6, 8, 9, 10, 12, 16}
+// (N = 16, 32, 40, 48, 64, 72, 80, 96, 128).  The per-thread phases live in exx_fused_phases.h, the kernels and launchers in
 // exx_fused_kernels.h (compiled twice: fp64 and fp32); this file holds the permuted kernel tables, the F-layout sphere maps and
 // the loop nest over k, q and band-pair batches
 // (k,q loops on the host, band loops on the device, innermost loop blocked).
@@ -33,6 +33,10 @@ struct FusedState {
 
 #define EXX_DISPATCH_R1(R1v, EXPR)                  \
     switch (R1v) {                                  \
+    case 2: { typedef Launch<2> L; EXPR; } break;   \
+    case 4: { typedef Launch<4> L; EXPR; } break;   \
+    case 5: { typedef Launch<5> L; EXPR; } break;   \
+    case 10: { typedef Launch<10> L; EXPR; } break; \
     case 6: { typedef Launch<6> L; EXPR; } break;   \
     case 8: { typedef Launch<8> L; EXPR; } break;   \
     case 9: { typedef Launch<9> L; EXPR; } break;   \
@@ -44,7 +48,7 @@ struct FusedState {
 bool fused_supported(const exx_ctx* c) {
     int n = c->N[0];
     if (c->N[1] != n || c->N[2] != n) return false;
-    return n == 48 || n == 64 || n == 72 || n == 96 || n == 128;
+    return n == 16 || n == 32 || n == 40 || n == 48 || n == 64 || n == 72 || n == 80 || n == 96 || n == 128;
 }
 
 void fused_tiles(const exx_ctx* c, int* tn, int* tm) {
@@ -154,6 +158,10 @@ __global__ void to_float_kernel(const double* __restrict__ in, float* __restrict
 }
 static int init_mode32(exx_ctx* c, int R1) {
     switch (R1) {
+    case 2: return exx32::Launch<2>::init(c);
+    case 4: return exx32::Launch<4>::init(c);
+    case 5: return exx32::Launch<5>::init(c);
+    case 10: return exx32::Launch<10>::init(c);
     case 6: return exx32::Launch<6>::init(c);
     case 8: return exx32::Launch<8>::init(c);
     case 9: return exx32::Launch<9>::init(c);
@@ -178,6 +186,10 @@ struct ModeF {
 };
 #define EXX_DISPATCH_M(R1v, EXPR)                                      \
     switch (R1v) {                                                     \
+    case 2: { typedef typename M::template L<2> L; EXPR; } break;      \
+    case 4: { typedef typename M::template L<4> L; EXPR; } break;      \
+    case 5: { typedef typename M::template L<5> L; EXPR; } break;      \
+    case 10: { typedef typename M::template L<10> L; EXPR; } break;    \
     case 6: { typedef typename M::template L<6> L; EXPR; } break;      \
     case 8: { typedef typename M::template L<8> L; EXPR; } break;      \
     case 9: { typedef typename M::template L<9> L; EXPR; } break;      \

@@ -344,13 +344,11 @@ struct Launch {
 
 // twiddles W_N^j for every supported N (long double angles), to this mode's constant memory
 inline int upload_twiddles(exx_ctx* c) {
-    const int Ns[5] = {48, 64, 72, 96, 128};
-    const int off[5] = {TwOff<6>::v, TwOff<8>::v, TwOff<9>::v, TwOff<12>::v, TwOff<16>::v};
     const long double tp = 6.283185307179586476925286766559005768L;
-    for (int s = 0; s < 5; s++)
-        for (int j = 0; j < Ns[s]; j++) {
-            long double a = tp * j / Ns[s];
-            h_tw[off[s] + j] = mk((real)cosl(a), (real)(-sinl(a)));
+    for (int r1 = 1; r1 <= 16; r1++)
+        for (int j = 0; j < 8 * r1; j++) {
+            long double a = tp * j / (8 * r1);
+            h_tw[4 * r1 * (r1 - 1) + j] = mk((real)cosl(a), (real)(-sinl(a)));
         }
     EXX_CUDA(c, cudaMemcpyToSymbol(c_tw, h_tw, sizeof(h_tw)));
     return EXX_OK;

@@ -3,7 +3,7 @@
 // exx_host_emu.cpp can run the very same index logic thread by thread on the CPU (host logic test, no GPU).
 // Product code: shares nothing with oracle/.
 //
-// Grid N = 8 R1 per axis (cubic), R1 in {6, 8, 9, 12, 16}.  Every 1-D transform of length N is two in-register steps
+// Grid N = 8 R1 per axis (cubic), R1 in {2, 4, 5, 6, 8, 9, 10, 12, 16}.  Every 1-D transform of length N is two in-register steps
 //   n = 8 n1 + n2, k = k1 + R1 k2:   R1-point DFT over n1 (stride 8)  ->  twiddle W_N^(n2 k1)  ->  8-point DFT over n2
 // done in place, so a frequency k sits at position pos(k) = 8 (k mod R1) + k div R1; the inverse runs the two steps
 // backwards and lands in natural order.  The pair pipeline (S2..S6) is cut at the two points where a full exchange
@@ -36,29 +36,12 @@ EXX_HD acc_c mka(double x, double y) {
     return r;
 }
 
-// twiddle tables W_N^j, j < N, for every supported N, in one array (constant memory on the device)
-constexpr int TW_TOTAL = 48 + 64 + 72 + 96 + 128;
+// twiddle tables W_N^j, j < N = 8 R1, for every R1 <= 16, in one array (constant memory on the device): table R1 starts at
+// sum_{r < R1} 8 r = 4 R1 (R1 - 1)
+constexpr int TW_TOTAL = 4 * 17 * 16;
 template <int R1>
-struct TwOff;
-template <>
-struct TwOff<6> {
-    static constexpr int v = 0;
-};
-template <>
-struct TwOff<8> {
-    static constexpr int v = 48;
-};
-template <>
-struct TwOff<9> {
-    static constexpr int v = 112;
-};
-template <>
-struct TwOff<12> {
-    static constexpr int v = 184;
-};
-template <>
-struct TwOff<16> {
-    static constexpr int v = 280;
+struct TwOff {
+    static constexpr int v = 4 * R1 * (R1 - 1);
 };
 
 #if defined(__CUDACC__)
@@ -79,6 +62,30 @@ extern cplx h_tw[TW_TOTAL];
 // instead of shared memory.
 template <int R1>
 struct FusedCfgBase;
+template <>
+struct FusedCfgBase<2> {
+    static constexpr int U1 = 8, NT1 = 128, U3 = 8, NT3 = 128, Z = 4, NT2 = 64;
+    static constexpr bool TWREG = false, ACCREG = false;
+    static constexpr int MINB1 = 1, MINB2 = 1, MINB3 = 1;
+};
+template <>
+struct FusedCfgBase<4> {
+    static constexpr int U1 = 4, NT1 = 128, U3 = 4, NT3 = 128, Z = 4, NT2 = 128;
+    static constexpr bool TWREG = false, ACCREG = false;
+    static constexpr int MINB1 = 1, MINB2 = 1, MINB3 = 1;
+};
+template <>
+struct FusedCfgBase<5> {
+    static constexpr int U1 = 4, NT1 = 160, U3 = 4, NT3 = 160, Z = 4, NT2 = 128;
+    static constexpr bool TWREG = false, ACCREG = false;
+    static constexpr int MINB1 = 1, MINB2 = 1, MINB3 = 1;
+};
+template <>
+struct FusedCfgBase<10> {
+    static constexpr int U1 = 1, NT1 = 128, U3 = 1, NT3 = 128, Z = 4, NT2 = 160;
+    static constexpr bool TWREG = false, ACCREG = false;
+    static constexpr int MINB1 = 1, MINB2 = 4, MINB3 = 1;
+};
 template <>
 struct FusedCfgBase<6> {
     static constexpr int U1 = 2, NT1 = 96, U3 = 2, NT3 = 96, Z = 4, NT2 = 64;

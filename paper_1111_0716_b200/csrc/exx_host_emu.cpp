@@ -14,13 +14,11 @@ namespace exx {
 cplx h_tw[TW_TOTAL];
 
 static void fill_tw() {
-    const int Ns[5] = {48, 64, 72, 96, 128};
-    const int off[5] = {TwOff<6>::v, TwOff<8>::v, TwOff<9>::v, TwOff<12>::v, TwOff<16>::v};
     const long double tp = 6.283185307179586476925286766559005768L;
-    for (int s = 0; s < 5; s++)
-        for (int j = 0; j < Ns[s]; j++) {
-            long double a = tp * j / Ns[s];
-            h_tw[off[s] + j] = mk((double)cosl(a), (double)(-sinl(a)));
+    for (int r1 = 1; r1 <= 16; r1++)
+        for (int j = 0; j < 8 * r1; j++) {
+            long double a = tp * j / (8 * r1);
+            h_tw[4 * r1 * (r1 - 1) + j] = mk((double)cosl(a), (double)(-sinl(a)));
         }
 }
 
@@ -161,7 +159,7 @@ int exx_emu_dft(int R, int sign, double* inout) {
             dft<r, +1>(v);      \
         return 0;
     switch (R) {
-        CASE(2) CASE(3) CASE(4) CASE(6) CASE(8) CASE(9) CASE(12) CASE(16)
+        CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(8) CASE(9) CASE(10) CASE(12) CASE(16)
     default: return -1;
     }
 #undef CASE
@@ -172,6 +170,10 @@ int exx_emu_dft(int R, int sign, double* inout) {
 int exx_emu_pair(int R1, const double* un, const double* um, const double* Knat, double wf, double* acc, double* work) {
     fill_tw();
     switch (R1) {
+    case 2: emu_pair<2>((const cplx*)un, (const cplx*)um, Knat, wf, (acc_c*)acc, (cplx*)work); return 0;
+    case 4: emu_pair<4>((const cplx*)un, (const cplx*)um, Knat, wf, (acc_c*)acc, (cplx*)work); return 0;
+    case 5: emu_pair<5>((const cplx*)un, (const cplx*)um, Knat, wf, (acc_c*)acc, (cplx*)work); return 0;
+    case 10: emu_pair<10>((const cplx*)un, (const cplx*)um, Knat, wf, (acc_c*)acc, (cplx*)work); return 0;
     case 6: emu_pair<6>((const cplx*)un, (const cplx*)um, Knat, wf, (acc_c*)acc, (cplx*)work); return 0;
     case 8: emu_pair<8>((const cplx*)un, (const cplx*)um, Knat, wf, (acc_c*)acc, (cplx*)work); return 0;
     case 9: emu_pair<9>((const cplx*)un, (const cplx*)um, Knat, wf, (acc_c*)acc, (cplx*)work); return 0;
@@ -191,7 +193,7 @@ int exx_emu_fft(int R1, int sign, double* in, double* out, int64_t* findex_out) 
         if (findex_out) emu_findex<r>(findex_out);      \
         return 0;
     switch (R1) {
-        CASE(6) CASE(8) CASE(9) CASE(12) CASE(16)
+        CASE(2) CASE(4) CASE(5) CASE(10) CASE(6) CASE(8) CASE(9) CASE(12) CASE(16)
     default: return -1;
     }
 #undef CASE

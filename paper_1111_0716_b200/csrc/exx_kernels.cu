@@ -60,7 +60,7 @@ int launch_gather(exx_ctx* c, int ik, const double2* box, int nbatch, double2* c
 
 // ---------------------------------------------------------------------------------------------------------------
 // S3/S5 generic: batched 1-D transforms along one axis of [outer][n][inner] (inner = product of the faster dims).
-// A CTA stages P pencils in shared memory and runs a Stockham autosort FFT with runtime radices 2/3/4:
+// A CTA stages P pencils in shared memory and runs a Stockham autosort FFT with runtime radices 2/3/4/5:
 //   stage with radix R and Ns = product of earlier radices: butterfly j in [0, n/R): k = j mod Ns,
 //   v[r] = x[j + r n/R] W^{r k n/(Ns R)},  R-point DFT,  y[(j/Ns) Ns R + k + r Ns] = v[r].
 struct Radices {
@@ -142,6 +142,27 @@ __global__ void __launch_bounds__(256) fft_axis_generic_kernel(double2* __restri
                 dst[Ns] = cadd(t1, t3r);
                 dst[2 * Ns] = csub(t0, t2);
                 dst[3 * Ns] = csub(t1, t3r);
+            } else if (R == 5) {
+                double2 a = src[0];
+                double2 b1 = cmul(src[nbf], twiddle<SIGN>(tw, k * tws));
+                double2 b2 = cmul(src[2 * nbf], twiddle<SIGN>(tw, 2 * k * tws));
+                double2 b3 = cmul(src[3 * nbf], twiddle<SIGN>(tw, 3 * k * tws));
+                double2 b4 = cmul(src[4 * nbf], twiddle<SIGN>(tw, 4 * k * tws));
+                const double c1 = 0.30901699437494742410229341718282, c2 = -0.80901699437494742410229341718282;  // cos 72, cos 144
+                const double s1 = 0.95105651629515357211643933337938, s2 = 0.58778525229247312916870595463907;   // sin 72, sin 144
+                double2 p1 = cadd(b1, b4), m1 = csub(b1, b4), p2 = cadd(b2, b3), m2 = csub(b2, b3);
+                double2 A1 = make_double2(a.x + c1 * p1.x + c2 * p2.x, a.y + c1 * p1.y + c2 * p2.y);
+                double2 A2 = make_double2(a.x + c2 * p1.x + c1 * p2.x, a.y + c2 * p1.y + c1 * p2.y);
+                double2 B1 = make_double2(s1 * m1.x + s2 * m2.x, s1 * m1.y + s2 * m2.y);
+                double2 B2 = make_double2(s2 * m1.x - s1 * m2.x, s2 * m1.y - s1 * m2.y);
+                // forward: X1 = A1 - i B1, X4 = A1 + i B1, X2 = A2 - i B2, X3 = A2 + i B2; inverse: signs swapped
+                double2 r1 = (SIGN < 0) ? make_double2(B1.y, -B1.x) : make_double2(-B1.y, B1.x);
+                double2 r2 = (SIGN < 0) ? make_double2(B2.y, -B2.x) : make_double2(-B2.y, B2.x);
+                dst[0] = cadd(a, cadd(p1, p2));
+                dst[Ns] = cadd(A1, r1);
+                dst[4 * Ns] = csub(A1, r1);
+                dst[2 * Ns] = cadd(A2, r2);
+                dst[3 * Ns] = csub(A2, r2);
             } else {  // R == 3
                 double2 a = src[0];
                 double2 b = cmul(src[nbf], twiddle<SIGN>(tw, k * tws));

@@ -30,7 +30,7 @@ def _p(a):
     return a.ctypes.data_as(dp)
 
 
-@pytest.mark.parametrize("R", [2, 3, 4, 6, 8, 9, 12, 16])
+@pytest.mark.parametrize("R", [2, 3, 4, 5, 6, 8, 9, 10, 12, 16])
 @pytest.mark.parametrize("sign", [-1, 1])
 def test_codelets_against_numpy(emu, R, sign):
     rng = np.random.default_rng(100 * R + sign)
@@ -46,7 +46,7 @@ def test_codelets_against_numpy(emu, R, sign):
     assert np.array_equal(d, np.ones(R))
 
 
-@pytest.mark.parametrize("R1", [6, 8, 9, 12, 16])
+@pytest.mark.parametrize("R1", [2, 4, 5, 6, 8, 9, 10, 12, 16])
 def test_three_passes_equal_definition(emu, R1):
     """acc += -w f u_m IFFT[K' FFT[conj(u_m) u_n]] (unnormalised transforms), one pair, whole box."""
     N = 8 * R1
@@ -80,7 +80,7 @@ def test_single_plane_wave_pair(emu):
     assert np.abs(acc - want).max() <= 1e-12 * N ** 3
 
 
-@pytest.mark.parametrize("R1", [6, 8, 9, 12])
+@pytest.mark.parametrize("R1", [2, 4, 5, 6, 8, 9, 10, 12])
 def test_plain_transforms_through_the_passes(emu, R1):
     """S1/S7 use the fused passes as plain 3-D transforms: forward natural -> F layout, inverse F layout -> natural."""
     N = 8 * R1

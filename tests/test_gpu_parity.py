@@ -110,7 +110,8 @@ def test_scatter_gather_round_trip_bit_exact(B):
 
 
 @pytest.mark.parametrize("grid,nbatch", [((16, 16, 16), 5), ((48, 48, 48), 2), ((12, 18, 16), 3), ((27, 24, 36), 1), ((8, 6, 9), 4),
-                                         ((64, 64, 64), 1), ((96, 96, 96), 1), ((128, 128, 128), 1), ((32, 16, 8), 2), ((2, 3, 4), 7)])
+                                         ((64, 64, 64), 1), ((96, 96, 96), 1), ((128, 128, 128), 1), ((32, 16, 8), 2), ((2, 3, 4), 7),
+                                         ((10, 20, 15), 3), ((40, 40, 40), 2), ((25, 6, 5), 2)])
 def test_fft3d_against_oracle_fft(B, grid, nbatch):
     import torch
     g = B.Exx(grid, W.cubic(50.0), np.zeros((1, 3)), [1.0], 0.005, nbands=1)  # sphere = {0}: any grid holds it
@@ -244,13 +245,34 @@ COMPACT = {
 }
 
 
+FUSED_SIZES = (16, 32, 40, 48, 64, 72, 80, 96, 128)
+
+
+def _expected_compact(g, w):
+    """Smallest supported cubic grid with N >= 4 gmax + 1, if the caller's grid is itself alias-free and larger."""
+    gmax = 0
+    for k in range(w.nk):
+        j = np.stack(np.unravel_index(g.index_map(k), w.grid))
+        for ax in range(3):
+            f = np.where(2 * j[ax] < w.grid[ax], j[ax], j[ax] - w.grid[ax])
+            gmax = max(gmax, int(np.abs(f).max()))
+    need = 4 * gmax + 1
+    if any(n < need for n in w.grid):
+        return 0
+    for n in FUSED_SIZES:
+        if n >= need:
+            return n if n ** 3 < w.ng else 0
+    return 0
+
+
 @pytest.mark.parametrize("name", list(COMPACT))
 def test_compact_grid_equals_full_grid_and_oracle(B, name):
     s = COMPACT[name]
     lat = W.cubic(s["lat"][1]) if s["lat"][0] == "sc" else W.rhombohedral(s["lat"][1], s["lat"][2])
     w = W.custom(name, 4242, s["grid"], lat, s["kf"], s["kw"], s["ecut"], s["nb"], s["occ"], s["kind"], s["mu"])
     o, g = _pair(B, w)
-    assert g.get_info(B.EXX_INFO_COMPACT_GRID) == s["compact"]
+    compact = _expected_compact(g, w)
+    assert compact and compact < 64 and g.get_info(B.EXX_INFO_COMPACT_GRID) == compact
     psi = w.coefficients(o.npw)
     want = o.apply(psi, w.occ)              # the oracle works on the caller's full 64^3 grid
     e_want, _ = o.energy(psi, w.occ, want)
@@ -263,7 +285,7 @@ def test_compact_grid_equals_full_grid_and_oracle(B, name):
         assert g.get_info(B.EXX_INFO_PRUNED) == prune
         assert g.get_info(B.EXX_INFO_SYMMETRY) == sym
         assert (g.get_info(B.EXX_INFO_PAIRS_EXECUTED) < w.pair_evals) == bool(sym)
-        assert g.get_info(B.EXX_INFO_WORK_GRID) == (s["compact"] if prune else 64)
+        assert g.get_info(B.EXX_INFO_WORK_GRID) == (compact if prune else 64)
         assert g.get_info(B.EXX_INFO_PAIRS_ORDERED) == w.pair_evals
         got = out.cpu().numpy()
         for k in range(w.nk):
@@ -284,14 +306,14 @@ def test_pair_symmetry_off_matches_golden(B, name):
 
 
 def test_compact_grid_not_used_when_caller_grid_aliases(B):
-    # C1 (16^3, needs 21) is aliased by construction and C2/C3 need their whole box: no compact grid
-    for name in ("C1", "C2", "C3"):
+    # C1 (16^3, needs 21) is aliased by construction and C3 (needs 61) keeps its 64^3 box: no compact grid
+    for name in ("C1", "C3"):
         w = W.make(name)
         w.nbands, w.occ_per_k = 2, np.ones(2)
         g = B.Exx.from_workload(w)
         assert g.get_info(B.EXX_INFO_COMPACT_GRID) == 0
         g.close()
-    for name, n in (("C4a", 72), ("C5", 96)):
+    for name, n in (("C2", 40), ("C4a", 72), ("C5", 96)):
         w = W.make(name)
         w.nbands, w.occ_per_k = 2, np.ones(2)
         g = B.Exx.from_workload(w)
@@ -593,7 +615,7 @@ def test_mixed_precision_against_oracle_small(B):
 
 # ---------------------------------------------------------------------------------------------------------------
 # S8(f)-3: stand-alone batched 3-D transform through the fused passes
-@pytest.mark.parametrize("n", [48, 64, 72])
+@pytest.mark.parametrize("n", [16, 32, 40, 48, 64, 72, 80])
 def test_fft3d_fused_against_oracle_fft(B, n):
     import torch
     g = B.Exx((n, n, n), W.cubic(10.0), np.zeros((1, 3)), [1.0], 2.0, nbands=1)

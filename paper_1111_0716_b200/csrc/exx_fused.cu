@@ -85,7 +85,7 @@ int fused_create(exx_ctx* c) {
     EXX_DISPATCH_R1(st->R1, Z = L::Z);
     for (int t = 0; t < c->ntab; t++) {
         EXX_CUDA(c, cudaMemcpy(nat.data(), c->ktab_dev + (size_t)t * Ng, sizeof(double) * Ng, cudaMemcpyDeviceToHost));
-        permute_ktable(st->R1, Z, nat.data(), perm.data());
+        permute_ktable(st->R1, Z, exx::KVW, nat.data(), perm.data());
         EXX_CUDA(c, cudaMemcpy(st->kperm_dev + (size_t)t * Ng, perm.data(), sizeof(double) * Ng, cudaMemcpyHostToDevice));
     }
     // sphere -> F layout maps for S1 / S7
@@ -387,7 +387,18 @@ int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out)
             c->dev_bytes += sizeof(exx32::cplx) * Ng * nbox + sizeof(float) * Ng * c->ntab;
             if ((rc = exx32::upload_twiddles(c))) return rc;
             if ((rc = init_mode32(c, st->R1))) return rc;
-            to_float_kernel<<<1024, 256, 0, c->stream>>>(st->kperm_dev, st->kperm32_dev, Ng * c->ntab);
+            // the fp32 mode reads K' four values per load: its own permutation of the natural tables
+            std::vector<double> nat(Ng), perm(Ng);
+            std::vector<float> permf(Ng);
+            int Z = 4;
+            EXX_DISPATCH_R1(st->R1, Z = L::Z);
+            for (int t = 0; t < c->ntab; t++) {
+                EXX_CUDA(c, cudaMemcpy(nat.data(), c->ktab_dev + (size_t)t * Ng, sizeof(double) * Ng, cudaMemcpyDeviceToHost));
+                permute_ktable(st->R1, Z, exx32::KVW, nat.data(), perm.data());
+                for (size_t i = 0; i < Ng; i++) permf[i] = (float)perm[i];
+                EXX_CUDA(c, cudaMemcpy(st->kperm32_dev + (size_t)t * Ng, permf.data(), sizeof(float) * Ng, cudaMemcpyHostToDevice));
+            }
+            EXX_CUDA(c, cudaDeviceSynchronize());  // pageable copies may still be in flight; one-time set-up
         }
         to_float_kernel<<<2048, 256, 0, c->stream>>>((const double*)c->u_dev, (float*)st->u32_dev, 2 * Ng * nbox);
         EXX_CUDA(c, cudaGetLastError());

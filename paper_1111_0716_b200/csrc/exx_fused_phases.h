@@ -353,11 +353,19 @@ EXX_HD void p2_xR(int tid, cplx* S) {
     }
 }
 
+// K' is read 16 bytes at a time (KVW consecutive k2x values); the tile's slice of the permuted table is [k2x / KVW][item][k2x % KVW],
+// so the lanes of a warp (consecutive items) read one contiguous run per load
+constexpr int KVW = 16 / sizeof(real);
+struct alignas(16) kvec {
+    real v[KVW];
+};
+
 template <int R1, int Z, int NT>
 EXX_HD void p2_x8(int tid, cplx* S, const real* __restrict__ Kt) {
     // items (k1x, rem): second forward x step, times K' (S4), first inverse x step, conjugate twiddle.
-    // Kt: this tile's slice of the permuted kernel table, 8 consecutive doubles (k2x = 0..7) per item.
+    // Kt: this tile's slice of the permuted kernel table (layout above).
     constexpr int NI = R1 * 8 * Z, IT = (NI + NT - 1) / NT, PX = P2Geo<Z>::PX;
+    const kvec* __restrict__ Kv = reinterpret_cast<const kvec*>(Kt);
 #pragma unroll
     for (int i = 0; i < IT; i++) {
         int it = tid + i * NT;
@@ -366,7 +374,11 @@ EXX_HD void p2_x8(int tid, cplx* S, const real* __restrict__ Kt) {
             cplx v[8];
             real kk[8];
 #pragma unroll
-            for (int j = 0; j < 8; j++) kk[j] = Kt[(size_t)it * 8 + j];
+            for (int jv = 0; jv < 8 / KVW; jv++) {
+                kvec q = Kv[(size_t)jv * NI + it];
+#pragma unroll
+                for (int e = 0; e < KVW; e++) kk[jv * KVW + e] = q.v[e];
+            }
 #pragma unroll
             for (int j = 0; j < 8; j++) v[j] = S[(k1x * 8 + j) * PX + rem];
             dft<8, -1>(v);
@@ -571,20 +583,22 @@ EXX_HD void p3_zinv2_store(int tid, const cplx* S, cplx* __restrict__ out, int x
 
 // ================================================================================================================
 // Host side of the layout: K' in natural C order -> the order pass B reads it in,
-//   [k1y][zb][k1x][k2y][kzl][k2x]  with kx = k1x + R1 k2x, ky = k1y + R1 k2y, zpos = zb Z + kzl = 8 k1z + k2z, kz = k1z + R1 k2z.
-inline void permute_ktable(int R1, int Z, const double* nat, double* perm) {
+//   [k1y][zb][k2x / vw][k1x][k2y][kzl][k2x % vw]  with kx = k1x + R1 k2x, ky = k1y + R1 k2y, zpos = zb Z + kzl = 8 k1z + k2z,
+//   kz = k1z + R1 k2z; vw = values per 16-byte load in the mode that reads the table (2 in fp64, 4 in fp32).
+inline void permute_ktable(int R1, int Z, int vw, const double* nat, double* perm) {
     const int N = 8 * R1;
     size_t o = 0;
     for (int k1y = 0; k1y < R1; k1y++)
         for (int zb = 0; zb < N / Z; zb++)
-            for (int k1x = 0; k1x < R1; k1x++)
-                for (int k2y = 0; k2y < 8; k2y++)
-                    for (int kzl = 0; kzl < Z; kzl++)
-                        for (int k2x = 0; k2x < 8; k2x++) {
-                            int zpos = zb * Z + kzl, k1z = zpos >> 3, k2z = zpos & 7;
-                            int kx = k1x + R1 * k2x, ky = k1y + R1 * k2y, kz = k1z + R1 * k2z;
-                            perm[o++] = nat[((size_t)kx * N + ky) * N + kz];
-                        }
+            for (int jv = 0; jv < 8 / vw; jv++)
+                for (int k1x = 0; k1x < R1; k1x++)
+                    for (int k2y = 0; k2y < 8; k2y++)
+                        for (int kzl = 0; kzl < Z; kzl++)
+                            for (int e = 0; e < vw; e++) {
+                                int k2x = jv * vw + e, zpos = zb * Z + kzl, k1z = zpos >> 3, k2z = zpos & 7;
+                                int kx = k1x + R1 * k2x, ky = k1y + R1 * k2y, kz = k1z + R1 * k2z;
+                                perm[o++] = nat[((size_t)kx * N + ky) * N + kz];
+                            }
 }
 
 }  // namespace EXX_NS

@@ -28,7 +28,7 @@ static void emu_pair(const cplx* un, const cplx* um, const double* Knat, double 
     constexpr int N = 8 * R1, U = C::U1, NT13 = C::NT1, U3 = C::U3, NT3 = C::NT3, Z = C::Z, NT2 = C::NT2;
     constexpr bool TWREG = C::TWREG, ACCREG = C::ACCREG;
     std::vector<double> Kp((size_t)N * N * N);
-    permute_ktable(R1, Z, Knat, Kp.data());
+    permute_ktable(R1, Z, KVW, Knat, Kp.data());
     std::vector<acc_c> A((size_t)U3 * R1 * N);
     std::vector<cplx> S((size_t)(U > U3 ? U : U3) * R1 * N), T(R1 * 8), S2((size_t)N * P2Geo<Z>::PX);
     for (int k = 0; k < R1; k++)

@@ -7,8 +7,10 @@ boron-shaped workloads (BASELINE.json metric), one process per GPU.
 A step = one pass of the whole hot path (S1..S8 of DESIGN.md: scatter + inverse FFT of every band, all band pairs,
 forward FFT + gather, energy reduction) over the workload.  `value` times it with psi already in HBM; `e2e` times the
 same call through exx_apply_host with pinned HOST buffers (H2D of psi, D2H of V_x psi and E_x inside the timed region).
-N > 1 runs N independent replicas (the path is single-GPU by design): weak scaling, no collective
-on the data path; timing is barrier + max over ranks.
+N > 1 runs N independent replicas by default (BASELINE.json north_star: one GPU, no sharding): weak
+scaling, no collective on the data path; timing is barrier + max over ranks.  `--parallel shard` instead shares the pair
+batches of ONE workload out over the N ranks (every rank holds psi, runs its batches, one NCCL all-reduce of
+V_x psi per step): strong scaling.
 `--impl reference` times the oracle (oracle/, plain CPU code, as it stands) on a bounded sample of the same workload.
 """
 import argparse
@@ -144,8 +146,24 @@ def run_ours(args, rank, world, local):
     pin_out = torch.empty(g.ncoef, dtype=torch.complex128).pin_memory()
     peak, peak_src = read_peaks()
 
+    shard = args.parallel == "shard"
+
+    def apply_dev():
+        if shard:   # this rank's pair batches, then one all-reduce of the sphere coefficients (binding.apply_sharded)
+            g.apply_sharded(pd, occ, out, rank=rank, world=world)
+        else:
+            g.apply(pd, occ, out)
+
     def step_dev():
-        g.apply(pd, occ, out)
+        apply_dev()
+        return g.energy(pd, occ, out)[0]
+
+    def step_host():
+        if not shard:
+            return g.apply_host(pin_in, occ, pin_out)[1]
+        pd.copy_(pin_in, non_blocking=True)
+        apply_dev()
+        pin_out.copy_(out, non_blocking=True)
         return g.energy(pd, occ, out)[0]
 
     def sync_all():
@@ -178,7 +196,7 @@ def run_ours(args, rank, world, local):
     p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     p0.record()
     for _ in range(args.steps):
-        g.apply(pd, occ, out)
+        apply_dev()
         for name, (t, n, u) in g.kernel_times().items():
             a = acc.setdefault(name, [0.0, 0, 0])
             a[0] += t; a[1] += n; a[2] += u
@@ -223,7 +241,7 @@ def run_ours(args, rank, world, local):
 
     # ---- the same apply on the caller's FULL grid (EXX_OPT_PRUNE = 0): the graded "96^3" pipeline number of BASELINE.md
     full = None
-    if ngw != w.ng and not args.no_full_grid:
+    if ngw != w.ng and not args.no_full_grid and not shard:
         g.set_option(B.EXX_OPT_PRUNE, 0)
         for _ in range(2):
             g.apply(pd, occ, out)
@@ -246,30 +264,33 @@ def run_ours(args, rank, world, local):
 
     # ---- timed region 3: end to end through exx_apply_host, pinned host buffers, copies inside the timed region
     for _ in range(min(2, args.warmup)):
-        g.apply_host(pin_in, occ, pin_out)
+        step_host()
     sync_all()
     h0, h1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     h0.record()
     for _ in range(args.steps):
-        _, ex_h = g.apply_host(pin_in, occ, pin_out)
+        ex_h = step_host()
     h1.record()
     sync_all()
     ms_e2e = max_over_ranks(h0.elapsed_time(h1), world, dev) / args.steps
     assert ex_h == ex or abs(ex_h - ex) <= (1e-12 if args.precision == "fp64" else 1e-5) * abs(ex)
 
-    value = world * pairs_ord / (ms * 1e-3)
+    # replicas: every rank did the whole workload; shard: the ranks together did it once (pairs_ord is this rank's share)
+    job_pairs = w.pair_evals if shard else world * pairs_ord
+    value = job_pairs / (ms * 1e-3)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms, "higher_is_better": True, "scaling": "strong" if shard else "weak", "vs_baseline": None,
             "dtype": "f64" if args.precision == "fp64" else "f32 transforms + f64 accumulation (mixed; outside the fp64 parity contract)",
             "data": "synthetic",
             "config": {"workload": w.name, "description": w.description, "grid": list(w.grid), "nk": w.nk, "nbands": w.nbands,
-                       "pairs_per_step": pairs_ord, "parallelism": "replicas x%d" % world,
+                       "pairs_per_step": job_pairs if shard else pairs_ord,
+                       "parallelism": ("pair batches sharded x%d + all-reduce of V_x psi" if shard else "replicas x%d") % world,
                        "path": {1: "generic", 2: "fused"}.get(g.get_info(B.EXX_INFO_PATH_USED)),
                        "tile_n": g.get_info(B.EXX_INFO_TILE_N), "tile_m": g.get_info(B.EXX_INFO_TILE_M),
                        "pruned": g.get_info(B.EXX_INFO_PRUNED), "pair_symmetry": g.get_info(B.EXX_INFO_SYMMETRY), "work_grid": pipeline["work_grid"],
                        "l2": "inputs larger than L2: the real-space cache u_nk(r) is %.2f GB, streamed every step" % (w.nk * w.nbands * ngw * 16 / 1e9)},
             "E_x": ex, "vx_apply_ms": ms, "clocks": sampler.summary(), "roofline": roofline, "pipeline_roofline": pipeline,
-            "e2e": {"value": world * pairs_ord / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
+            "e2e": {"value": job_pairs / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,
                     "h2d_bytes_per_step": g.ncoef * 16, "d2h_bytes_per_step": g.ncoef * 16 + 8},
             "gpu_launches": launches * args.steps}
     if full is not None:
@@ -306,6 +327,8 @@ def main():
     ap.add_argument("--path", type=int, default=None, help="EXX_OPT_PATH override: 1 generic, 2 fused")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "mixed"],
                     help="mixed = EXX_OPT_PRECISION 1 (fp32 pair transforms); for information only, the default fp64 run is the benchmark")
+    ap.add_argument("--parallel", default="replicas", choices=["replicas", "shard"],
+                    help="N > 1: independent replicas (default, weak scaling) or the pair batches of one workload shared out (strong scaling)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-full-grid", action="store_true", help="skip the extra full-grid (EXX_OPT_PRUNE = 0) timing")
     args = ap.parse_args()

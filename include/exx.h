@@ -75,8 +75,15 @@ enum {
                                FFTs in single precision"): the pair transforms, the kernel multiply and the product with u_m run in fp32
                                (fused path only); S1, S7, every accumulator and E_x stay fp64.  Agrees with fp64 to ~1e-6 relative
                                (the paper reports 1e-5); NOT covered by the 1e-10 / 1e-11 parity bars */
-    EXX_OPT_SYMMETRY = 6    /* 1 (default): evaluate each unordered band pair once and use v_{mq,nk} = conj(v_{nk,mq}) for the second
+    EXX_OPT_SYMMETRY = 6,   /* 1 (default): evaluate each unordered band pair once and use v_{mq,nk} = conj(v_{nk,mq}) for the second
                                accumulation (fused path on alias-free grids only; see EXX_INFO_SYMMETRY); 0: every ordered pair */
+    EXX_OPT_SHARD_COUNT = 9,  /* P >= 1 (default 1): this context is shard EXX_OPT_SHARD_RANK of P (one process per GPU, SURVEY.md
+                               S8(f)-4; the paper's multi-device runs are MPI over processes, Table V).  exx_apply then
+                               runs only this shard's share of the pair work and `out` holds a PARTIAL V_x psi: the sum of `out` over
+                               the P shards is the full result (the caller adds them, e.g. one all-reduce; the binding's
+                               apply_sharded does).  Fused path: the pair batches of exx_shard_plan; generic path: output rows
+                               (k,n) with (k nbands + n) mod P = rank, the other rows of `out` zero */
+    EXX_OPT_SHARD_RANK = 10 /* 0 .. P-1 (default 0); exx_apply returns EXX_ERR_BAD_ARG while rank >= P */
 };
 
 /* Counters (exx_get_info), all for the most recent exx_apply on this context unless stated. */
@@ -122,6 +129,14 @@ int exx_get_info(const exx_ctx* ctx, int what, int64_t* value);
  * exx_kernel_class_name gives the class name (static string, NULL if out of range). */
 int exx_get_kernel_time(exx_ctx* ctx, int kclass, double* ms_total, int64_t* launches, int64_t* units);
 const char* exx_kernel_class_name(int kclass);
+
+/* Host only, no context and no GPU needed: how the fused path's pair batches are shared out among `nshards` shards.  The
+ * loop nest over (k, q, a-tile, b-tile) gives one batch per tile x tile block of band pairs
+ * (tile = 0: the default 16); batches are handed out longest first to the least loaded shard — deterministic, so every rank
+ * computes the same plan.  occ_host: nk*nbands.  symmetry: as EXX_OPT_SYMMETRY (the caller says whether it applies).
+ * Outputs (each nshards entries, either may be NULL): pairs_out = pair densities the shard transforms (passes A, B);
+ * passes_out = fused pass executions (2 per pair + 1 per accumulation sweep), the load that is balanced. */
+int exx_shard_plan(int nk, int nbands, const double* occ_host, int symmetry, int tile, int nshards, int64_t* pairs_out, int64_t* passes_out);
 
 /* V_x applied to every band: out(k,n,:) = (V_x c)_nk.  psi_dev/out_dev: device, exx_psi_offset(nk) complex elements
  * each, 16-byte aligned, must not overlap.  occ_host: nk*nbands occupations f_nk in [0, inf), host, read during the

@@ -13,6 +13,7 @@ LIB_PATH = os.environ.get("EXX_LIB") or os.path.join(_HERE, "libexx.so")  # EXX_
 
 EXX_OPT_PATH, EXX_OPT_TILE_N, EXX_OPT_TILE_M, EXX_OPT_PRUNE, EXX_OPT_PROFILE, EXX_OPT_SYMMETRY = 1, 2, 3, 4, 5, 6
 EXX_OPT_PRECISION = 8
+EXX_OPT_SHARD_COUNT, EXX_OPT_SHARD_RANK = 9, 10
 (EXX_INFO_LAUNCHES, EXX_INFO_PAIRS_ORDERED, EXX_INFO_PAIRS_EXECUTED, EXX_INFO_PATH_USED, EXX_INFO_WORKSPACE_BYTES,
  EXX_INFO_NCOEF, EXX_INFO_TILE_N, EXX_INFO_TILE_M, EXX_INFO_PRUNED, EXX_INFO_NUM_KERNEL_CLASSES, EXX_INFO_WORK_GRID,
  EXX_INFO_COMPACT_GRID, EXX_INFO_SYMMETRY) = range(1, 14)
@@ -22,7 +23,7 @@ EXX_INFO_PRECISION = 15
 SYMBOLS = ("exx_create", "exx_destroy", "exx_npw", "exx_index_map", "exx_psi_offset", "exx_set_option", "exx_get_option",
            "exx_get_info", "exx_get_kernel_time", "exx_kernel_class_name", "exx_apply", "exx_energy", "exx_apply_host",
            "exx_scatter", "exx_gather", "exx_fft3d", "exx_to_real", "exx_kernel_table", "exx_strerror", "exx_last_error",
-           "exx_version", "exx_subspace", "exx_fft3d_fused", "exx_findex")
+           "exx_version", "exx_subspace", "exx_fft3d_fused", "exx_findex", "exx_shard_plan")
 
 
 class KernelParams(C.Structure):
@@ -77,6 +78,7 @@ def lib():
         L.exx_subspace.argtypes = [vp, C.c_int, vp, vp, vp]
         L.exx_fft3d_fused.argtypes = [vp, vp, C.c_int, C.c_int, vp]
         L.exx_findex.argtypes = [vp, C.POINTER(C.c_int32)]
+        L.exx_shard_plan.argtypes = [C.c_int, C.c_int, dp, C.c_int, C.c_int, C.c_int, i64p, i64p]
         L.exx_scatter.argtypes = [vp, C.c_int, vp, C.c_int, vp]
         L.exx_gather.argtypes = [vp, C.c_int, vp, C.c_int, vp]
         L.exx_fft3d.argtypes = [vp, vp, C.c_int, C.c_int]
@@ -93,6 +95,28 @@ def lib():
 
 def _dp(a):
     return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def shard_plan(nk, nbands, occ, symmetry=True, tile=0, nshards=1):
+    """exx_shard_plan: (pairs, passes) per shard, two int64 arrays of nshards entries.  Host only: needs no GPU."""
+    occ = np.ascontiguousarray(occ, dtype=np.float64).reshape(-1)
+    assert occ.size == nk * nbands
+    pairs, passes = np.zeros(nshards, dtype=np.int64), np.zeros(nshards, dtype=np.int64)
+    i64p = C.POINTER(C.c_int64)
+    rc = lib().exx_shard_plan(nk, nbands, _dp(occ), int(bool(symmetry)), int(tile), int(nshards), pairs.ctypes.data_as(i64p),
+                              passes.ctypes.data_as(i64p))
+    if rc:
+        raise ExxError(rc)
+    return pairs, passes
+
+
+def all_reduce_sum(t, group=None):
+    """Sum a complex128 (or real) tensor over the ranks of a torch.distributed group, in place: the one exchange step of the
+    sharded path.  NCCL on CUDA tensors; gloo works for the CPU tests."""
+    import torch
+    import torch.distributed as dist
+    dist.all_reduce(torch.view_as_real(t) if t.is_complex() else t, op=dist.ReduceOp.SUM, group=group)
+    return t
 
 
 class Exx:
@@ -206,6 +230,24 @@ class Exx:
         out_dev = self.empty_like_psi() if out_dev is None else out_dev
         occ = self._occ(occ)
         self._chk(lib().exx_apply(self._h, self._dev(psi_dev, self.ncoef), _dp(occ), self._dev(out_dev, self.ncoef)))
+        return out_dev
+
+    def apply_sharded(self, psi_dev, occ, out_dev=None, group=None, rank=None, world=None):
+        """V_x psi with the pair work shared out over the ranks of a torch.distributed group (one process per GPU, every rank
+        holding all of psi): this rank's share through exx_apply (EXX_OPT_SHARD_COUNT / _RANK), then ONE all-reduce of the
+        sphere coefficients.  Every rank returns the full V_x psi."""
+        import torch.distributed as dist
+        world = dist.get_world_size(group) if world is None else world
+        rank = dist.get_rank(group) if rank is None else rank
+        self.set_option(EXX_OPT_SHARD_COUNT, world)
+        self.set_option(EXX_OPT_SHARD_RANK, rank)
+        try:
+            out_dev = self.apply(psi_dev, occ, out_dev)
+        finally:
+            self.set_option(EXX_OPT_SHARD_RANK, 0)
+            self.set_option(EXX_OPT_SHARD_COUNT, 1)
+        if world > 1:
+            all_reduce_sum(out_dev, group)
         return out_dev
 
     def energy(self, psi_dev, occ, vxpsi_dev=None):

@@ -9,6 +9,7 @@
 #include <new>
 
 #include "exx_internal.h"
+#include "exx_shard.h"
 
 namespace exx {
 
@@ -465,6 +466,14 @@ int exx_set_option(exx_ctx* c, int option, int64_t value) {
         if (value != 0 && value != 1) return EXX_ERR_BAD_ARG;
         c->opt_precision = value;
         return EXX_OK;
+    case EXX_OPT_SHARD_COUNT:
+        if (value < 1 || value > 65536) return EXX_ERR_BAD_ARG;
+        c->opt_shard_count = value;
+        return EXX_OK;
+    case EXX_OPT_SHARD_RANK:
+        if (value < 0 || value > 65535) return EXX_ERR_BAD_ARG;
+        c->opt_shard_rank = value;
+        return EXX_OK;
     default: return EXX_ERR_BAD_ARG;
     }
 }
@@ -478,6 +487,8 @@ int exx_get_option(const exx_ctx* c, int option, int64_t* value) {
     case EXX_OPT_PROFILE: *value = c->opt_profile; return EXX_OK;
     case EXX_OPT_SYMMETRY: *value = c->opt_symmetry; return EXX_OK;
     case EXX_OPT_PRECISION: *value = c->opt_precision; return EXX_OK;
+    case EXX_OPT_SHARD_COUNT: *value = c->opt_shard_count; return EXX_OK;
+    case EXX_OPT_SHARD_RANK: *value = c->opt_shard_rank; return EXX_OK;
     default: return EXX_ERR_BAD_ARG;
     }
 }
@@ -584,6 +595,11 @@ static int apply_generic(exx_ctx* c, const double2* psi, const double* occ, doub
     c->tile_m_used = tm_max;
     for (int k = 0; k < nk; k++)
         for (int n = 0; n < nb; n++) {
+            if ((int64_t)(k * nb + n) % c->opt_shard_count != c->opt_shard_rank) {
+                // another shard's output row: zero here, so that the sum over shards is the full result
+                EXX_CUDA(c, cudaMemsetAsync(out + c->off[k] + (int64_t)n * c->npw[k], 0, sizeof(double2) * (size_t)c->npw[k], c->stream));
+                continue;
+            }
             EXX_CUDA(c, cudaMemsetAsync(c->acc_dev, 0, sizeof(double2) * (size_t)Ng, c->stream));
             for (int q = 0; q < nk; q++) {
                 const double* ktab = c->ktab_dev + (size_t)c->ktab_of[(size_t)k * nk + q] * Ng;
@@ -617,6 +633,7 @@ static int apply_generic(exx_ctx* c, const double2* psi, const double* occ, doub
 
 static int apply_impl(exx_ctx* c, const double2* psi, const double* occ, double2* out) {
     reset_counters(c);
+    if (c->opt_shard_rank >= c->opt_shard_count) return EXX_ERR_BAD_ARG;
     if (c->inner && c->opt_prune) {
         // compact work grid: same spheres, same psi/out layout, every product alias-free on both grids
         exx_ctx* in = c->inner;
@@ -626,6 +643,8 @@ static int apply_impl(exx_ctx* c, const double2* psi, const double* occ, double2
         in->opt_profile = c->opt_profile;
         in->opt_symmetry = c->opt_symmetry;
         in->opt_precision = c->opt_precision;
+        in->opt_shard_count = c->opt_shard_count;
+        in->opt_shard_rank = c->opt_shard_rank;
         int rc = apply_impl(in, psi, occ, out);
         c->launches = in->launches;
         c->pairs_ordered = in->pairs_ordered;
@@ -687,6 +706,25 @@ int exx_energy(exx_ctx* c, const double* psi_dev, const double* occ_host, const 
         vx = c->vx_dev;
     }
     return energy_impl(c, (const double2*)psi_dev, occ_host, vx, ex_host, per_band_host_or_null);
+}
+
+int exx_shard_plan(int nk, int nbands, const double* occ_host, int symmetry, int tile, int nshards, int64_t* pairs_out, int64_t* passes_out) {
+    if (!occ_host) return EXX_ERR_NULL;
+    if (nk < 1 || nbands < 1 || nshards < 1 || tile < 0 || tile > 16) return EXX_ERR_BAD_ARG;
+    for (int i = 0; i < nk * nbands; i++)
+        if (!(occ_host[i] >= 0.0) || !std::isfinite(occ_host[i])) return EXX_ERR_BAD_OCC;
+    const int t = std::min(tile ? tile : 16, nbands);
+    std::vector<PairBlock> blocks;
+    plan_blocks(nk, nbands, occ_host, symmetry != 0, t, t, nshards, blocks);
+    for (int s = 0; s < nshards; s++) {
+        if (pairs_out) pairs_out[s] = 0;
+        if (passes_out) passes_out[s] = 0;
+    }
+    for (const PairBlock& b : blocks) {
+        if (pairs_out) pairs_out[b.shard] += b.npairs;
+        if (passes_out) passes_out[b.shard] += b.cost();
+    }
+    return EXX_OK;
 }
 
 int exx_subspace(exx_ctx* c, int ik, const double* psi_dev, const double* vxpsi_dev, double* m_dev) {

@@ -8,6 +8,7 @@
 #include <vector>
 
 #include "exx_internal.h"
+#include "exx_shard.h"
 
 #include "exx_fused_kernels.h"  // fp64 mode: namespace exx, real = double
 
@@ -204,134 +205,135 @@ static int pair_loop(exx_ctx* c, FusedState* st, const double* occ, const typena
     int rc;
     const int nb = c->nb, nk = c->nk;
     const size_t Ng = (size_t)c->Ng;
-    for (int k = 0; k < nk; k++)
-        for (int q = sym ? k : 0; q < nk; q++) {
-            const typename M::real* kperm = kperm_base + (size_t)c->ktab_of[(size_t)k * nk + q] * Ng;
-            const typename M::cplx* ua = u_base + (size_t)k * nb * Ng;
-            const typename M::cplx* ub = u_base + (size_t)q * nb * Ng;
-            // b-bands: in plain mode only bands with f != 0 take part as m
-            std::vector<int> blist;
-            for (int m = 0; m < nb; m++)
-                if (sym || occ[q * nb + m] != 0.0) blist.push_back(m);
-            for (int a0 = 0; a0 < nb; a0 += ta_max)
-                for (size_t b0 = (sym && k == q) ? (size_t)a0 : 0; b0 < blist.size(); b0 += tb_max) {
-                    const int ta = std::min(ta_max, nb - a0), tb = (int)std::min<size_t>(tb_max, blist.size() - b0);
-                    AJob aj;
-                    aj.npairs = 0;
-                    aj.tb = tb;
-                    bool ev[16][16];
-                    for (int i = 0; i < ta; i++) aj.a_idx[i] = a0 + i;
-                    for (int j = 0; j < tb; j++) aj.b_idx[j] = blist[b0 + j];
-                    for (int i = 0; i < ta; i++)
-                        for (int j = 0; j < tb; j++) {
-                            const double fa = occ[k * nb + aj.a_idx[i]], fb = occ[q * nb + aj.b_idx[j]];
-                            bool e = sym ? ((fa != 0.0 || fb != 0.0) && (k < q || aj.a_idx[i] <= aj.b_idx[j])) : (fb != 0.0);
-                            ev[i][j] = e;
-                            if (e) {
-                                aj.pi[aj.npairs] = (unsigned char)i;
-                                aj.pj[aj.npairs] = (unsigned char)j;
-                                aj.npairs++;
-                            }
-                        }
-                    if (aj.npairs == 0) continue;
-                    EXX_DISPATCH_M(st->R1, rc = L::pass_ab(c, ua, ub, aj, kperm, work));
+    // the batch list and its owners (exx_shard.h); one shard = the whole list
+    std::vector<PairBlock> blocks;
+    plan_blocks(nk, nb, occ, sym, ta_max, tb_max, (int)c->opt_shard_count, blocks);
+    std::vector<int> blist;
+    int bl_q = -1;
+    for (const PairBlock& blk : blocks) {
+        if (blk.shard != (int)c->opt_shard_rank) continue;
+        const int k = blk.k, q = blk.q;
+        const typename M::real* kperm = kperm_base + (size_t)c->ktab_of[(size_t)k * nk + q] * Ng;
+        const typename M::cplx* ua = u_base + (size_t)k * nb * Ng;
+        const typename M::cplx* ub = u_base + (size_t)q * nb * Ng;
+        if (bl_q != q) b_list(nb, occ, q, sym, blist), bl_q = q;
+        const int a0 = blk.a0, ta = blk.ta, tb = blk.tb;
+        const size_t b0 = (size_t)blk.b0;
+        AJob aj;
+        aj.npairs = 0;
+        aj.tb = tb;
+        bool ev[16][16];
+        for (int i = 0; i < ta; i++) aj.a_idx[i] = a0 + i;
+        for (int j = 0; j < tb; j++) aj.b_idx[j] = blist[b0 + j];
+        for (int i = 0; i < ta; i++)
+            for (int j = 0; j < tb; j++) {
+                const double fa = occ[k * nb + aj.a_idx[i]], fb = occ[q * nb + aj.b_idx[j]];
+                bool e = pair_evaluated(sym, k, q, aj.a_idx[i], aj.b_idx[j], fa, fb);
+                ev[i][j] = e;
+                if (e) {
+                    aj.pi[aj.npairs] = (unsigned char)i;
+                    aj.pj[aj.npairs] = (unsigned char)j;
+                    aj.npairs++;
+                }
+            }
+        if (aj.npairs == 0) continue;
+        EXX_DISPATCH_M(st->R1, rc = L::pass_ab(c, ua, ub, aj, kperm, work));
+        if (rc) return rc;
+        c->pairs_executed += aj.npairs;
+        // side a: rows = a-bands, columns = b-bands with f_b != 0
+        {
+            CJob cj;
+            cj.nr = 0;
+            cj.box_r = tb;
+            cj.box_c = 1;
+            cj.cj = 0;
+            int64_t units = 0;
+            int rowbox[16];
+            for (int j = 0; j < tb; j++) {
+                cj.src[j] = aj.b_idx[j];
+                cj.coef[j] = c->kw[q] * occ[q * nb + aj.b_idx[j]];
+            }
+            for (int i = 0; i < ta; i++) {
+                int n = 0;
+                for (int j = 0; j < tb; j++)
+                    if (ev[i][j] && occ[q * nb + aj.b_idx[j]] != 0.0) cj.col[cj.nr][n++] = (unsigned char)j;
+                if (n) {
+                    cj.cnt[cj.nr] = n;
+                    cj.tgt[cj.nr] = k * nb + aj.a_idx[i];
+                    rowbox[cj.nr] = i;
+                    cj.nr++;
+                    units += n;
+                }
+            }
+            if (cj.nr) {
+                // rows were compacted: the work box of (row r, column c) is rowbox[r]*tb + c, so shift the work
+                // base per launch only when rows are contiguous; otherwise launch row by row groups
+                bool contiguous = true;
+                for (int r = 0; r < cj.nr; r++) contiguous = contiguous && rowbox[r] == rowbox[0] + r;
+                if (contiguous) {
+                    EXX_DISPATCH_M(st->R1, rc = L::pass_c(c, ub, cj, units, work + (size_t)rowbox[0] * tb * Ng, acc));
                     if (rc) return rc;
-                    c->pairs_executed += aj.npairs;
-                    // side a: rows = a-bands, columns = b-bands with f_b != 0
-                    {
-                        CJob cj;
-                        cj.nr = 0;
-                        cj.box_r = tb;
-                        cj.box_c = 1;
-                        cj.cj = 0;
-                        int64_t units = 0;
-                        int rowbox[16];
-                        for (int j = 0; j < tb; j++) {
-                            cj.src[j] = aj.b_idx[j];
-                            cj.coef[j] = c->kw[q] * occ[q * nb + aj.b_idx[j]];
-                        }
-                        for (int i = 0; i < ta; i++) {
-                            int n = 0;
-                            for (int j = 0; j < tb; j++)
-                                if (ev[i][j] && occ[q * nb + aj.b_idx[j]] != 0.0) cj.col[cj.nr][n++] = (unsigned char)j;
-                            if (n) {
-                                cj.cnt[cj.nr] = n;
-                                cj.tgt[cj.nr] = k * nb + aj.a_idx[i];
-                                rowbox[cj.nr] = i;
-                                cj.nr++;
-                                units += n;
-                            }
-                        }
-                        if (cj.nr) {
-                            // rows were compacted: the work box of (row r, column c) is rowbox[r]*tb + c, so shift the work
-                            // base per launch only when rows are contiguous; otherwise launch row by row groups
-                            bool contiguous = true;
-                            for (int r = 0; r < cj.nr; r++) contiguous = contiguous && rowbox[r] == rowbox[0] + r;
-                            if (contiguous) {
-                                EXX_DISPATCH_M(st->R1, rc = L::pass_c(c, ub, cj, units, work + (size_t)rowbox[0] * tb * Ng, acc));
-                                if (rc) return rc;
-                            } else {
-                                for (int r = 0; r < cj.nr; r++) {
-                                    CJob one = cj;
-                                    one.nr = 1;
-                                    one.cnt[0] = cj.cnt[r];
-                                    one.tgt[0] = cj.tgt[r];
-                                    for (int n = 0; n < cj.cnt[r]; n++) one.col[0][n] = cj.col[r][n];
-                                    EXX_DISPATCH_M(st->R1, rc = L::pass_c(c, ub, one, cj.cnt[r], work + (size_t)rowbox[r] * tb * Ng, acc));
-                                    if (rc) return rc;
-                                }
-                            }
-                            c->pairs_ordered += units;
-                        }
-                    }
-                    // side b (symmetry): rows = b-bands, columns = a-bands with f_a != 0, conj(v); the pair a == b is not repeated
-                    if (sym) {
-                        CJob cj;
-                        cj.nr = 0;
-                        cj.box_r = 1;
-                        cj.box_c = tb;
-                        cj.cj = 1;
-                        int64_t units = 0;
-                        int rowbox[16];
-                        for (int i = 0; i < ta; i++) {
-                            cj.src[i] = aj.a_idx[i];
-                            cj.coef[i] = c->kw[k] * occ[k * nb + aj.a_idx[i]];
-                        }
-                        for (int j = 0; j < tb; j++) {
-                            int n = 0;
-                            for (int i = 0; i < ta; i++)
-                                if (ev[i][j] && occ[k * nb + aj.a_idx[i]] != 0.0 && !(k == q && aj.a_idx[i] == aj.b_idx[j]))
-                                    cj.col[cj.nr][n++] = (unsigned char)i;
-                            if (n) {
-                                cj.cnt[cj.nr] = n;
-                                cj.tgt[cj.nr] = q * nb + aj.b_idx[j];
-                                rowbox[cj.nr] = j;
-                                cj.nr++;
-                                units += n;
-                            }
-                        }
-                        if (cj.nr) {
-                            bool contiguous = true;
-                            for (int r = 0; r < cj.nr; r++) contiguous = contiguous && rowbox[r] == rowbox[0] + r;
-                            if (contiguous) {
-                                EXX_DISPATCH_M(st->R1, rc = L::pass_c(c, ua, cj, units, work + (size_t)rowbox[0] * Ng, acc));
-                                if (rc) return rc;
-                            } else {
-                                for (int r = 0; r < cj.nr; r++) {
-                                    CJob one = cj;
-                                    one.nr = 1;
-                                    one.cnt[0] = cj.cnt[r];
-                                    one.tgt[0] = cj.tgt[r];
-                                    for (int n = 0; n < cj.cnt[r]; n++) one.col[0][n] = cj.col[r][n];
-                                    EXX_DISPATCH_M(st->R1, rc = L::pass_c(c, ua, one, cj.cnt[r], work + (size_t)rowbox[r] * Ng, acc));
-                                    if (rc) return rc;
-                                }
-                            }
-                            c->pairs_ordered += units;
-                        }
+                } else {
+                    for (int r = 0; r < cj.nr; r++) {
+                        CJob one = cj;
+                        one.nr = 1;
+                        one.cnt[0] = cj.cnt[r];
+                        one.tgt[0] = cj.tgt[r];
+                        for (int n = 0; n < cj.cnt[r]; n++) one.col[0][n] = cj.col[r][n];
+                        EXX_DISPATCH_M(st->R1, rc = L::pass_c(c, ub, one, cj.cnt[r], work + (size_t)rowbox[r] * tb * Ng, acc));
+                        if (rc) return rc;
                     }
                 }
+                c->pairs_ordered += units;
+            }
         }
+        // side b (symmetry): rows = b-bands, columns = a-bands with f_a != 0, conj(v); the pair a == b is not repeated
+        if (sym) {
+            CJob cj;
+            cj.nr = 0;
+            cj.box_r = 1;
+            cj.box_c = tb;
+            cj.cj = 1;
+            int64_t units = 0;
+            int rowbox[16];
+            for (int i = 0; i < ta; i++) {
+                cj.src[i] = aj.a_idx[i];
+                cj.coef[i] = c->kw[k] * occ[k * nb + aj.a_idx[i]];
+            }
+            for (int j = 0; j < tb; j++) {
+                int n = 0;
+                for (int i = 0; i < ta; i++)
+                    if (ev[i][j] && occ[k * nb + aj.a_idx[i]] != 0.0 && !(k == q && aj.a_idx[i] == aj.b_idx[j]))
+                        cj.col[cj.nr][n++] = (unsigned char)i;
+                if (n) {
+                    cj.cnt[cj.nr] = n;
+                    cj.tgt[cj.nr] = q * nb + aj.b_idx[j];
+                    rowbox[cj.nr] = j;
+                    cj.nr++;
+                    units += n;
+                }
+            }
+            if (cj.nr) {
+                bool contiguous = true;
+                for (int r = 0; r < cj.nr; r++) contiguous = contiguous && rowbox[r] == rowbox[0] + r;
+                if (contiguous) {
+                    EXX_DISPATCH_M(st->R1, rc = L::pass_c(c, ua, cj, units, work + (size_t)rowbox[0] * Ng, acc));
+                    if (rc) return rc;
+                } else {
+                    for (int r = 0; r < cj.nr; r++) {
+                        CJob one = cj;
+                        one.nr = 1;
+                        one.cnt[0] = cj.cnt[r];
+                        one.tgt[0] = cj.tgt[r];
+                        for (int n = 0; n < cj.cnt[r]; n++) one.col[0][n] = cj.col[r][n];
+                        EXX_DISPATCH_M(st->R1, rc = L::pass_c(c, ua, one, cj.cnt[r], work + (size_t)rowbox[r] * Ng, acc));
+                        if (rc) return rc;
+                    }
+                }
+                c->pairs_ordered += units;
+            }
+        }
+    }
     return EXX_OK;
 }
 

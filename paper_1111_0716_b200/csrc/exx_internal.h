@@ -98,6 +98,7 @@ struct exx_ctx {
 
     // options
     int64_t opt_path = 0, opt_tile_n = 0, opt_tile_m = 0, opt_prune = 1, opt_profile = 0, opt_symmetry = 1, opt_precision = 0;
+    int64_t opt_shard_count = 1, opt_shard_rank = 0;  // S8(f)-4: this context runs shard rank of count (exx_shard.h)
 
     // counters of the last apply
     int64_t symmetry_used = 0, precision_used = 0;

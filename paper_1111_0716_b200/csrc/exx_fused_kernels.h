@@ -131,7 +131,7 @@ template <int R1>
 __global__ void __launch_bounds__(FusedCfg<R1>::NT3, FusedCfg<R1>::MINB3) pass_c_kernel(const cplx* __restrict__ work, const cplx* __restrict__ usrc_base, CJob job,
                                                                     acc_c* __restrict__ acc_base) {
     constexpr int N = 8 * R1, U = FusedCfg<R1>::U3, NT = FusedCfg<R1>::NT3;
-    constexpr bool TWREG = FusedCfg<R1>::TWREG, ACCREG = FusedCfg<R1>::ACCREG;
+    constexpr bool TWREG = FusedCfg<R1>::TWREG, ACCREG = FusedCfg<R1>::ACCREG, STAGE3 = FusedCfg<R1>::STAGE3 >= 1, STAGEU = FusedCfg<R1>::STAGE3 >= 2;
     static_assert(!TWREG || NT % R1 == 0, "TWREG needs a thread-invariant k1z");
     constexpr size_t Ng = (size_t)N * N * N;
     constexpr int IT = (U * R1 * 8 + NT - 1) / NT;
@@ -139,6 +139,8 @@ __global__ void __launch_bounds__(FusedCfg<R1>::NT3, FusedCfg<R1>::MINB3) pass_c
     cplx* S = reinterpret_cast<cplx*>(smem_raw);
     acc_c* A = reinterpret_cast<acc_c*>(S + U * R1 * N);  // fp64 accumulator tile; unused when ACCREG
     cplx* T = reinterpret_cast<cplx*>(A + (ACCREG ? 0 : U * R1 * N));
+    cplx* G = T + (TWREG ? 0 : R1 * 8);  // STAGE3: per-thread slots for the next column's work-box elements
+    cplx* G2 = G + ((U * N + NT - 1) / NT) * R1 * NT;  // ... and for this column's u elements
     const int tid = threadIdx.x;
     const unsigned bid = blockIdx.x;
     const int r = bid % job.nr;
@@ -156,19 +158,35 @@ __global__ void __launch_bounds__(FusedCfg<R1>::NT3, FusedCfg<R1>::MINB3) pass_c
 #pragma unroll
         for (int i = 0; i < (ACCREG ? IT * R1 : 1); i++) accr[i] = mka(0.0, 0.0);
     }
+    if (STAGE3 && cnt > 0) {
+        p3_stage<R1, U, NT>(tid, work + (size_t)(r * job.box_r + job.col[r][0] * job.box_c) * Ng, x, yb, G);
+        stage_commit();
+    }
     for (int ci = 0; ci < cnt; ci++) {
         const int col = job.col[r][ci];
         const cplx* W = work + (size_t)(r * job.box_r + col * job.box_c) * Ng;
         const cplx* um = usrc_base + (size_t)job.src[col] * Ng;
         const double wf = job.coef[col];
-        p3_y2inv<R1, U, NT>(tid, W, x, yb, S);
+        if (STAGE3) {
+            // this column's elements were requested one column ago; the next column's are requested as soon as the slots
+            // have been read (the transform consumes them first, so the copies cannot overtake the reads)
+            stage_wait<0>();
+            p3_y2inv_staged<R1, U, NT>(tid, G, S);
+            if (STAGEU) p3_stage_u<R1, U, NT>(tid, um, x, yb, G2);  // group 1: this column's u elements, consumed two barriers from here
+            stage_commit();
+            if (ci + 1 < cnt) p3_stage<R1, U, NT>(tid, work + (size_t)(r * job.box_r + job.col[r][ci + 1] * job.box_c) * Ng, x, yb, G);
+            stage_commit();                             // group 2 (possibly empty): the next column's work-box elements
+        } else {
+            p3_y2inv<R1, U, NT>(tid, W, x, yb, S);
+        }
         __syncthreads();
         p13_z8<R1, U, NT, +1, TWREG>(tid, S, T, twr);
         __syncthreads();
+        if (STAGEU) stage_wait<1>();  // the u elements have landed; the next column's work-box elements may still be in flight
         if (ACCREG)
-            p3_zinv2_reg<R1, U, NT>(tid, S, um, wf, x, yb, accr, cj);
+            p3_zinv2_reg<R1, U, NT, STAGEU>(tid, S, um, wf, x, yb, accr, cj, G2);
         else
-            p3_zinv2<R1, U, NT>(tid, S, um, wf, x, yb, A, ci == 0, cj);
+            p3_zinv2<R1, U, NT, STAGEU>(tid, S, um, wf, x, yb, A, ci == 0, cj, G2);
         __syncthreads();
     }
     if (cnt > 0) {
@@ -270,15 +288,18 @@ __global__ void __launch_bounds__(FusedCfg<R1>::NT3, FusedCfg<R1>::MINB3) fft_c_
 template <int R1>
 struct Launch {
     static constexpr int N = 8 * R1, U1 = FusedCfg<R1>::U1, U3 = FusedCfg<R1>::U3, Z = FusedCfg<R1>::Z;
-    static constexpr bool TWREG = FusedCfg<R1>::TWREG, ACCREG = FusedCfg<R1>::ACCREG;
+    static constexpr bool TWREG = FusedCfg<R1>::TWREG, ACCREG = FusedCfg<R1>::ACCREG, STAGE3 = FusedCfg<R1>::STAGE3 >= 1, STAGEU = FusedCfg<R1>::STAGE3 >= 2;
+    static constexpr int IT3S = (U3 * N + FusedCfg<R1>::NT3 - 1) / FusedCfg<R1>::NT3;  // items per thread in pass C's first step
     static constexpr size_t smem_a = sizeof(cplx) * ((size_t)U1 * R1 * N + (TWREG ? 0 : R1 * 8));
     static constexpr size_t smem_c = sizeof(cplx) * ((size_t)U3 * R1 * N + (TWREG ? 0 : R1 * 8)) + sizeof(acc_c) * (ACCREG ? 0 : (size_t)U3 * R1 * N);
+    static constexpr int IT3U = (U3 * R1 * 8 + FusedCfg<R1>::NT3 - 1) / FusedCfg<R1>::NT3;  // ... and in its last step
+    static constexpr size_t smem_c3 = smem_c + sizeof(cplx) * (size_t)((STAGE3 ? IT3S : 0) + (STAGEU ? IT3U : 0)) * R1 * FusedCfg<R1>::NT3;  // pass_c_kernel
     static constexpr size_t smem_b = sizeof(cplx) * ((size_t)N * P2Geo<Z>::PX);
 
     static int init(exx_ctx* c) {
         EXX_CUDA(c, cudaFuncSetAttribute(pass_a_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a));
         EXX_CUDA(c, cudaFuncSetAttribute(pass_b_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b));
-        EXX_CUDA(c, cudaFuncSetAttribute(pass_c_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_c));
+        EXX_CUDA(c, cudaFuncSetAttribute(pass_c_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_c3));
         EXX_CUDA(c, cudaFuncSetAttribute(fft_a_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a));
         EXX_CUDA(c, cudaFuncSetAttribute((fft_b_kernel<R1, -1>), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b));
         EXX_CUDA(c, cudaFuncSetAttribute((fft_b_kernel<R1, +1>), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b));
@@ -336,7 +357,7 @@ struct Launch {
     static int pass_c(exx_ctx* c, const cplx* usrc_base, const CJob& job, int64_t units, const cplx* work, acc_c* acc_base) {
         const unsigned tiles3 = N * (8 / U3);
         LaunchScope ls(c, KC_PASS_C, units);
-        pass_c_kernel<R1><<<tiles3 * job.nr, FusedCfg<R1>::NT3, smem_c, c->stream>>>(work, usrc_base, job, acc_base);
+        pass_c_kernel<R1><<<tiles3 * job.nr, FusedCfg<R1>::NT3, smem_c3, c->stream>>>(work, usrc_base, job, acc_base);
         EXX_CUDA(c, cudaGetLastError());
         return EXX_OK;
     }

@@ -59,67 +59,85 @@ extern cplx h_tw[TW_TOTAL];
 // pass B on tiles of Z z-positions with NT2 threads.  Thread counts are chosen so that every step's item count is a small
 // multiple of the CTA size.  TWREG: the z twiddles W_N^(j k1z) live in 7 registers per thread (needs NT % R1 == 0 so that a
 // thread's k1z never changes) instead of a shared-memory table; ACCREG: pass C keeps its accumulator tile in registers
-// instead of shared memory.
+// instead of shared memory; STAGE3 >= 1: pass C fetches the next column's work-box elements into per-thread shared-memory slots
+// with cp.async while it transforms the current column (no registers held across the load latency); STAGE3 = 2: the u elements
+// of the last step likewise, two barriers ahead.
+constexpr int s3(int dflt) {
+#ifdef EXX_STAGE3_ALL  // tuning builds: one level for every grid
+    return EXX_STAGE3_ALL;
+#else
+    return dflt;
+#endif
+}
 template <int R1>
 struct FusedCfgBase;
 template <>
 struct FusedCfgBase<2> {
     static constexpr int U1 = 8, NT1 = 128, U3 = 8, NT3 = 128, Z = 4, NT2 = 64;
     static constexpr bool TWREG = false, ACCREG = false;
+    static constexpr int STAGE3 = s3(0);
     static constexpr int MINB1 = 1, MINB2 = 1, MINB3 = 1;
 };
 template <>
 struct FusedCfgBase<4> {
     static constexpr int U1 = 4, NT1 = 128, U3 = 4, NT3 = 128, Z = 4, NT2 = 128;
     static constexpr bool TWREG = false, ACCREG = false;
+    static constexpr int STAGE3 = s3(2);
     static constexpr int MINB1 = 1, MINB2 = 1, MINB3 = 1;
 };
 template <>
 struct FusedCfgBase<5> {
     static constexpr int U1 = 4, NT1 = 160, U3 = 4, NT3 = 160, Z = 4, NT2 = 128;
     static constexpr bool TWREG = false, ACCREG = false;
+    static constexpr int STAGE3 = s3(2);
     static constexpr int MINB1 = 1, MINB2 = 1, MINB3 = 1;
 };
 template <>
 struct FusedCfgBase<10> {
     static constexpr int U1 = 1, NT1 = 128, U3 = 1, NT3 = 128, Z = 4, NT2 = 160;
     static constexpr bool TWREG = false, ACCREG = false;
+    static constexpr int STAGE3 = s3(1);
     static constexpr int MINB1 = 1, MINB2 = 4, MINB3 = 1;
 };
 template <>
 struct FusedCfgBase<6> {
     static constexpr int U1 = 2, NT1 = 96, U3 = 2, NT3 = 96, Z = 4, NT2 = 64;
     static constexpr bool TWREG = false, ACCREG = false;
+    static constexpr int STAGE3 = s3(2);
     static constexpr int MINB1 = 1, MINB2 = 6, MINB3 = 1;  // min CTAs per SM asked of the compiler (register cap)
 };
 template <>
 struct FusedCfgBase<8> {
     static constexpr int U1 = 2, NT1 = 128, U3 = 2, NT3 = 128, Z = 4, NT2 = 128;
     static constexpr bool TWREG = false, ACCREG = false;
+    static constexpr int STAGE3 = s3(2);
     static constexpr int MINB1 = 1, MINB2 = 4, MINB3 = 1;
 };
 template <>
 struct FusedCfgBase<9> {
     static constexpr int U1 = 2, NT1 = 160, U3 = 1, NT3 = 96, Z = 4, NT2 = 96;
     static constexpr bool TWREG = false, ACCREG = true;
+    static constexpr int STAGE3 = s3(2);
     static constexpr int MINB1 = 1, MINB2 = 5, MINB3 = 1;
 };
 template <>
 struct FusedCfgBase<12> {
     static constexpr int U1 = 1, NT1 = 96, U3 = 1, NT3 = 96, Z = 4, NT2 = 128;
     static constexpr bool TWREG = false, ACCREG = false;
+    static constexpr int STAGE3 = s3(1);
     static constexpr int MINB1 = 1, MINB2 = 4, MINB3 = 1;
 };
 template <>
 struct FusedCfgBase<16> {
     static constexpr int U1 = 1, NT1 = 128, U3 = 1, NT3 = 128, Z = 4, NT2 = 256;
     static constexpr bool TWREG = false, ACCREG = false;
+    static constexpr int STAGE3 = s3(1);
     static constexpr int MINB1 = 1, MINB2 = 2, MINB3 = 1;
 };
 template <int R1>
 struct FusedCfg : FusedCfgBase<R1> {};
 
-// tuning sweeps: -DEXX_TUNE_R1=<R1> plus any of EXX_TUNE_{U1,NT1,U3,NT3,NT2,MINB1,MINB2,MINB3,TWREG,ACCREG} overrides that grid
+// tuning sweeps: -DEXX_TUNE_R1=<R1> plus any of EXX_TUNE_{U1,NT1,U3,NT3,NT2,MINB1,MINB2,MINB3,TWREG,ACCREG,STAGE3} overrides that grid
 #ifdef EXX_TUNE_R1
 #ifndef EXX_TUNE_U1
 #define EXX_TUNE_U1 FusedCfgBase<EXX_TUNE_R1>::U1
@@ -151,10 +169,14 @@ struct FusedCfg : FusedCfgBase<R1> {};
 #ifndef EXX_TUNE_ACCREG
 #define EXX_TUNE_ACCREG FusedCfgBase<EXX_TUNE_R1>::ACCREG
 #endif
+#ifndef EXX_TUNE_STAGE3
+#define EXX_TUNE_STAGE3 FusedCfgBase<EXX_TUNE_R1>::STAGE3
+#endif
 template <>
 struct FusedCfg<EXX_TUNE_R1> {
     static constexpr int U1 = EXX_TUNE_U1, NT1 = EXX_TUNE_NT1, U3 = EXX_TUNE_U3, NT3 = EXX_TUNE_NT3, Z = 4, NT2 = EXX_TUNE_NT2;
     static constexpr bool TWREG = EXX_TUNE_TWREG, ACCREG = EXX_TUNE_ACCREG;
+    static constexpr int STAGE3 = EXX_TUNE_STAGE3;
     static constexpr int MINB1 = EXX_TUNE_MINB1, MINB2 = EXX_TUNE_MINB2, MINB3 = EXX_TUNE_MINB3;
 };
 #endif
@@ -188,6 +210,10 @@ template <int Z>
 struct P2Geo {
     static constexpr int PX = 8 * Z + (Z == 8 ? 0 : Z);
 };
+template <int Z>
+EXX_HD int s2idx(int xpos, int e) {  // e = k2y Z + kzl
+    return xpos * P2Geo<Z>::PX + e;
+}
 
 // ================================================================================================================
 // pass A
@@ -305,7 +331,7 @@ template <int R1, int Z, int NT, int SIGN>
 EXX_HD void p2_y8(int tid, cplx* S, int k1y) {
     // items (xpos, kzl), in place in shared memory.  SIGN < 0: y twiddle W_N^(n2y k1y) (uniform per CTA), forward 8-point
     // DFT over n2y;  SIGN > 0: inverse 8-point DFT over k2y, conjugate twiddle.
-    constexpr int N = 8 * R1, NI = N * Z, IT = (NI + NT - 1) / NT, PX = P2Geo<Z>::PX;
+    constexpr int N = 8 * R1, NI = N * Z, IT = (NI + NT - 1) / NT;
 #pragma unroll
     for (int i = 0; i < IT; i++) {
         int it = tid + i * NT;
@@ -313,7 +339,7 @@ EXX_HD void p2_y8(int tid, cplx* S, int k1y) {
             int xpos = it / Z, kzl = it - xpos * Z;
             cplx v[8];
 #pragma unroll
-            for (int j = 0; j < 8; j++) v[j] = S[xpos * PX + j * Z + kzl];
+            for (int j = 0; j < 8; j++) v[j] = S[s2idx<Z>(xpos, j * Z + kzl)];
             if (SIGN < 0) {
 #pragma unroll
                 for (int j = 1; j < 8; j++) v[j] = v[j] * EXX_TW(R1, j * k1y);
@@ -324,7 +350,7 @@ EXX_HD void p2_y8(int tid, cplx* S, int k1y) {
                 for (int j = 1; j < 8; j++) v[j] = mul_conj_b(v[j], EXX_TW(R1, j * k1y));
             }
 #pragma unroll
-            for (int j = 0; j < 8; j++) S[xpos * PX + j * Z + kzl] = v[j];
+            for (int j = 0; j < 8; j++) S[s2idx<Z>(xpos, j * Z + kzl)] = v[j];
         }
     }
 }
@@ -333,7 +359,7 @@ template <int R1, int Z, int NT, int SIGN>
 EXX_HD void p2_xR(int tid, cplx* S) {
     // the R1-point x step on items (n2x, rem = k2y*Z + kzl).  Forward: DFT then twiddle W_N^(n2x k1x); inverse: DFT only
     // (the conjugate twiddle was applied at the end of p2_x8).
-    constexpr int NI = 8 * 8 * Z, IT = (NI + NT - 1) / NT, PX = P2Geo<Z>::PX;
+    constexpr int NI = 8 * 8 * Z, IT = (NI + NT - 1) / NT;
 #pragma unroll
     for (int i = 0; i < IT; i++) {
         int it = tid + i * NT;
@@ -341,14 +367,14 @@ EXX_HD void p2_xR(int tid, cplx* S) {
             int n2x = it / (8 * Z), rem = it - n2x * (8 * Z);
             cplx v[R1];
 #pragma unroll
-            for (int j = 0; j < R1; j++) v[j] = S[(j * 8 + n2x) * PX + rem];
+            for (int j = 0; j < R1; j++) v[j] = S[s2idx<Z>(j * 8 + n2x, rem)];
             dft<R1, SIGN>(v);
             if (SIGN < 0) {
 #pragma unroll
                 for (int j = 1; j < R1; j++) v[j] = v[j] * EXX_TW(R1, n2x * j);
             }
 #pragma unroll
-            for (int j = 0; j < R1; j++) S[(j * 8 + n2x) * PX + rem] = v[j];
+            for (int j = 0; j < R1; j++) S[s2idx<Z>(j * 8 + n2x, rem)] = v[j];
         }
     }
 }
@@ -364,7 +390,7 @@ template <int R1, int Z, int NT>
 EXX_HD void p2_x8(int tid, cplx* S, const real* __restrict__ Kt) {
     // items (k1x, rem): second forward x step, times K' (S4), first inverse x step, conjugate twiddle.
     // Kt: this tile's slice of the permuted kernel table (layout above).
-    constexpr int NI = R1 * 8 * Z, IT = (NI + NT - 1) / NT, PX = P2Geo<Z>::PX;
+    constexpr int NI = R1 * 8 * Z, IT = (NI + NT - 1) / NT;
     const kvec* __restrict__ Kv = reinterpret_cast<const kvec*>(Kt);
 #pragma unroll
     for (int i = 0; i < IT; i++) {
@@ -380,7 +406,7 @@ EXX_HD void p2_x8(int tid, cplx* S, const real* __restrict__ Kt) {
                 for (int e = 0; e < KVW; e++) kk[jv * KVW + e] = q.v[e];
             }
 #pragma unroll
-            for (int j = 0; j < 8; j++) v[j] = S[(k1x * 8 + j) * PX + rem];
+            for (int j = 0; j < 8; j++) v[j] = S[s2idx<Z>(k1x * 8 + j, rem)];
             dft<8, -1>(v);
 #pragma unroll
             for (int j = 0; j < 8; j++) v[j] = scale(kk[j], v[j]);
@@ -388,7 +414,7 @@ EXX_HD void p2_x8(int tid, cplx* S, const real* __restrict__ Kt) {
 #pragma unroll
             for (int j = 1; j < 8; j++) v[j] = mul_conj_b(v[j], EXX_TW(R1, j * k1x));
 #pragma unroll
-            for (int j = 0; j < 8; j++) S[(k1x * 8 + j) * PX + rem] = v[j];
+            for (int j = 0; j < 8; j++) S[s2idx<Z>(k1x * 8 + j, rem)] = v[j];
         }
     }
 }
@@ -414,8 +440,84 @@ EXX_HD void p3_y2inv(int tid, const cplx* __restrict__ W, int x, int yb, cplx* S
     }
 }
 
+// STAGE3: the same step with the work-box elements fetched ahead of time.  Element j of item tid + i NT lives in the slot
+// G[(i R1 + j) NT + tid], written and read by this thread only (no barrier needed): p3_stage copies them there (cp.async on the
+// device, one element each, so the thread does not wait for them; a plain copy on the host), p3_y2inv_staged consumes them.
+EXX_HD void stage_elem(cplx* dst, const cplx* src) {
+#if defined(__CUDA_ARCH__)
+    if (sizeof(cplx) == 16)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+    else
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+#else
+    *dst = *src;
+#endif
+}
+// copies are grouped (stage_commit closes a group, possibly an empty one); stage_wait<P> returns when at most the P most
+// recent groups of this thread are still in flight
+EXX_HD void stage_commit() {
+#if defined(__CUDA_ARCH__)
+    asm volatile("cp.async.commit_group;" ::: "memory");
+#endif
+}
+template <int P>
+EXX_HD void stage_wait() {
+#if defined(__CUDA_ARCH__)
+    asm volatile("cp.async.wait_group %0;" ::"n"(P) : "memory");
+#endif
+}
 template <int R1, int U, int NT>
-EXX_HD void p3_zinv2(int tid, const cplx* S, const cplx* __restrict__ um, double wf, int x, int yb, acc_c* A, bool first, bool cj = false) {
+EXX_HD void p3_stage(int tid, const cplx* __restrict__ W, int x, int yb, cplx* G) {
+    static_assert(sizeof(cplx) == 16 || sizeof(cplx) == 8, "cplx size");
+    constexpr int N = 8 * R1, NI = U * N, IT = (NI + NT - 1) / NT;
+#pragma unroll
+    for (int i = 0; i < IT; i++) {
+        int it = tid + i * NT;
+        if (it < NI) {
+            int kzl = it & 3, u = (it >> 2) % U, kzpos = (it / (4 * U)) * 4 + kzl;
+            size_t base = widx<R1>(0, kzpos, x, yb * U + u);
+#pragma unroll
+            for (int j = 0; j < R1; j++) stage_elem(G + (i * R1 + j) * NT + tid, W + base + (size_t)j * (N / 4) * N * 32);
+        }
+    }
+}
+// the u_m elements of the last step, same scheme: element j of item tid + i NT in slot G2[(i R1 + j) NT + tid]
+template <int R1, int U, int NT>
+EXX_HD void p3_stage_u(int tid, const cplx* __restrict__ um, int x, int yb, cplx* G2) {
+    constexpr int N = 8 * R1, NI = U * R1 * 8, IT = (NI + NT - 1) / NT;
+#pragma unroll
+    for (int i = 0; i < IT; i++) {
+        int it = tid + i * NT;
+        if (it < NI) {
+            int row = it >> 3, n2z = it & 7;
+            int u = row / R1, n1y = row - u * R1;
+            size_t base = ((size_t)x * N + (n1y * 8 + yb * U + u)) * N + n2z;
+#pragma unroll
+            for (int j = 0; j < R1; j++) stage_elem(G2 + (i * R1 + j) * NT + tid, um + base + j * 8);
+        }
+    }
+}
+template <int R1, int U, int NT>
+EXX_HD void p3_y2inv_staged(int tid, const cplx* G, cplx* S) {
+    constexpr int N = 8 * R1, NI = U * N, IT = (NI + NT - 1) / NT;
+#pragma unroll
+    for (int i = 0; i < IT; i++) {
+        int it = tid + i * NT;
+        if (it < NI) {
+            int kzl = it & 3, u = (it >> 2) % U, kzpos = (it / (4 * U)) * 4 + kzl;
+            cplx v[R1];
+#pragma unroll
+            for (int j = 0; j < R1; j++) v[j] = G[(i * R1 + j) * NT + tid];
+            dft<R1, +1>(v);
+#pragma unroll
+            for (int j = 0; j < R1; j++) S[sidx<R1>(u, j, kzpos >> 3, kzpos & 7)] = v[j];
+        }
+    }
+}
+
+template <int R1, int U, int NT, bool USTG = false>
+EXX_HD void p3_zinv2(int tid, const cplx* S, const cplx* __restrict__ um, double wf, int x, int yb, acc_c* A, bool first, bool cj = false,
+                     const cplx* G2 = nullptr) {
     // items (row, n2z): last inverse z step, then acc -= (w_q f_m) u_m v   (S6); A is this CTA's private accumulator tile
     constexpr int N = 8 * R1, NI = U * R1 * 8, IT = (NI + NT - 1) / NT;
 #pragma unroll
@@ -427,7 +529,7 @@ EXX_HD void p3_zinv2(int tid, const cplx* S, const cplx* __restrict__ um, double
             size_t base = ((size_t)x * N + (n1y * 8 + yb * U + u)) * N + n2z;
             cplx b[R1], v[R1];
 #pragma unroll
-            for (int j = 0; j < R1; j++) b[j] = um[base + j * 8];
+            for (int j = 0; j < R1; j++) b[j] = USTG ? G2[(i * R1 + j) * NT + tid] : um[base + j * 8];
 #pragma unroll
             for (int j = 0; j < R1; j++) v[j] = S[sidx<R1>(u, n1y, j, n2z)];
             dft<R1, +1>(v);
@@ -464,8 +566,9 @@ EXX_HD void p3_flush(int tid, const acc_c* A, acc_c* __restrict__ accg, int x, i
 }
 
 // register-accumulator variants (ACCREG): acc[i*R1 + j] belongs to item tid + i*NT, element n1z = j
-template <int R1, int U, int NT>
-EXX_HD void p3_zinv2_reg(int tid, const cplx* S, const cplx* __restrict__ um, double wf, int x, int yb, acc_c* acc, bool cj = false) {
+template <int R1, int U, int NT, bool USTG = false>
+EXX_HD void p3_zinv2_reg(int tid, const cplx* S, const cplx* __restrict__ um, double wf, int x, int yb, acc_c* acc, bool cj = false,
+                         const cplx* G2 = nullptr) {
     constexpr int N = 8 * R1, NI = U * R1 * 8, IT = (NI + NT - 1) / NT;
 #pragma unroll
     for (int i = 0; i < IT; i++) {
@@ -476,7 +579,7 @@ EXX_HD void p3_zinv2_reg(int tid, const cplx* S, const cplx* __restrict__ um, do
             size_t base = ((size_t)x * N + (n1y * 8 + yb * U + u)) * N + n2z;
             cplx b[R1], v[R1];
 #pragma unroll
-            for (int j = 0; j < R1; j++) b[j] = um[base + j * 8];
+            for (int j = 0; j < R1; j++) b[j] = USTG ? G2[(i * R1 + j) * NT + tid] : um[base + j * 8];
 #pragma unroll
             for (int j = 0; j < R1; j++) v[j] = S[sidx<R1>(u, n1y, j, n2z)];
             dft<R1, +1>(v);
@@ -540,7 +643,7 @@ EXX_HD void p1_z1_single(int tid, const cplx* __restrict__ un, int x, int yb, cp
 template <int R1, int Z, int NT, int SIGN>
 EXX_HD void p2_x8_half(int tid, cplx* S) {
     // items (k1x, rem).  SIGN < 0: second forward x step only;  SIGN > 0: first inverse x step + conjugate twiddle
-    constexpr int NI = R1 * 8 * Z, IT = (NI + NT - 1) / NT, PX = P2Geo<Z>::PX;
+    constexpr int NI = R1 * 8 * Z, IT = (NI + NT - 1) / NT;
 #pragma unroll
     for (int i = 0; i < IT; i++) {
         int it = tid + i * NT;
@@ -548,14 +651,14 @@ EXX_HD void p2_x8_half(int tid, cplx* S) {
             int k1x = it / (8 * Z), rem = it - k1x * (8 * Z);
             cplx v[8];
 #pragma unroll
-            for (int j = 0; j < 8; j++) v[j] = S[(k1x * 8 + j) * PX + rem];
+            for (int j = 0; j < 8; j++) v[j] = S[s2idx<Z>(k1x * 8 + j, rem)];
             dft<8, SIGN>(v);
             if (SIGN > 0) {
 #pragma unroll
                 for (int j = 1; j < 8; j++) v[j] = mul_conj_b(v[j], EXX_TW(R1, j * k1x));
             }
 #pragma unroll
-            for (int j = 0; j < 8; j++) S[(k1x * 8 + j) * PX + rem] = v[j];
+            for (int j = 0; j < 8; j++) S[s2idx<Z>(k1x * 8 + j, rem)] = v[j];
         }
     }
 }

@@ -26,7 +26,7 @@ template <int R1>
 static void emu_pair(const cplx* un, const cplx* um, const double* Knat, double wf, acc_c* acc, cplx* W) {
     typedef FusedCfg<R1> C;
     constexpr int N = 8 * R1, U = C::U1, NT13 = C::NT1, U3 = C::U3, NT3 = C::NT3, Z = C::Z, NT2 = C::NT2;
-    constexpr bool TWREG = C::TWREG, ACCREG = C::ACCREG;
+    constexpr bool TWREG = C::TWREG, ACCREG = C::ACCREG, STAGE3 = C::STAGE3 >= 1, STAGEU = C::STAGE3 >= 2;
     std::vector<double> Kp((size_t)N * N * N);
     permute_ktable(R1, Z, KVW, Knat, Kp.data());
     std::vector<acc_c> A((size_t)U3 * R1 * N);
@@ -63,7 +63,16 @@ static void emu_pair(const cplx* un, const cplx* um, const double* Knat, double 
     for (int x = 0; x < N; x++)
         for (int yb = 0; yb < 8 / U3; yb++) {
             for (auto& a : accr) a = mka(0.0, 0.0);
-            for (int t = 0; t < NT3; t++) p3_y2inv<R1, U3, NT3>(t, W, x, yb, S.data());
+            std::vector<cplx> G2((size_t)IT3 * R1 * NT3);
+            if (STAGE3) {  // per-thread staging slots, as pass_c_kernel uses them
+                std::vector<cplx> G((size_t)((U3 * N + NT3 - 1) / NT3) * R1 * NT3);
+                for (int t = 0; t < NT3; t++) p3_stage<R1, U3, NT3>(t, W, x, yb, G.data());
+                for (int t = 0; t < NT3; t++) p3_y2inv_staged<R1, U3, NT3>(t, G.data(), S.data());
+                if (STAGEU)
+                    for (int t = 0; t < NT3; t++) p3_stage_u<R1, U3, NT3>(t, um, x, yb, G2.data());
+            } else {
+                for (int t = 0; t < NT3; t++) p3_y2inv<R1, U3, NT3>(t, W, x, yb, S.data());
+            }
             for (int t = 0; t < NT3; t++) {
                 cplx twr[8];
                 load_twr<R1>(t, twr);
@@ -71,9 +80,9 @@ static void emu_pair(const cplx* un, const cplx* um, const double* Knat, double 
             }
             for (int t = 0; t < NT3; t++) {
                 if (ACCREG)
-                    p3_zinv2_reg<R1, U3, NT3>(t, S.data(), um, wf, x, yb, accr.data() + (size_t)t * IT3 * R1);
+                    p3_zinv2_reg<R1, U3, NT3, STAGEU>(t, S.data(), um, wf, x, yb, accr.data() + (size_t)t * IT3 * R1, false, G2.data());
                 else
-                    p3_zinv2<R1, U3, NT3>(t, S.data(), um, wf, x, yb, A.data(), true);
+                    p3_zinv2<R1, U3, NT3, STAGEU>(t, S.data(), um, wf, x, yb, A.data(), true, false, G2.data());
             }
             for (int t = 0; t < NT3; t++) {
                 if (ACCREG)

@@ -81,8 +81,10 @@ __device__ __forceinline__ void bulk_s2g(void* gdst, const void* smem_src, uint3
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(smem_u32(smem_src)), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void bulk_commit_wait_all() {
+    // .read: wait only until the shared-memory source has been read (the CTA may then retire and free its tile); the global
+    // writes are complete at the kernel boundary, which is where the next pass starts
     asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-    asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
 __device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 

@@ -564,6 +564,40 @@ def test_fused_128_full_grid_against_live_oracle(B):
     g.close()
 
 
+FUSED_EVERY = {
+    # N: (lattice, kfrac, kweight, ecut, occupations, kernel kind, mu) — one small cell per instantiation of the fused passes that
+    # no BASELINE configuration reaches on its own; run on the caller's grid (EXX_OPT_PRUNE = 0)
+    32: (("rh", 8.0, 70.0), [[0, 0, 0], [0.5, 0.25, 0]], [0.5, 0.5], 3.0, [1, 0.5, 0, 1], 0, 0.0),        # alias-free: pair symmetry on
+    "32a": (("sc", 10.0), [[0, 0, 0]], [1.0], 20.0, [1, 1, 0.5, 0, 1], 1, 0.106),                         # needs 41 > 32: aliased, symmetry off
+    40: (("sc", 11.0), [[0.25, 0.25, 0.25]], [1.0], 5.0, [1, 0, 0.5, 1, 1], 0, 0.0),
+    80: (("rh", 16.0, 62.0), [[0, 0, 0], [0.25, -0.25, 0.25]], [0.25, 0.75], 4.0, [1, 0.5, 0, 1], 1, 0.2),
+}
+
+
+@pytest.mark.parametrize("key", list(FUSED_EVERY))
+def test_fused_every_instantiation_against_live_oracle(B, key):
+    lat, kf, kw, ecut, occ, kind, mu = FUSED_EVERY[key]
+    n = int(str(key).rstrip("a"))
+    lattice = W.cubic(lat[1]) if lat[0] == "sc" else W.rhombohedral(lat[1], lat[2])
+    w = W.custom("fused%s" % key, 31 + n, (n, n, n), lattice, kf, kw, ecut, len(occ), occ, kind, mu)
+    o, g = _pair(B, w)
+    psi = w.coefficients(o.npw)
+    want = o.apply(psi, w.occ)
+    e_want, _ = o.energy(psi, w.occ, want)
+    pd = g.to_device(psi)
+    g.set_option(B.EXX_OPT_PRUNE, 0)
+    out = g.apply(pd, w.occ)
+    assert g.get_info(B.EXX_INFO_WORK_GRID) == n and g.get_info(B.EXX_INFO_PATH_USED) == 2
+    assert g.get_info(B.EXX_INFO_SYMMETRY) == (0 if str(key).endswith("a") else 1)
+    got = out.cpu().numpy()
+    for k in range(w.nk):
+        for b in range(w.nbands):
+            assert _rel(o.band(got, k, b), o.band(want, k, b)) < TOL_VX, (key, k, b)
+    e, _ = g.energy(pd, w.occ, out)
+    assert abs(e - e_want) <= TOL_EX * abs(e_want)
+    g.close()
+
+
 # ---------------------------------------------------------------------------------------------------------------
 # S8(f)-2: mixed precision (EXX_OPT_PRECISION = 1): fp32 pair transforms, fp64 S1 / S7 / accumulators.  The paper's own bar
 # for this mode is 1e-5 relative agreement with fp64; the fp64 bars above do not apply to it.

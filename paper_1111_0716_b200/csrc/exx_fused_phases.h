@@ -83,14 +83,14 @@ struct FusedCfgBase<4> {
     static constexpr int U1 = 4, NT1 = 128, U3 = 4, NT3 = 128, Z = 4, NT2 = 128;
     static constexpr bool TWREG = false, ACCREG = false;
     static constexpr int STAGE3 = s3(2);
-    static constexpr int MINB1 = 1, MINB2 = 1, MINB3 = 1;
+    static constexpr int MINB1 = 1, MINB2 = 6, MINB3 = 1;
 };
 template <>
 struct FusedCfgBase<5> {
-    static constexpr int U1 = 4, NT1 = 160, U3 = 4, NT3 = 160, Z = 4, NT2 = 128;
-    static constexpr bool TWREG = false, ACCREG = false;
+    static constexpr int U1 = 4, NT1 = 160, U3 = 4, NT3 = 160, Z = 4, NT2 = 160;
+    static constexpr bool TWREG = false, ACCREG = true;
     static constexpr int STAGE3 = s3(2);
-    static constexpr int MINB1 = 1, MINB2 = 1, MINB3 = 1;
+    static constexpr int MINB1 = 1, MINB2 = 6, MINB3 = 1;
 };
 template <>
 struct FusedCfgBase<10> {

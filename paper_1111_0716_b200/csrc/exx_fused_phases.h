@@ -108,10 +108,10 @@ struct FusedCfgBase<6> {
 };
 template <>
 struct FusedCfgBase<8> {
-    static constexpr int U1 = 2, NT1 = 128, U3 = 2, NT3 = 128, Z = 4, NT2 = 128;
-    static constexpr bool TWREG = false, ACCREG = false;
+    static constexpr int U1 = 2, NT1 = 128, U3 = 2, NT3 = 128, Z = 4, NT2 = 96;
+    static constexpr bool TWREG = false, ACCREG = true;
     static constexpr int STAGE3 = s3(2);
-    static constexpr int MINB1 = 1, MINB2 = 4, MINB3 = 1;
+    static constexpr int MINB1 = 1, MINB2 = 6, MINB3 = 1;
 };
 template <>
 struct FusedCfgBase<9> {

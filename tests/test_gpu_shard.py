@@ -124,3 +124,41 @@ def test_apply_sharded_through_nccl_world_of_one(B):
     finally:
         if created:
             dist.destroy_process_group()
+
+
+def test_shards_of_C4a_add_up_at_full_size(B):
+    """BASELINE configs[3] (C4a, 160 bands, compact 72^3 grid, pair symmetry) cut into 8 shards, run one after the other: every
+    shard executes the pairs the plan gives it, the shards' outputs add up to the one-GPU apply to 1e-13 per band, and the rows
+    the oracle stored (and their energies) are met at 1e-10 / 1e-11."""
+    import json
+    import torch
+    w = W.make("C4a")
+    g = B.Exx.from_workload(w)
+    pd = g.to_device(w.coefficients(g.npw))
+    full = g.apply(pd, w.occ).clone()
+    P = 8
+    plan, _ = B.shard_plan(w.nk, w.nbands, w.occ, True, 0, P)
+    acc = torch.zeros_like(full)
+    part = g.empty_like_psi()
+    for r in range(P):
+        g.set_option(B.EXX_OPT_SHARD_COUNT, P)
+        g.set_option(B.EXX_OPT_SHARD_RANK, r)
+        g.apply(pd, w.occ, part)
+        assert g.get_info(B.EXX_INFO_PAIRS_EXECUTED) == plan[r]
+        acc += part
+    g.set_option(B.EXX_OPT_SHARD_COUNT, 1)
+    g.set_option(B.EXX_OPT_SHARD_RANK, 0)
+    a, f = acc.cpu().numpy(), full.cpu().numpy()
+    for n in range(w.nbands):
+        assert np.linalg.norm(g.band(a, 0, n) - g.band(f, 0, n)) <= 1e-13 * np.linalg.norm(g.band(f, 0, n))
+    # against the stored oracle rows (tests/golden/make_golden.py calls only oracle/): the north_star bars
+    gdir = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    gold = json.load(open(os.path.join(gdir, "exx_C4a.json")))
+    rows = np.load(os.path.join(gdir, "exx_C4a_rows.npz"))
+    e, pb = g.energy(pd, w.occ, acc)
+    for i, (k, n) in enumerate(gold["rows"]):
+        want = rows["row%d" % i]
+        assert np.linalg.norm(g.band(a, k, n) - want) <= 1e-10 * np.linalg.norm(want)
+        assert abs(pb[k * w.nbands + n] - gold["row_energy"][i]) <= 1e-11 * abs(gold["row_energy"][i])
+    assert e < 0 and abs(pb.sum() - e) <= 1e-13 * abs(e)
+    g.close()

@@ -321,6 +321,23 @@ def test_compact_grid_not_used_when_caller_grid_aliases(B):
         g.close()
 
 
+@pytest.mark.parametrize("name,prune", [("C2", 1), ("C3", 1), ("C4a", 1), ("C4a", 0)])
+def test_apply_is_bitwise_reproducible_at_full_size(B, name, prune):
+    """No atomics, fixed summation order, per-thread staging slots: two applies of the same input give identical bits (a race in the
+    cp.async staging or in the accumulator updates would show up here) — on the instantiations the BASELINE configs run
+    (N = 40, 64, 72 and, with EXX_OPT_PRUNE = 0, 96)."""
+    import torch
+    w = W.make(name)
+    g = B.Exx.from_workload(w)
+    g.set_option(B.EXX_OPT_PRUNE, prune)
+    pd = g.to_device(w.coefficients(g.npw))
+    a = g.apply(pd, w.occ).clone()
+    b = g.apply(pd, w.occ)
+    assert torch.equal(torch.view_as_real(a), torch.view_as_real(b))
+    assert bool(torch.isfinite(torch.view_as_real(a)).all())
+    g.close()
+
+
 def test_apply_C4a_full_grid_parity(B):
     """C4a on the caller's full 96^3 grid (EXX_OPT_PRUNE = 0); test_apply_C4a_parity covers the default (compact 72^3)."""
     _check_golden(B, "C4a", prune=0)

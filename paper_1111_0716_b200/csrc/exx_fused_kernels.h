@@ -98,7 +98,11 @@ __global__ void __launch_bounds__(FusedCfg<R1>::NT2, FusedCfg<R1>::MINB2) pass_b
     constexpr uint32_t ROWB = 8 * Z * sizeof(cplx);
     extern __shared__ __align__(16) unsigned char smem_raw[];
     cplx* S = reinterpret_cast<cplx*>(smem_raw);
-    __shared__ __align__(8) uint64_t bar;
+    // the tile arrives in chunks of NT / Z rows, one mbarrier each: iteration i of the first step touches chunk i only, so it can
+    // start as soon as that chunk has landed
+    constexpr int CR = NT / Z, NCH = (N + CR - 1) / CR;
+    static_assert(NT % Z == 0, "chunks are whole rows");
+    __shared__ __align__(8) uint64_t bar[NCH];
     const int tid = threadIdx.x;
     const unsigned bid = blockIdx.x;
     const int p = bid % job.npairs;
@@ -106,12 +110,11 @@ __global__ void __launch_bounds__(FusedCfg<R1>::NT2, FusedCfg<R1>::MINB2) pass_b
     const int k1y = tile / (N / Z);
     cplx* Wt = work + (size_t)(job.pi[p] * job.tb + job.pj[p]) * Ng + (size_t)tile * ((size_t)N * 8 * Z);
     const real* Kt = kperm + (size_t)tile * ((size_t)N * 8 * Z);
-    if (tid == 0) mbar_init(&bar, 1);
+    if (tid < NCH) mbar_init(&bar[tid], 1);
     __syncthreads();
-    if (tid == 0) mbar_arrive_expect_tx(&bar, ROWB * N);
-    for (int x = tid; x < N; x += NT) bulk_g2s(S + x * PX, Wt + x * 8 * Z, ROWB, &bar);
-    mbar_wait(&bar, 0);
-    p2_y8<R1, Z, NT, -1>(tid, S, k1y);
+    if (tid < NCH) mbar_arrive_expect_tx(&bar[tid], ROWB * (uint32_t)((tid + 1) * CR <= N ? CR : N - tid * CR));
+    for (int x = tid; x < N; x += NT) bulk_g2s(S + x * PX, Wt + x * 8 * Z, ROWB, &bar[x / CR]);
+    p2_y8<R1, Z, NT, -1>(tid, S, k1y, [&](int i) { mbar_wait(&bar[i], 0); });
     __syncthreads();
     p2_xR<R1, Z, NT, -1>(tid, S);
     __syncthreads();

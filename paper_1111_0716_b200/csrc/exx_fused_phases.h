@@ -327,14 +327,20 @@ inline void p2_copy_rows(cplx* S, cplx* Wt, bool load) {
         }
 }
 
-template <int R1, int Z, int NT, int SIGN>
-EXX_HD void p2_y8(int tid, cplx* S, int k1y) {
+// called by p2_y8 before iteration i touches its rows (rows i NT/Z .. (i+1) NT/Z - 1): the kernel waits there for the bulk copy of
+// that chunk of rows; the host emulation and the later steps pass nothing
+struct NoWait {
+    EXX_HD void operator()(int) const {}
+};
+template <int R1, int Z, int NT, int SIGN, class WAIT = NoWait>
+EXX_HD void p2_y8(int tid, cplx* S, int k1y, WAIT wait = WAIT()) {
     // items (xpos, kzl), in place in shared memory.  SIGN < 0: y twiddle W_N^(n2y k1y) (uniform per CTA), forward 8-point
     // DFT over n2y;  SIGN > 0: inverse 8-point DFT over k2y, conjugate twiddle.
     constexpr int N = 8 * R1, NI = N * Z, IT = (NI + NT - 1) / NT;
 #pragma unroll
     for (int i = 0; i < IT; i++) {
         int it = tid + i * NT;
+        wait(i);
         if (it < NI) {
             int xpos = it / Z, kzl = it - xpos * Z;
             cplx v[8];

@@ -102,9 +102,10 @@ enum {
     EXX_INFO_SYMMETRY = 13,       /* 1 if the last apply used the pair symmetry (then PAIRS_EXECUTED < PAIRS_ORDERED) */
     EXX_INFO_PRECISION = 15,      /* 0 fp64, 1 mixed: what the last apply ran in */
     EXX_INFO_COMPACT_GRID = 12    /* (no apply needed) N of the compact work grid, 0 if none: the smallest supported cubic grid with
-                                     N >= 4 max|g_i| + 1, used when it is smaller than the caller's box and the caller's box is itself
-                                     alias-free (N_i >= 4 max|g_i| + 1).  Then no product the method forms wraps around on either grid and
-                                     V_x psi on the sphere is the same up to rounding */
+                                     N >= 4 max|g_i| + 1, used when the caller's box is itself alias-free (N_i >= 4 max|g_i| + 1) and the
+                                     cubic grid has fewer points — or, if the caller's grid has no fused kernels (non-cubic, or a cubic
+                                     size outside the fused list), at most 4x as many.  No product the method forms wraps around on
+                                     either grid, so V_x psi on the sphere is the same up to rounding */
 };
 
 /* Create a context.  grid: N1,N2,N3.  lattice: 9 doubles, row i = a_i in bohr.  kfrac: nk*3 fractional reciprocal

@@ -93,6 +93,7 @@ struct exx_ctx {
     // no inner context, else on the first apply with pruning switched off).
     bool fft_ready = false;           // twiddles/attributes of the fused kernels set up for exx_fft3d_fused
     exx_ctx* inner = nullptr;
+    bool inner_larger = false;        // the inner grid has MORE points than this one (taken for its fused kernels only)
     bool big_alloc = false;
     int last_pruned = 0;
 

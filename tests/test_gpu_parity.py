@@ -259,9 +259,10 @@ def _expected_compact(g, w):
     need = 4 * gmax + 1
     if any(n < need for n in w.grid):
         return 0
+    fused = len(set(w.grid)) == 1 and w.grid[0] in FUSED_SIZES
     for n in FUSED_SIZES:
         if n >= need:
-            return n if n ** 3 < w.ng else 0
+            return n if (n ** 3 < w.ng or (not fused and n ** 3 <= 4 * w.ng)) else 0
     return 0
 
 
@@ -303,6 +304,43 @@ def test_compact_grid_equals_full_grid_and_oracle(B, name):
 def test_pair_symmetry_off_matches_golden(B, name):
     """The default runs use the pair symmetry; this one evaluates every ordered pair (EXX_OPT_SYMMETRY = 0)."""
     _check_golden(B, name, symmetry=0)
+
+
+NOFUSED = {
+    # alias-free caller grids that have no fused kernels of their own: a cubic work grid with up to 4x the points is used instead
+    "rect_50_50_64": dict(grid=(50, 50, 64), lat=("sc", 12.0), kf=[[0, 0, 0], [0.25, 0.25, -0.25]], kw=[0.5, 0.5], ecut=20.0, nb=3,
+                          occ=[1, 0.5, 0], kind=0, mu=0.0),
+    "cubic_54": dict(grid=(54, 54, 54), lat=("sc", 12.0), kf=[[0, 0, 0]], kw=[1.0], ecut=24.5, nb=3, occ=[1, 0.5, 0.25], kind=1, mu=0.106),
+}
+
+
+@pytest.mark.parametrize("name", list(NOFUSED))
+def test_cubic_work_grid_for_grids_without_fused_kernels(B, name):
+    s = NOFUSED[name]
+    lat = W.cubic(s["lat"][1]) if s["lat"][0] == "sc" else W.rhombohedral(s["lat"][1], s["lat"][2])
+    w = W.custom(name, 808, s["grid"], lat, s["kf"], s["kw"], s["ecut"], s["nb"], s["occ"], s["kind"], s["mu"])
+    o, g = _pair(B, w)
+    compact = _expected_compact(g, w)
+    assert compact and compact ** 3 >= w.ng and g.get_info(B.EXX_INFO_COMPACT_GRID) == compact   # larger than the caller's box
+    psi = w.coefficients(o.npw)
+    want = o.apply(psi, w.occ)                 # the oracle works on the caller's grid
+    e_want, _ = o.energy(psi, w.occ, want)
+    pd = g.to_device(psi)
+    res = {}
+    for path in (0, 1):                        # auto: fused passes on the cubic grid; 1: generic kernels on the caller's grid
+        g.set_option(B.EXX_OPT_PATH, path)
+        out = g.apply(pd, w.occ)
+        assert g.get_info(B.EXX_INFO_PATH_USED) == (2 if path == 0 else 1)
+        assert g.get_info(B.EXX_INFO_PRUNED) == (1 if path == 0 else 0)
+        got = out.cpu().numpy()
+        for k in range(w.nk):
+            for n in range(w.nbands):
+                assert _rel(o.band(got, k, n), o.band(want, k, n)) < TOL_VX, (name, path, k, n)
+        e, _ = g.energy(pd, w.occ, out)
+        assert abs(e - e_want) <= TOL_EX * abs(e_want)
+        res[path] = got
+    assert _rel(res[0], res[1]) < 1e-13
+    g.close()
 
 
 def test_compact_grid_not_used_when_caller_grid_aliases(B):

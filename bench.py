@@ -305,16 +305,19 @@ def run_ours(args, rank, world, local):
     return 0
 
 
-def cpu_baseline(w, psi):
-    """The oracle as it stands on the host cores: one V_x row (all (q,m) pairs of band (0,0)) of the same workload."""
+def cpu_baseline(w, psi, nrows=3):
+    """The oracle as it stands on the host cores: `nrows` V_x rows (all (q,m) pairs of bands 0.. of k-point 0) of the same
+    workload, about 10-15 s of CPU work at C4a."""
     from oracle import exx_ref as R
     o = R.RefExx(w.grid, w.lattice, w.kfrac, w.kweight, w.ecut, w.kernel_kind, w.mu, w.scale, w.nbands)
-    pairs = w.nk * w.nocc
+    nrows = min(nrows, w.nbands)
+    pairs = nrows * w.nk * w.nocc
     t0 = time.perf_counter()
-    o.apply_rows(psi, w.occ, [(0, 0)])
+    o.apply_rows(psi, w.occ, [(0, n) for n in range(nrows)])
     dt = time.perf_counter() - t0
     return {"value": pairs / dt, "unit": UNIT, "cores": R.num_threads(), "kind": "oracle", "seconds": dt,
-            "sample": "one V_x row (k0, band 0): %d pair evaluations incl. the real-space transforms of the %d bands it needs" % (pairs, pairs + 1)}
+            "sample": "%d V_x rows (k0, bands 0..%d): %d pair evaluations incl. the real-space transforms of the bands they need "
+                      "(done once)" % (nrows, nrows - 1, pairs)}
 
 
 def main():

@@ -66,8 +66,8 @@ enum {
  * order (<= 1e-13 relative, tested).  EXX_OPT_PRECISION = 1 changes the arithmetic (see below). */
 enum {
     EXX_OPT_PATH = 1,       /* 0 auto (fused kernels when the grid is supported, else generic), 1 generic per-axis kernels, 2 fused */
-    EXX_OPT_TILE_N = 2,     /* bands per row tile of a pair batch (0 = auto = 16; at most 16 on the fused path) */
-    EXX_OPT_TILE_M = 3,     /* bands per column tile of a pair batch (0 = auto = 16) */
+    EXX_OPT_TILE_N = 2,     /* bands per row tile of a pair batch (0 = auto: 32, or 16 when sharded; at most 32; shrunk to fit the workspace) */
+    EXX_OPT_TILE_M = 3,     /* bands per column tile of a pair batch (0 = auto, as above; at most 32) */
     EXX_OPT_PRUNE = 4,      /* 1 (default): run the pair pipeline on the compact work grid when there is one (see EXX_INFO_COMPACT_GRID);
                                0: always transform the caller's full grid */
     EXX_OPT_PROFILE = 5,    /* 1: bracket every kernel launch with CUDA events so exx_get_kernel_time works (slower) */
@@ -133,7 +133,7 @@ const char* exx_kernel_class_name(int kclass);
 
 /* Host only, no context and no GPU needed: how the fused path's pair batches are shared out among `nshards` shards.  The
  * loop nest over (k, q, a-tile, b-tile) gives one batch per tile x tile block of band pairs
- * (tile = 0: the default 16); batches are handed out longest first to the least loaded shard — deterministic, so every rank
+ * (tile = 0: the default, 32 for one shard and 16 for several; at most 32); batches are handed out longest first to the least loaded shard — deterministic, so every rank
  * computes the same plan.  occ_host: nk*nbands.  symmetry: as EXX_OPT_SYMMETRY (the caller says whether it applies).
  * Outputs (each nshards entries, either may be NULL): pairs_out = pair densities the shard transforms (passes A, B);
  * passes_out = fused pass executions (2 per pair + 1 per accumulation sweep), the load that is balanced. */

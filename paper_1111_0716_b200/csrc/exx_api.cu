@@ -451,11 +451,11 @@ int exx_set_option(exx_ctx* c, int option, int64_t value) {
         c->opt_path = value;
         return EXX_OK;
     case EXX_OPT_TILE_N:
-        if (value < 0 || value > 64) return EXX_ERR_BAD_ARG;
+        if (value < 0 || value > TMAX) return EXX_ERR_BAD_ARG;
         c->opt_tile_n = value;
         return EXX_OK;
     case EXX_OPT_TILE_M:
-        if (value < 0 || value > 32) return EXX_ERR_BAD_ARG;
+        if (value < 0 || value > TMAX) return EXX_ERR_BAD_ARG;
         c->opt_tile_m = value;
         return EXX_OK;
     case EXX_OPT_PRUNE:
@@ -716,10 +716,10 @@ int exx_energy(exx_ctx* c, const double* psi_dev, const double* occ_host, const 
 
 int exx_shard_plan(int nk, int nbands, const double* occ_host, int symmetry, int tile, int nshards, int64_t* pairs_out, int64_t* passes_out) {
     if (!occ_host) return EXX_ERR_NULL;
-    if (nk < 1 || nbands < 1 || nshards < 1 || tile < 0 || tile > 16) return EXX_ERR_BAD_ARG;
+    if (nk < 1 || nbands < 1 || nshards < 1 || tile < 0 || tile > TMAX) return EXX_ERR_BAD_ARG;
     for (int i = 0; i < nk * nbands; i++)
         if (!(occ_host[i] >= 0.0) || !std::isfinite(occ_host[i])) return EXX_ERR_BAD_OCC;
-    const int t = std::min(tile ? tile : 16, nbands);
+    const int t = std::min(tile ? tile : (nshards > 1 ? std::min(EXX_DEFAULT_TILE, EXX_SHARD_TILE) : EXX_DEFAULT_TILE), nbands);
     std::vector<PairBlock> blocks;
     plan_blocks(nk, nbands, occ_host, symmetry != 0, t, t, nshards, blocks);
     for (int s = 0; s < nshards; s++) {

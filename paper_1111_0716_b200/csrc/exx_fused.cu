@@ -53,16 +53,17 @@ bool fused_supported(const exx_ctx* c) {
 }
 
 void fused_tiles(const exx_ctx* c, int* tn, int* tm) {
-    // defaults: 16 x 16 pairs per batch (fewer, longer launches: measured 5 % faster than 4 x 16), shrunk so that the pair
-    // workspace stays below ~4 GiB
+    // defaults: EXX_DEFAULT_TILE^2 pairs per batch (fewer, longer launches and fewer accumulator round trips: 16 x 16 measured
+    // 5 % faster than 4 x 16, 32 x 32 another 3 % at C4a), shrunk so that the pair workspace stays below EXX_WORK_CAP_GIB
 #ifdef EXX_TUNE_TN
     int n = EXX_TUNE_TN, m = EXX_TUNE_TM;
 #else
-    int n = 16, m = 16;
+    int n = EXX_DEFAULT_TILE, m = EXX_DEFAULT_TILE;
 #endif
     size_t box = sizeof(cplx) * (size_t)c->Ng;
-    while ((size_t)n * m * box > ((size_t)4 << 30) && m > 4) m /= 2;
-    while ((size_t)n * m * box > ((size_t)4 << 30) && n > 4) n /= 2;
+    const size_t cap = (size_t)EXX_WORK_CAP_GIB << 30;
+    while ((size_t)n * m * box > cap && m > 4) m /= 2;
+    while ((size_t)n * m * box > cap && n > 4) n /= 2;
     *tn = std::min(n, c->nb);
     *tm = std::min(m, c->nb);
 }
@@ -222,7 +223,7 @@ static int pair_loop(exx_ctx* c, FusedState* st, const double* occ, const typena
         AJob aj;
         aj.npairs = 0;
         aj.tb = tb;
-        bool ev[16][16];
+        bool ev[TMAX][TMAX];
         for (int i = 0; i < ta; i++) aj.a_idx[i] = a0 + i;
         for (int j = 0; j < tb; j++) aj.b_idx[j] = blist[b0 + j];
         for (int i = 0; i < ta; i++)
@@ -248,7 +249,7 @@ static int pair_loop(exx_ctx* c, FusedState* st, const double* occ, const typena
             cj.box_c = 1;
             cj.cj = 0;
             int64_t units = 0;
-            int rowbox[16];
+            int rowbox[TMAX];
             for (int j = 0; j < tb; j++) {
                 cj.src[j] = aj.b_idx[j];
                 cj.coef[j] = c->kw[q] * occ[q * nb + aj.b_idx[j]];
@@ -295,7 +296,7 @@ static int pair_loop(exx_ctx* c, FusedState* st, const double* occ, const typena
             cj.box_c = tb;
             cj.cj = 1;
             int64_t units = 0;
-            int rowbox[16];
+            int rowbox[TMAX];
             for (int i = 0; i < ta; i++) {
                 cj.src[i] = aj.a_idx[i];
                 cj.coef[i] = c->kw[k] * occ[k * nb + aj.a_idx[i]];
@@ -338,7 +339,7 @@ static int pair_loop(exx_ctx* c, FusedState* st, const double* occ, const typena
 }
 
 // The loop nest (k and q on the host, band loops on the device, innermost loop blocked).  Bands are cut into
-// a-tiles (k-point k) and b-tiles (k-point q) of at most 16; every batch evaluates v for the pairs of one (a-tile, b-tile)
+// a-tiles (k-point k) and b-tiles (k-point q) of at most TMAX; every batch evaluates v for the pairs of one (a-tile, b-tile)
 // block (passes A, B) and sweeps pass C once per side that receives a contribution.
 //   plain mode:    all ordered (k, q); pair (a, b) evaluated iff f_b != 0;   acc_a -= w_q f_b u_b v
 //   symmetry mode: k <= q, and a <= b when k == q; pair evaluated iff f_a != 0 or f_b != 0;
@@ -362,7 +363,9 @@ int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out)
             if (rc) return rc;
         }
     }
-    int ta_max = 16, tb_max = 16;
+    int ta_max = TMAX, tb_max = TMAX;
+    fused_tiles(c, &ta_max, &tb_max);
+    if (c->opt_shard_count > 1) ta_max = std::min(ta_max, EXX_SHARD_TILE), tb_max = std::min(tb_max, EXX_SHARD_TILE);
     while ((size_t)ta_max * tb_max > c->work_boxes && tb_max > 1) tb_max /= 2;
     while ((size_t)ta_max * tb_max > c->work_boxes && ta_max > 1) ta_max /= 2;
     if (c->opt_tile_n > 0) ta_max = (int)std::min<int64_t>(ta_max, c->opt_tile_n);

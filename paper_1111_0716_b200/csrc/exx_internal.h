@@ -139,20 +139,30 @@ struct MTile {
     int m_idx[32];     // band indices within k-point q
     double wf[32];     // w_q * f_mq
 };
-// one batch of band pairs for the fused passes: a-bands (k-point ka) x b-bands (k-point kb), at most 16 x 16.
+// one batch of band pairs for the fused passes: a-bands (k-point ka) x b-bands (k-point kb), at most TMAX x TMAX.
 // Pair p = (pi[p], pj[p]) evaluates v = IFFT K' FFT[conj(u_b) u_a]; its work box is pi*tb + pj.
+constexpr int TMAX = 32;  // most bands per side of a batch
+#ifndef EXX_DEFAULT_TILE
+#define EXX_DEFAULT_TILE 32  // bands per side of a batch unless EXX_OPT_TILE_N/M say otherwise (32 vs 16: C4a -3 %, C2 -11 %)
+#endif
+#ifndef EXX_SHARD_TILE
+#define EXX_SHARD_TILE 16    // ... when the batches are shared out over shards (more, smaller batches balance better)
+#endif
+#ifndef EXX_WORK_CAP_GIB
+#define EXX_WORK_CAP_GIB 16  // the pair workspace (tile_n x tile_m boxes) is kept below this
+#endif
 struct AJob {
     int npairs, tb;
-    int a_idx[16], b_idx[16];          // band indices within their k-points
-    unsigned char pi[256], pj[256];
+    int a_idx[TMAX], b_idx[TMAX];      // band indices within their k-points
+    unsigned char pi[TMAX * TMAX], pj[TMAX * TMAX];
 };
 // one accumulation sweep of pass C: CTA row r owns accumulator box tgt[r] and loops over its cnt[r] columns:
 //   acc[tgt[r]] -= coef[c] * u[src[c]] * (cj ? conj(v) : v),   v in work box r*box_r + c*box_c
 struct CJob {
     int nr, box_r, box_c, cj;
-    int tgt[16], cnt[16], src[16];
-    double coef[16];
-    unsigned char col[16][16];
+    int tgt[TMAX], cnt[TMAX], src[TMAX];
+    double coef[TMAX];
+    unsigned char col[TMAX][TMAX];
 };
 int fft_generic_init(exx_ctx* c);
 int launch_scatter(exx_ctx* c, int ik, const double2* coef, int nbatch, double2* box, const int32_t* map = nullptr);  // map: override (F layout)

@@ -64,7 +64,7 @@ def test_plan_is_deterministic_and_rejects_bad_arguments():
     a = B.shard_plan(2, 20, occ, True, 8, 3)
     b = B.shard_plan(2, 20, occ, True, 8, 3)
     assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
-    for bad in (dict(nshards=0), dict(tile=17), dict(tile=-1)):
+    for bad in (dict(nshards=0), dict(tile=33), dict(tile=-1)):
         kw = dict(symmetry=True, tile=0, nshards=2)
         kw.update(bad)
         with pytest.raises(B.ExxError):

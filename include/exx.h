@@ -83,7 +83,13 @@ enum {
                                the P shards is the full result (the caller adds them, e.g. one all-reduce; the binding's
                                apply_sharded does).  Fused path: the pair batches of exx_shard_plan; generic path: output rows
                                (k,n) with (k nbands + n) mod P = rank, the other rows of `out` zero */
-    EXX_OPT_SHARD_RANK = 10 /* 0 .. P-1 (default 0); exx_apply returns EXX_ERR_BAD_ARG while rank >= P */
+    EXX_OPT_SHARD_RANK = 10, /* 0 .. P-1 (default 0); exx_apply returns EXX_ERR_BAD_ARG while rank >= P */
+    EXX_OPT_ENERGY_ROUTE = 11 /* what exx_energy does when it is given no V_x psi.  0 (default): the pair-density route
+                               E_x = -1/2 sum w_k w_q f_nk f_mq sum_g K'_{k-q}(g) |rho^_{nk,mq}(g)|^2 (form (E2) of DESIGN.md section 2:
+                               Eq. 2 of PAPER.md, L127-130, written in reciprocal space) wherever the fused kernels run: the co-density
+                               and the forward transform only, pairs of two occupied bands only, no inverse transform and no
+                               accumulation (2.7x less work than V_x psi at C4a); otherwise, and with 1, V_x psi into an
+                               internal buffer and then (E1).  Both give the same number up to rounding (K' is real: Parseval) */
 };
 
 /* Counters (exx_get_info), all for the most recent exx_apply on this context unless stated. */
@@ -101,6 +107,7 @@ enum {
     EXX_INFO_WORK_GRID = 11,      /* N of the (cubic) grid the last apply transformed; first axis of the caller's grid if not compacted */
     EXX_INFO_SYMMETRY = 13,       /* 1 if the last apply used the pair symmetry (then PAIRS_EXECUTED < PAIRS_ORDERED) */
     EXX_INFO_PRECISION = 15,      /* 0 fp64, 1 mixed: what the last apply ran in */
+    EXX_INFO_ENERGY_ROUTE = 16,   /* most recent exx_energy: 1 = (E1) from V_x psi, 2 = pair-density route (E2); 0 before any */
     EXX_INFO_COMPACT_GRID = 12    /* (no apply needed) N of the compact work grid, 0 if none: the smallest supported cubic grid with
                                      N >= 4 max|g_i| + 1, used when the caller's box is itself alias-free (N_i >= 4 max|g_i| + 1) and the
                                      cubic grid has fewer points — or, if the caller's grid has no fused kernels (non-cubic, or a cubic
@@ -144,9 +151,11 @@ int exx_shard_plan(int nk, int nbands, const double* occ_host, int symmetry, int
  * call.  Bands with f = 0 are skipped as m (they contribute exactly 0) and kept as n.  Asynchronous on the stream. */
 int exx_apply(exx_ctx* ctx, const double* psi_dev, const double* occ_host, double* out_dev);
 
-/* E_x = 1/2 sum w_k f_nk Re<c_nk|(V_x c)_nk>.  If vxpsi_dev_or_null is NULL the library first applies V_x into an
- * internal buffer.  ex_host: 1 double.  per_band_host_or_null: nk*nbands terms 1/2 w_k f_nk Re<c|V_x c> (or NULL).
- * Synchronises the stream. */
+/* E_x = 1/2 sum w_k f_nk Re<c_nk|(V_x c)_nk> (Eq. 2).  If vxpsi_dev_or_null is NULL the library evaluates E_x
+ * from psi alone: by the pair-density route (EXX_OPT_ENERGY_ROUTE = 0, fused kernels; the counters of exx_get_info then describe
+ * this call) or by applying V_x into an internal buffer first.  ex_host: 1 double.  per_band_host_or_null: nk*nbands terms
+ * 1/2 w_k f_nk Re<c|V_x c> (or NULL); they add up to E_x.  With shards (EXX_OPT_SHARD_COUNT > 1) and no V_x psi given, the
+ * result is this shard's partial sum.  Synchronises the stream. */
 int exx_energy(exx_ctx* ctx, const double* psi_dev, const double* occ_host, const double* vxpsi_dev_or_null, double* ex_host,
                double* per_band_host_or_null);
 

@@ -14,10 +14,12 @@ LIB_PATH = os.environ.get("EXX_LIB") or os.path.join(_HERE, "libexx.so")  # EXX_
 EXX_OPT_PATH, EXX_OPT_TILE_N, EXX_OPT_TILE_M, EXX_OPT_PRUNE, EXX_OPT_PROFILE, EXX_OPT_SYMMETRY = 1, 2, 3, 4, 5, 6
 EXX_OPT_PRECISION = 8
 EXX_OPT_SHARD_COUNT, EXX_OPT_SHARD_RANK = 9, 10
+EXX_OPT_ENERGY_ROUTE = 11
 (EXX_INFO_LAUNCHES, EXX_INFO_PAIRS_ORDERED, EXX_INFO_PAIRS_EXECUTED, EXX_INFO_PATH_USED, EXX_INFO_WORKSPACE_BYTES,
  EXX_INFO_NCOEF, EXX_INFO_TILE_N, EXX_INFO_TILE_M, EXX_INFO_PRUNED, EXX_INFO_NUM_KERNEL_CLASSES, EXX_INFO_WORK_GRID,
  EXX_INFO_COMPACT_GRID, EXX_INFO_SYMMETRY) = range(1, 14)
 EXX_INFO_PRECISION = 15
+EXX_INFO_ENERGY_ROUTE = 16
 
 # every symbol include/exx.h declares (tests/test_abi.py checks the library exports them all)
 SYMBOLS = ("exx_create", "exx_destroy", "exx_npw", "exx_index_map", "exx_psi_offset", "exx_set_option", "exx_get_option",
@@ -251,6 +253,7 @@ class Exx:
         return out_dev
 
     def energy(self, psi_dev, occ, vxpsi_dev=None):
+        """(E_x, per-band terms).  Without vxpsi_dev the library works from psi alone (EXX_OPT_ENERGY_ROUTE)."""
         occ = self._occ(occ)
         ex = C.c_double()
         pb = np.empty(self.nk * self.nbands)

@@ -479,6 +479,10 @@ int exx_set_option(exx_ctx* c, int option, int64_t value) {
         if (value < 0 || value > 65535) return EXX_ERR_BAD_ARG;
         c->opt_shard_rank = value;
         return EXX_OK;
+    case EXX_OPT_ENERGY_ROUTE:
+        if (value != 0 && value != 1) return EXX_ERR_BAD_ARG;
+        c->opt_energy_route = value;
+        return EXX_OK;
     default: return EXX_ERR_BAD_ARG;
     }
 }
@@ -494,6 +498,7 @@ int exx_get_option(const exx_ctx* c, int option, int64_t* value) {
     case EXX_OPT_PRECISION: *value = c->opt_precision; return EXX_OK;
     case EXX_OPT_SHARD_COUNT: *value = c->opt_shard_count; return EXX_OK;
     case EXX_OPT_SHARD_RANK: *value = c->opt_shard_rank; return EXX_OK;
+    case EXX_OPT_ENERGY_ROUTE: *value = c->opt_energy_route; return EXX_OK;
     default: return EXX_ERR_BAD_ARG;
     }
 }
@@ -513,6 +518,7 @@ int exx_get_info(const exx_ctx* c, int what, int64_t* value) {
     case EXX_INFO_PRUNED: *value = c->pruned_used; return EXX_OK;
     case EXX_INFO_SYMMETRY: *value = c->symmetry_used; return EXX_OK;
     case EXX_INFO_PRECISION: *value = c->precision_used; return EXX_OK;
+    case EXX_INFO_ENERGY_ROUTE: *value = c->energy_route_used; return EXX_OK;
     case EXX_INFO_NUM_KERNEL_CLASSES: *value = KC_COUNT; return EXX_OK;
     default: return EXX_ERR_BAD_ARG;
     }
@@ -636,6 +642,30 @@ static int apply_generic(exx_ctx* c, const double2* psi, const double* occ, doub
     return EXX_OK;
 }
 
+static void options_to_inner(const exx_ctx* c, exx_ctx* in) {
+    in->opt_path = c->opt_path == 1 ? 1 : 0;
+    in->opt_tile_n = c->opt_tile_n;
+    in->opt_tile_m = c->opt_tile_m;
+    in->opt_profile = c->opt_profile;
+    in->opt_symmetry = c->opt_symmetry;
+    in->opt_precision = c->opt_precision;
+    in->opt_shard_count = c->opt_shard_count;
+    in->opt_shard_rank = c->opt_shard_rank;
+}
+static void counters_from_inner(exx_ctx* c, const exx_ctx* in, int rc) {
+    c->launches = in->launches;
+    c->pairs_ordered = in->pairs_ordered;
+    c->pairs_executed = in->pairs_executed;
+    c->path_used = in->path_used;
+    c->tile_n_used = in->tile_n_used;
+    c->tile_m_used = in->tile_m_used;
+    c->symmetry_used = in->symmetry_used;
+    c->precision_used = in->precision_used;
+    c->pruned_used = 1;
+    c->last_pruned = 1;
+    if (rc) c->last_error = in->last_error;
+}
+
 static int apply_impl(exx_ctx* c, const double2* psi, const double* occ, double2* out) {
     reset_counters(c);
     if (c->opt_shard_rank >= c->opt_shard_count) return EXX_ERR_BAD_ARG;
@@ -643,26 +673,9 @@ static int apply_impl(exx_ctx* c, const double2* psi, const double* occ, double2
     if (c->inner && c->opt_prune && !(c->inner_larger && c->opt_path == 1)) {
         // compact work grid: same spheres, same psi/out layout, every product alias-free on both grids
         exx_ctx* in = c->inner;
-        in->opt_path = c->opt_path == 1 ? 1 : 0;
-        in->opt_tile_n = c->opt_tile_n;
-        in->opt_tile_m = c->opt_tile_m;
-        in->opt_profile = c->opt_profile;
-        in->opt_symmetry = c->opt_symmetry;
-        in->opt_precision = c->opt_precision;
-        in->opt_shard_count = c->opt_shard_count;
-        in->opt_shard_rank = c->opt_shard_rank;
+        options_to_inner(c, in);
         int rc = apply_impl(in, psi, occ, out);
-        c->launches = in->launches;
-        c->pairs_ordered = in->pairs_ordered;
-        c->pairs_executed = in->pairs_executed;
-        c->path_used = in->path_used;
-        c->tile_n_used = in->tile_n_used;
-        c->tile_m_used = in->tile_m_used;
-        c->symmetry_used = in->symmetry_used;
-        c->precision_used = in->precision_used;
-        c->pruned_used = 1;
-        c->last_pruned = 1;
-        if (rc) c->last_error = in->last_error;
+        counters_from_inner(c, in, rc);
         return rc;
     }
     c->last_pruned = 0;
@@ -701,13 +714,56 @@ static int energy_impl(exx_ctx* c, const double2* psi, const double* occ, const 
     return EXX_OK;
 }
 
+// E_x without V_x psi: the pair-density route (E2), where the fused kernels run.  Same recursion onto the compact
+// work grid as apply_impl.  EXX_E2_UNAVAILABLE: this context would run the generic kernels; the caller falls back to (E1).
+static const int EXX_E2_UNAVAILABLE = 1;
+static int energy_pairs_run(exx_ctx* c, const double2* psi, const double* occ, double* band_e2_host) {
+    reset_counters(c);
+    if (c->opt_shard_rank >= c->opt_shard_count) return EXX_ERR_BAD_ARG;
+    if (c->inner && c->opt_prune && !(c->inner_larger && c->opt_path == 1)) {
+        exx_ctx* in = c->inner;
+        options_to_inner(c, in);
+        int rc = energy_pairs_run(in, psi, occ, band_e2_host);
+        if (rc != EXX_E2_UNAVAILABLE) counters_from_inner(c, in, rc);
+        return rc;
+    }
+    if (!(fused_supported(c) && c->opt_path != 1)) return EXX_E2_UNAVAILABLE;
+    c->last_pruned = 0;
+    int rc = ensure_big(c);
+    if (rc) return rc;
+    return fused_energy(c, occ, psi, band_e2_host);
+}
+static int energy_pairs_impl(exx_ctx* c, const double2* psi, const double* occ, double* ex, double* per_band) {
+    const int nbt = c->nk * c->nb;
+    double* h = c->host_pinned;
+    int rc = energy_pairs_run(c, psi, occ, h);
+    if (rc) return rc;
+    // fixed order: bands ascending within k-points ascending
+    double e = 0.0;
+    for (int i = 0; i < nbt; i++) {
+        h[i] *= -0.5;
+        e += h[i];
+    }
+    *ex = e;
+    if (per_band) memcpy(per_band, h, sizeof(double) * nbt);
+    return EXX_OK;
+}
+
 int exx_energy(exx_ctx* c, const double* psi_dev, const double* occ_host, const double* vxpsi_dev_or_null, double* ex_host,
                double* per_band_host_or_null) {
     if (!c || !psi_dev || !occ_host || !ex_host) return EXX_ERR_NULL;
     int rc = check_occ(c, occ_host);
     if (rc) return rc;
     const double2* vx = (const double2*)vxpsi_dev_or_null;
+    c->energy_route_used = 1;
     if (!vx) {
+        if (c->opt_energy_route == 0) {
+            rc = energy_pairs_impl(c, (const double2*)psi_dev, occ_host, ex_host, per_band_host_or_null);
+            if (rc != EXX_E2_UNAVAILABLE) {
+                if (rc == EXX_OK) c->energy_route_used = 2;
+                return rc;
+            }
+        }
         if ((rc = apply_impl(c, (const double2*)psi_dev, occ_host, c->vx_dev))) return rc;
         vx = c->vx_dev;
     }

@@ -30,6 +30,10 @@ struct FusedState {
     // mixed precision (allocated on first use): fp32 copies of the u cache and of the permuted kernel tables
     exx32::cplx* u32_dev = nullptr;
     float* kperm32_dev = nullptr;
+    // energy route (fused_energy): per-CTA partial sums of one batch, per-pair sums, per-band sums
+    double* epart_dev = nullptr;
+    double* pairsum_dev = nullptr;
+    double* band_e2_dev = nullptr;
 };
 
 #define EXX_DISPATCH_R1(R1v, EXPR)                  \
@@ -100,6 +104,16 @@ int fused_create(exx_ctx* c) {
         EXX_DISPATCH_R1(st->R1, L::fill_fmap(c->map_h[k].data(), c->npw[k], fm.data()));
         EXX_CUDA(c, cudaMemcpy(st->fmap_dev + c->map_off[k], fm.data(), sizeof(int32_t) * c->npw[k], cudaMemcpyHostToDevice));
     }
+    {
+        const size_t tiles2 = (size_t)st->R1 * (c->N[0] / Z);
+        if (cudaMalloc((void**)&st->epart_dev, sizeof(double) * TMAX * TMAX * tiles2) != cudaSuccess ||
+            cudaMalloc((void**)&st->pairsum_dev, sizeof(double) * TMAX * TMAX) != cudaSuccess ||
+            cudaMalloc((void**)&st->band_e2_dev, sizeof(double) * (size_t)c->nk * c->nb) != cudaSuccess) {
+            cudaGetLastError();
+            return EXX_ERR_ALLOC;
+        }
+        c->dev_bytes += sizeof(double) * (TMAX * TMAX * (tiles2 + 1) + (size_t)c->nk * c->nb);
+    }
     int rc = EXX_OK;
     EXX_DISPATCH_R1(st->R1, rc = L::init(c));
     return rc;
@@ -112,6 +126,9 @@ void fused_destroy(exx_ctx* c) {
     cudaFree(st->fmap_dev);
     cudaFree(st->u32_dev);
     cudaFree(st->kperm32_dev);
+    cudaFree(st->epart_dev);
+    cudaFree(st->pairsum_dev);
+    cudaFree(st->band_e2_dev);
     delete st;
     c->fused = nullptr;
 }
@@ -338,6 +355,73 @@ static int pair_loop(exx_ctx* c, FusedState* st, const double* occ, const typena
     return EXX_OK;
 }
 
+// S1: sphere coefficients -> F-layout work boxes (scatter) -> inverse transform through passes B/C -> u cache
+static int fused_u_cache(exx_ctx* c, FusedState* st, const double2* psi) {
+    int rc;
+    const int nb = c->nb, nk = c->nk;
+    const size_t Ng = (size_t)c->Ng;
+    for (int k = 0; k < nk; k++) {
+        const int bmax = (int)std::min<size_t>(c->work_boxes, (size_t)nb);
+        for (int n0 = 0; n0 < nb; n0 += bmax) {
+            const int bn = std::min(bmax, nb - n0);
+            if ((rc = launch_scatter(c, k, psi + c->off[k] + (int64_t)n0 * c->npw[k], bn, (double2*)c->work_dev, st->fmap_dev + c->map_off[k]))) return rc;
+            EXX_DISPATCH_R1(st->R1, rc = L::fft_inverse(c, (cplx*)c->work_dev, bn, (cplx*)c->u_dev + ((size_t)k * nb + n0) * Ng));
+            if (rc) return rc;
+        }
+    }
+    return EXX_OK;
+}
+
+// bands per side of a batch and whether the pair symmetry applies (options, workspace, shards); recorded in the counters
+static void fused_batch_shape(exx_ctx* c, int* ta, int* tb, bool* symmetry) {
+    int ta_max = TMAX, tb_max = TMAX;
+    fused_tiles(c, &ta_max, &tb_max);
+    if (c->opt_shard_count > 1) ta_max = std::min(ta_max, EXX_SHARD_TILE), tb_max = std::min(tb_max, EXX_SHARD_TILE);
+    while ((size_t)ta_max * tb_max > c->work_boxes && tb_max > 1) tb_max /= 2;
+    while ((size_t)ta_max * tb_max > c->work_boxes && ta_max > 1) ta_max /= 2;
+    if (c->opt_tile_n > 0) ta_max = (int)std::min<int64_t>(ta_max, c->opt_tile_n);
+    if (c->opt_tile_m > 0) tb_max = (int)std::min<int64_t>(tb_max, c->opt_tile_m);
+    const bool sym = c->opt_symmetry && c->alias_free;
+    if (sym) ta_max = tb_max = std::min(ta_max, tb_max);  // diagonal blocks need matching tiles
+    c->tile_n_used = ta_max;
+    c->tile_m_used = tb_max;
+    c->symmetry_used = sym ? 1 : 0;
+    *ta = ta_max, *tb = tb_max, *symmetry = sym;
+}
+
+// mixed precision: fp32 copies of the permuted kernel tables (built once) and of the u cache (refreshed for this psi)
+static int fused_mode32_ready(exx_ctx* c, FusedState* st) {
+    int rc;
+    const int nb = c->nb, nk = c->nk;
+    const size_t Ng = (size_t)c->Ng;
+    const size_t nbox = (size_t)nk * nb;
+    if (!st->u32_dev) {
+        if (cudaMalloc((void**)&st->u32_dev, sizeof(exx32::cplx) * Ng * nbox) != cudaSuccess ||
+            cudaMalloc((void**)&st->kperm32_dev, sizeof(float) * Ng * c->ntab) != cudaSuccess) {
+            cudaGetLastError();
+            return EXX_ERR_ALLOC;
+        }
+        c->dev_bytes += sizeof(exx32::cplx) * Ng * nbox + sizeof(float) * Ng * c->ntab;
+        if ((rc = exx32::upload_twiddles(c))) return rc;
+        if ((rc = init_mode32(c, st->R1))) return rc;
+        // the fp32 mode reads K' four values per load: its own permutation of the natural tables
+        std::vector<double> nat(Ng), perm(Ng);
+        std::vector<float> permf(Ng);
+        int Z = 4;
+        EXX_DISPATCH_R1(st->R1, Z = L::Z);
+        for (int t = 0; t < c->ntab; t++) {
+            EXX_CUDA(c, cudaMemcpy(nat.data(), c->ktab_dev + (size_t)t * Ng, sizeof(double) * Ng, cudaMemcpyDeviceToHost));
+            permute_ktable(st->R1, Z, exx32::KVW, nat.data(), perm.data());
+            for (size_t i = 0; i < Ng; i++) permf[i] = (float)perm[i];
+            EXX_CUDA(c, cudaMemcpy(st->kperm32_dev + (size_t)t * Ng, permf.data(), sizeof(float) * Ng, cudaMemcpyHostToDevice));
+        }
+        EXX_CUDA(c, cudaDeviceSynchronize());  // pageable copies may still be in flight; one-time set-up
+    }
+    to_float_kernel<<<2048, 256, 0, c->stream>>>((const double*)c->u_dev, (float*)st->u32_dev, 2 * Ng * nbox);
+    EXX_CUDA(c, cudaGetLastError());
+    return EXX_OK;
+}
+
 // The loop nest (k and q on the host, band loops on the device, innermost loop blocked).  Bands are cut into
 // a-tiles (k-point k) and b-tiles (k-point q) of at most TMAX; every batch evaluates v for the pairs of one (a-tile, b-tile)
 // block (passes A, B) and sweeps pass C once per side that receives a contribution.
@@ -353,28 +437,10 @@ int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out)
     const size_t Ng = (size_t)c->Ng;
     c->path_used = 2;
     c->pruned_used = 0;
-    // S1: sphere coefficients -> F-layout work boxes (scatter) -> inverse transform through passes B/C -> u cache
-    for (int k = 0; k < nk; k++) {
-        const int bmax = (int)std::min<size_t>(c->work_boxes, (size_t)nb);
-        for (int n0 = 0; n0 < nb; n0 += bmax) {
-            const int bn = std::min(bmax, nb - n0);
-            if ((rc = launch_scatter(c, k, psi + c->off[k] + (int64_t)n0 * c->npw[k], bn, (double2*)c->work_dev, st->fmap_dev + c->map_off[k]))) return rc;
-            EXX_DISPATCH_R1(st->R1, rc = L::fft_inverse(c, (cplx*)c->work_dev, bn, (cplx*)c->u_dev + ((size_t)k * nb + n0) * Ng));
-            if (rc) return rc;
-        }
-    }
-    int ta_max = TMAX, tb_max = TMAX;
-    fused_tiles(c, &ta_max, &tb_max);
-    if (c->opt_shard_count > 1) ta_max = std::min(ta_max, EXX_SHARD_TILE), tb_max = std::min(tb_max, EXX_SHARD_TILE);
-    while ((size_t)ta_max * tb_max > c->work_boxes && tb_max > 1) tb_max /= 2;
-    while ((size_t)ta_max * tb_max > c->work_boxes && ta_max > 1) ta_max /= 2;
-    if (c->opt_tile_n > 0) ta_max = (int)std::min<int64_t>(ta_max, c->opt_tile_n);
-    if (c->opt_tile_m > 0) tb_max = (int)std::min<int64_t>(tb_max, c->opt_tile_m);
-    const bool sym = c->opt_symmetry && c->alias_free;
-    if (sym) ta_max = tb_max = std::min(ta_max, tb_max);  // diagonal blocks need matching tiles
-    c->tile_n_used = ta_max;
-    c->tile_m_used = tb_max;
-    c->symmetry_used = sym ? 1 : 0;
+    if ((rc = fused_u_cache(c, st, psi))) return rc;
+    int ta_max, tb_max;
+    bool sym;
+    fused_batch_shape(c, &ta_max, &tb_max, &sym);
     cplx* work = (cplx*)c->work_dev;
     acc_c* acc = (acc_c*)c->acc_dev;  // one accumulator box per (k, band), always fp64
     EXX_CUDA(c, cudaMemsetAsync(acc, 0, sizeof(acc_c) * Ng * (size_t)nk * nb, c->stream));
@@ -382,31 +448,7 @@ int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out)
     if (c->opt_precision == 1) {
         // mixed precision (the paper's second mode): pair transforms, kernel multiply and the product with u in fp32;
         // S1, S7 and every accumulator stay fp64
-        const size_t nbox = (size_t)nk * nb;
-        if (!st->u32_dev) {
-            if (cudaMalloc((void**)&st->u32_dev, sizeof(exx32::cplx) * Ng * nbox) != cudaSuccess ||
-                cudaMalloc((void**)&st->kperm32_dev, sizeof(float) * Ng * c->ntab) != cudaSuccess) {
-                cudaGetLastError();
-                return EXX_ERR_ALLOC;
-            }
-            c->dev_bytes += sizeof(exx32::cplx) * Ng * nbox + sizeof(float) * Ng * c->ntab;
-            if ((rc = exx32::upload_twiddles(c))) return rc;
-            if ((rc = init_mode32(c, st->R1))) return rc;
-            // the fp32 mode reads K' four values per load: its own permutation of the natural tables
-            std::vector<double> nat(Ng), perm(Ng);
-            std::vector<float> permf(Ng);
-            int Z = 4;
-            EXX_DISPATCH_R1(st->R1, Z = L::Z);
-            for (int t = 0; t < c->ntab; t++) {
-                EXX_CUDA(c, cudaMemcpy(nat.data(), c->ktab_dev + (size_t)t * Ng, sizeof(double) * Ng, cudaMemcpyDeviceToHost));
-                permute_ktable(st->R1, Z, exx32::KVW, nat.data(), perm.data());
-                for (size_t i = 0; i < Ng; i++) permf[i] = (float)perm[i];
-                EXX_CUDA(c, cudaMemcpy(st->kperm32_dev + (size_t)t * Ng, permf.data(), sizeof(float) * Ng, cudaMemcpyHostToDevice));
-            }
-            EXX_CUDA(c, cudaDeviceSynchronize());  // pageable copies may still be in flight; one-time set-up
-        }
-        to_float_kernel<<<2048, 256, 0, c->stream>>>((const double*)c->u_dev, (float*)st->u32_dev, 2 * Ng * nbox);
-        EXX_CUDA(c, cudaGetLastError());
+        if ((rc = fused_mode32_ready(c, st))) return rc;
         if ((rc = pair_loop<ModeF>(c, st, occ, st->u32_dev, (exx32::cplx*)c->work_dev, st->kperm32_dev, acc, sym, ta_max, tb_max))) return rc;
         c->precision_used = 1;
     } else {
@@ -422,6 +464,84 @@ int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out)
             if ((rc = launch_gather(c, k, (const double2*)work, bn, out + c->off[k] + (int64_t)n0 * c->npw[k], st->fmap_dev + c->map_off[k]))) return rc;
         }
     }
+    return EXX_OK;
+}
+
+// ---- energy route (E2) ------------------------------------------------------------------------------------------------------
+// E_x = -1/2 sum_{k,q} w_k w_q sum_{a,b} f_a f_b sum_g K'_{k-q}(g) |rho^_{ak,bq}(g)|^2   ((E2); equal to (E1)
+// on any grid because K' is real: Parseval).  Only pairs with f_a != 0 and f_b != 0 count, no inverse transform and no pass C:
+// passes A and the forward half of B per pair, then fixed-order sums.  With the pair symmetry an unordered pair is transformed
+// once and credited to both bands (|rho^_{bq,ak}(g)|^2 K'_{q-k}(g) summed over g is the same number).
+template <class M>
+static int pair_energy_loop(exx_ctx* c, FusedState* st, const double* occ, const typename M::cplx* u_base, typename M::cplx* work,
+                            const typename M::real* kperm_base, bool sym, int ta_max, int tb_max) {
+    int rc;
+    const int nb = c->nb, nk = c->nk;
+    const size_t Ng = (size_t)c->Ng;
+    std::vector<PairBlock> blocks;
+    plan_blocks(nk, nb, occ, sym, ta_max, tb_max, (int)c->opt_shard_count, blocks);
+    std::vector<int> blist;
+    int bl_q = -1;
+    for (const PairBlock& blk : blocks) {
+        if (blk.shard != (int)c->opt_shard_rank) continue;
+        const int k = blk.k, q = blk.q;
+        const typename M::real* kperm = kperm_base + (size_t)c->ktab_of[(size_t)k * nk + q] * Ng;
+        const typename M::cplx* ua = u_base + (size_t)k * nb * Ng;
+        const typename M::cplx* ub = u_base + (size_t)q * nb * Ng;
+        if (bl_q != q) b_list(nb, occ, q, sym, blist), bl_q = q;
+        const int a0 = blk.a0, ta = blk.ta, tb = blk.tb;
+        const size_t b0 = (size_t)blk.b0;
+        AJob aj;
+        EJob ej;
+        aj.npairs = 0;
+        aj.tb = tb;
+        ej.tgt_a = k * nb, ej.tgt_b = q * nb, ej.sym = sym ? 1 : 0, ej.same_k = k == q ? 1 : 0;
+        for (int i = 0; i < TMAX; i++) ej.wa[i] = ej.wb[i] = 0.0;
+        for (int i = 0; i < ta; i++) aj.a_idx[i] = a0 + i, ej.wa[i] = c->kw[k] * occ[k * nb + a0 + i];
+        for (int j = 0; j < tb; j++) aj.b_idx[j] = blist[b0 + j], ej.wb[j] = c->kw[q] * occ[q * nb + blist[b0 + j]];
+        int64_t ordered = 0;
+        for (int i = 0; i < ta; i++)
+            for (int j = 0; j < tb; j++) {
+                const double fa = occ[k * nb + aj.a_idx[i]], fb = occ[q * nb + aj.b_idx[j]];
+                if (fa == 0.0 || fb == 0.0 || !pair_evaluated(sym, k, q, aj.a_idx[i], aj.b_idx[j], fa, fb)) continue;
+                aj.pi[aj.npairs] = (unsigned char)i;
+                aj.pj[aj.npairs] = (unsigned char)j;
+                aj.npairs++;
+                ordered += (sym && !(k == q && aj.a_idx[i] == aj.b_idx[j])) ? 2 : 1;
+            }
+        if (aj.npairs == 0) continue;
+        EXX_DISPATCH_M(st->R1, rc = L::pass_a_energy(c, ua, ub, aj, ej, kperm, work, st->epart_dev, st->pairsum_dev, st->band_e2_dev));
+        if (rc) return rc;
+        c->pairs_executed += aj.npairs;
+        c->pairs_ordered += ordered;
+    }
+    return EXX_OK;
+}
+
+// band_e2_host[k nb + n] = w_k f_nk sum_{q,m} w_q f_mq sum_g K' |rho^|^2  (this shard's batches); the caller applies the -1/2.
+// Synchronises the stream.
+int fused_energy(exx_ctx* c, const double* occ, const double2* psi, double* band_e2_host) {
+    FusedState* st = (FusedState*)c->fused;
+    if (!st) return EXX_ERR_BAD_ARG;
+    int rc;
+    const int nb = c->nb, nk = c->nk;
+    c->path_used = 2;
+    c->pruned_used = 0;
+    if ((rc = fused_u_cache(c, st, psi))) return rc;
+    int ta_max, tb_max;
+    bool sym;
+    fused_batch_shape(c, &ta_max, &tb_max, &sym);
+    EXX_CUDA(c, cudaMemsetAsync(st->band_e2_dev, 0, sizeof(double) * (size_t)nk * nb, c->stream));
+    c->precision_used = 0;
+    if (c->opt_precision == 1) {
+        if ((rc = fused_mode32_ready(c, st))) return rc;
+        if ((rc = pair_energy_loop<ModeF>(c, st, occ, st->u32_dev, (exx32::cplx*)c->work_dev, st->kperm32_dev, sym, ta_max, tb_max))) return rc;
+        c->precision_used = 1;
+    } else {
+        if ((rc = pair_energy_loop<ModeD>(c, st, occ, (const cplx*)c->u_dev, (cplx*)c->work_dev, st->kperm_dev, sym, ta_max, tb_max))) return rc;
+    }
+    EXX_CUDA(c, cudaMemcpyAsync(band_e2_host, st->band_e2_dev, sizeof(double) * (size_t)nk * nb, cudaMemcpyDeviceToHost, c->stream));
+    EXX_CUDA(c, cudaStreamSynchronize(c->stream));
     return EXX_OK;
 }
 

@@ -12,6 +12,11 @@ using ::exx::KC_PASS_A;
 using ::exx::KC_PASS_B;
 using ::exx::KC_PASS_C;
 using ::exx::KC_FFT_FUSED;
+using ::exx::KC_ENERGY;
+using ::exx::EJob;
+using ::exx::TMAX;
+using ::exx::pair_sum_kernel;
+using ::exx::band_energy_kernel;
 #endif
 
 cplx h_tw[TW_TOTAL];  // host copy of the twiddle tables (source of the constant-memory upload)
@@ -128,6 +133,81 @@ __global__ void __launch_bounds__(FusedCfg<R1>::NT2, FusedCfg<R1>::MINB2) pass_b
     for (int x = tid; x < N; x += NT) bulk_s2g(Wt + x * 8 * Z, S + x * PX, ROWB);
     bulk_commit_wait_all();
 }
+
+// Energy route (E2): pass B cut after the forward x transform.  Instead of multiplying by K' and
+// transforming back, the CTA sums K'(g) |rho^(g)|^2 over its tile in a fixed order (thread-serial, xor-shuffle tree, warps in
+// order) and writes ONE double: epart[pair * tiles + tile].  The work box is only read.
+template <int R1>
+__global__ void __launch_bounds__(FusedCfg<R1>::NT2, FusedCfg<R1>::MINB2) pass_b_energy_kernel(const cplx* __restrict__ work, const real* __restrict__ kperm, AJob job,
+                                                                                         double* __restrict__ epart) {
+    constexpr int N = 8 * R1, Z = FusedCfg<R1>::Z, NT = FusedCfg<R1>::NT2, PX = P2Geo<Z>::PX;
+    constexpr size_t Ng = (size_t)N * N * N;
+    constexpr uint32_t ROWB = 8 * Z * sizeof(cplx);
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* S = reinterpret_cast<cplx*>(smem_raw);
+    constexpr int CR = NT / Z, NCH = (N + CR - 1) / CR;
+    static_assert(NT % Z == 0, "chunks are whole rows");
+    __shared__ __align__(8) uint64_t bar[NCH];
+    __shared__ double wsum[(NT + 31) / 32];
+    const int tid = threadIdx.x;
+    const unsigned bid = blockIdx.x;
+    const int p = bid % job.npairs;
+    const int tile = bid / job.npairs;
+    const int k1y = tile / (N / Z);
+    const cplx* Wt = work + (size_t)(job.pi[p] * job.tb + job.pj[p]) * Ng + (size_t)tile * ((size_t)N * 8 * Z);
+    const real* Kt = kperm + (size_t)tile * ((size_t)N * 8 * Z);
+    if (tid < NCH) mbar_init(&bar[tid], 1);
+    __syncthreads();
+    if (tid < NCH) mbar_arrive_expect_tx(&bar[tid], ROWB * (uint32_t)((tid + 1) * CR <= N ? CR : N - tid * CR));
+    for (int x = tid; x < N; x += NT) bulk_g2s(S + x * PX, Wt + x * 8 * Z, ROWB, &bar[x / CR]);
+    p2_y8<R1, Z, NT, -1>(tid, S, k1y, [&](int i) { mbar_wait(&bar[i], 0); });
+    __syncthreads();
+    p2_xR<R1, Z, NT, -1>(tid, S);
+    __syncthreads();
+    double e = p2_x8_energy<R1, Z, NT>(tid, S, Kt);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) e += __shfl_xor_sync(0xffffffffu, e, o);
+    if ((tid & 31) == 0) wsum[tid >> 5] = e;
+    __syncthreads();
+    if (tid == 0) {
+        double t = 0.0;
+        for (int w = 0; w < (NT + 31) / 32; w++) t += wsum[w];
+        epart[(size_t)p * (R1 * (N / Z)) + tile] = t;
+    }
+}
+
+#ifndef EXX_SECOND_MODE
+// pairsum[p] = sum over the tiles of pair p, fixed order: lane-strided serial sums, then an xor-shuffle tree.  One warp per pair.
+__global__ void pair_sum_kernel(const double* __restrict__ epart, int ntiles, double* __restrict__ pairsum) {
+    const double* e = epart + (size_t)blockIdx.x * ntiles;
+    double s = 0.0;
+    for (int t = threadIdx.x; t < ntiles; t += 32) s += e[t];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if (threadIdx.x == 0) pairsum[blockIdx.x] = s;
+}
+// band_e2[band] += (w f)_band * sum over the band's pairs of (w f)_partner * pairsum: one thread per band and side, pairs in list
+// order, side a before side b (a diagonal block has the same bands on both sides), launches serial on the stream: deterministic.
+__global__ void band_energy_kernel(AJob job, EJob ej, const double* __restrict__ pairsum, double* __restrict__ band_e2) {
+    const int t = threadIdx.x;
+    if (t < TMAX) {
+        double s = 0.0;
+        bool any = false;
+        for (int p = 0; p < job.npairs; p++)
+            if (job.pi[p] == t) s += ej.wb[job.pj[p]] * pairsum[p], any = true;
+        if (any) band_e2[ej.tgt_a + job.a_idx[t]] += ej.wa[t] * s;
+    }
+    __syncthreads();
+    if (t >= TMAX && ej.sym) {
+        const int j = t - TMAX;
+        double s = 0.0;
+        bool any = false;
+        for (int p = 0; p < job.npairs; p++)
+            if (job.pj[p] == j && !(ej.same_k && job.a_idx[job.pi[p]] == job.b_idx[j])) s += ej.wa[job.pi[p]] * pairsum[p], any = true;
+        if (any) band_e2[ej.tgt_b + job.b_idx[j]] += ej.wb[j] * s;
+    }
+}
+#endif
 
 // pass C: second inverse y step, inverse z, acc -= coef u v.  One CTA per (tile, row) loops over the row's columns with
 // its accumulator tile on chip, then adds it to the row's accumulator box in global memory once (fixed summation order).
@@ -305,6 +385,7 @@ struct Launch {
         EXX_CUDA(c, cudaFuncSetAttribute(pass_a_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a));
         EXX_CUDA(c, cudaFuncSetAttribute(pass_b_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b));
         EXX_CUDA(c, cudaFuncSetAttribute(pass_c_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_c3));
+        EXX_CUDA(c, cudaFuncSetAttribute(pass_b_energy_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b));
         EXX_CUDA(c, cudaFuncSetAttribute(fft_a_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a));
         EXX_CUDA(c, cudaFuncSetAttribute((fft_b_kernel<R1, -1>), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b));
         EXX_CUDA(c, cudaFuncSetAttribute((fft_b_kernel<R1, +1>), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b));
@@ -321,6 +402,29 @@ struct Launch {
         {
             LaunchScope ls(c, KC_PASS_B, job.npairs);
             pass_b_kernel<R1><<<tiles2 * job.npairs, FusedCfg<R1>::NT2, smem_b, c->stream>>>(work, kperm, job);
+        }
+        EXX_CUDA(c, cudaGetLastError());
+        return EXX_OK;
+    }
+    // energy route: pass A, the forward half of pass B with the K' |rho^|^2 sum, and the two small fixed-order reductions
+    static int pass_a_energy(exx_ctx* c, const cplx* ua_base, const cplx* ub_base, const AJob& job, const EJob& ej, const real* kperm, cplx* work,
+                             double* epart, double* pairsum, double* band_e2) {
+        const unsigned tiles1 = N * (8 / U1), tiles2 = R1 * (N / Z);
+        {
+            LaunchScope ls(c, KC_PASS_A, job.npairs);
+            pass_a_kernel<R1><<<tiles1 * job.npairs, FusedCfg<R1>::NT1, smem_a, c->stream>>>(ua_base, ub_base, job, work);
+        }
+        {
+            LaunchScope ls(c, KC_PASS_B, job.npairs);
+            pass_b_energy_kernel<R1><<<tiles2 * job.npairs, FusedCfg<R1>::NT2, smem_b, c->stream>>>(work, kperm, job, epart);
+        }
+        {
+            LaunchScope ls(c, KC_ENERGY, job.npairs);
+            pair_sum_kernel<<<job.npairs, 32, 0, c->stream>>>(epart, (int)tiles2, pairsum);
+        }
+        {
+            LaunchScope ls(c, KC_ENERGY, job.npairs);
+            band_energy_kernel<<<1, 2 * TMAX, 0, c->stream>>>(job, ej, pairsum, band_e2);
         }
         EXX_CUDA(c, cudaGetLastError());
         return EXX_OK;

@@ -425,6 +425,36 @@ EXX_HD void p2_x8(int tid, cplx* S, const real* __restrict__ Kt) {
     }
 }
 
+// Energy route (E2 of DESIGN.md section 2): second forward x step only, then this thread's share of
+//   sum_g K'(g) |rho^(g)|^2   (fp64 whatever the mode of the transforms).  Nothing is written back to the tile.
+template <int R1, int Z, int NT>
+EXX_HD double p2_x8_energy(int tid, const cplx* S, const real* __restrict__ Kt) {
+    constexpr int NI = R1 * 8 * Z, IT = (NI + NT - 1) / NT;
+    const kvec* __restrict__ Kv = reinterpret_cast<const kvec*>(Kt);
+    double e = 0.0;
+#pragma unroll
+    for (int i = 0; i < IT; i++) {
+        int it = tid + i * NT;
+        if (it < NI) {
+            int k1x = it / (8 * Z), rem = it - k1x * (8 * Z);
+            cplx v[8];
+            real kk[8];
+#pragma unroll
+            for (int jv = 0; jv < 8 / KVW; jv++) {
+                kvec q = Kv[(size_t)jv * NI + it];
+#pragma unroll
+                for (int e2 = 0; e2 < KVW; e2++) kk[jv * KVW + e2] = q.v[e2];
+            }
+#pragma unroll
+            for (int j = 0; j < 8; j++) v[j] = S[s2idx<Z>(k1x * 8 + j, rem)];
+            dft<8, -1>(v);
+#pragma unroll
+            for (int j = 0; j < 8; j++) e += (double)kk[j] * ((double)v[j].x * (double)v[j].x + (double)v[j].y * (double)v[j].y);
+        }
+    }
+    return e;
+}
+
 // ================================================================================================================
 // pass C
 template <int R1, int U, int NT>

@@ -99,6 +99,8 @@ struct exx_ctx {
 
     // options
     int64_t opt_path = 0, opt_tile_n = 0, opt_tile_m = 0, opt_prune = 1, opt_profile = 0, opt_symmetry = 1, opt_precision = 0;
+    int64_t opt_energy_route = 0;  // 0 auto (pair-density route E2 where the fused path runs), 1 always E1 from V_x psi
+    int64_t energy_route_used = 0;
     int64_t opt_shard_count = 1, opt_shard_rank = 0;  // S8(f)-4: this context runs shard rank of count (exx_shard.h)
 
     // counters of the last apply
@@ -164,6 +166,12 @@ struct CJob {
     double coef[TMAX];
     unsigned char col[TMAX][TMAX];
 };
+// weights of one batch on the energy route: band (a,k) gets  wa[i] * sum_j wb[j] S_ij,  band (b,q) (pair symmetry) the mirror image
+struct EJob {
+    double wa[TMAX], wb[TMAX];   // w_k f_a, w_q f_b
+    int tgt_a, tgt_b;            // k*nb, q*nb: first entry of the k-point's bands in the per-band energy array
+    int sym, same_k;             // pair symmetry on; k == q (then the pair a == b is counted once)
+};
 int fft_generic_init(exx_ctx* c);
 int launch_scatter(exx_ctx* c, int ik, const double2* coef, int nbatch, double2* box, const int32_t* map = nullptr);  // map: override (F layout)
 int launch_gather(exx_ctx* c, int ik, const double2* box, int nbatch, double2* coef, const int32_t* map = nullptr);
@@ -181,6 +189,7 @@ void fused_tiles(const exx_ctx* c, int* tn, int* tm);
 int fused_create(exx_ctx* c);
 void fused_destroy(exx_ctx* c);
 int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out);
+int fused_energy(exx_ctx* c, const double* occ, const double2* psi, double* band_e2_host);  // E2 route: per-band sums w f w f K'|rho^|^2
 int fused_fft3d(exx_ctx* c, double2* in, int nbatch, int sign, double2* out);
 int fused_findex(const exx_ctx* c, int32_t* host_out);
 

@@ -149,10 +149,16 @@ def _check_full(B, w, paths=(0,), tile_m=(0,)):
             assert np.abs(pb - pb_want).max() <= TOL_EX * abs(e_want)
             assert abs(pb.sum() - e) <= 1e-14 * abs(e)
             assert e <= 0
-            e2, _ = g.energy(pd, w.occ, None)          # library applies V_x itself
-            assert abs(e2 - e) <= 1e-15 * abs(e)
+            g.set_option(B.EXX_OPT_ENERGY_ROUTE, 1)
+            e2, _ = g.energy(pd, w.occ, None)          # library applies V_x itself, then (E1)
+            assert abs(e2 - e) <= 1e-15 * abs(e) and g.get_info(B.EXX_INFO_ENERGY_ROUTE) == 1
             assert g.get_info(B.EXX_INFO_PAIRS_ORDERED) == w.pair_evals
             assert g.get_info(B.EXX_INFO_LAUNCHES) > 0
+            g.set_option(B.EXX_OPT_ENERGY_ROUTE, 0)
+            e3, pb3 = g.energy(pd, w.occ, None)        # pair-density route (E2) where the fused kernels run
+            assert g.get_info(B.EXX_INFO_ENERGY_ROUTE) == (2 if g.get_info(B.EXX_INFO_PATH_USED) == 2 else 1)
+            assert abs(e3 - e_want) <= TOL_EX * abs(e_want)
+            assert np.abs(pb3 - pb_want).max() <= TOL_EX * abs(e_want)
     g.close()
     return o, psi, want
 
@@ -424,6 +430,7 @@ def test_apply_host_matches_device_path(B):
     o, g = _pair(B, w)
     psi = w.coefficients(o.npw)
     out_d = g.apply(g.to_device(psi), w.occ).cpu().numpy()
+    g.set_option(B.EXX_OPT_ENERGY_ROUTE, 1)            # (E1) from V_x psi, as apply_host does
     e_d, _ = g.energy(g.to_device(psi), w.occ, None)
     out_h, e_h = g.apply_host(psi, w.occ)
     assert np.array_equal(out_h.view(np.float64), out_d.view(np.float64)) and e_h == e_d
@@ -505,10 +512,12 @@ def test_gpu_closed_form_single_plane_waves(B):
                 want -= 0.5 / a ** 3 * f[n] * f[k] * 4 * np.pi / ((2 * np.pi / a) ** 2 * float(d @ d))
     pd = g.to_device(psi.reshape(-1))
     for sym in (1, 0):
-        g.set_option(B.EXX_OPT_SYMMETRY, sym)
-        e, _ = g.energy(pd, f, None)
-        assert g.get_info(B.EXX_INFO_PATH_USED) == 2
-        assert abs(e - want) <= 1e-13 * abs(want)
+        for route in (0, 1):                           # pair-density route (E2) and V_x psi + (E1)
+            g.set_option(B.EXX_OPT_SYMMETRY, sym)
+            g.set_option(B.EXX_OPT_ENERGY_ROUTE, route)
+            e, _ = g.energy(pd, f, None)
+            assert g.get_info(B.EXX_INFO_PATH_USED) == 2 and g.get_info(B.EXX_INFO_ENERGY_ROUTE) == 2 - route
+            assert abs(e - want) <= 1e-13 * abs(want)
     g.close()
 
 
@@ -767,3 +776,93 @@ def test_fused_degenerate_cases(B):
                 e_want, _ = o.energy(psi, w.occ, want)
                 assert abs(e - e_want) <= TOL_EX * abs(e_want)
         g.close()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# E_x from psi alone: the pair-density route (E2), EXX_OPT_ENERGY_ROUTE = 0
+@pytest.mark.parametrize("tile", [0, 5])
+def test_energy_route_ragged_tiles_occupation_holes_kpoints(B, tile):
+    """Every combination the batch logic has: k-points with unequal weights, fractional and zero occupations, ragged tiles,
+    pair symmetry on and off, against the oracle's (E1) and its independent (E2); bitwise reproducible."""
+    nb = 19
+    occ = np.array([1, 0, 1, 0.5, 0, 0, 1, 1, 0.25, 0, 1, 0, 0, 0, 1, 0.75, 0, 0, 0], dtype=float)
+    w = W.custom("ragged48", 2024, (48, 48, 48), W.rhombohedral(7.5, 66.0), [[0.0, 0.0, 0.0], [0.25, -0.25, 0.5]], [0.4, 0.6], 5.0, nb, occ)
+    o, g = _pair(B, w)
+    psi = w.coefficients(o.npw)
+    e_want, pb_want = o.energy(psi, w.occ, o.apply(psi, w.occ))
+    e2_want = o.energy_e2(psi, w.occ)
+    assert abs(e2_want - e_want) <= 1e-12 * abs(e_want)
+    pd = g.to_device(psi)
+    nocc = int((np.asarray(w.occ) != 0).reshape(w.nk, nb).sum(axis=1)[0])
+    for sym in (1, 0):
+        g.set_option(B.EXX_OPT_SYMMETRY, sym)
+        g.set_option(B.EXX_OPT_TILE_N, tile)
+        g.set_option(B.EXX_OPT_TILE_M, tile)
+        e, pb = g.energy(pd, w.occ, None)
+        assert g.get_info(B.EXX_INFO_ENERGY_ROUTE) == 2 and g.get_info(B.EXX_INFO_SYMMETRY) == sym
+        # only pairs of two occupied bands are transformed
+        assert g.get_info(B.EXX_INFO_PAIRS_ORDERED) == (w.nk * nocc) ** 2
+        assert g.get_info(B.EXX_INFO_PAIRS_EXECUTED) == ((w.nk * nocc) * (w.nk * nocc + 1) // 2 if sym else (w.nk * nocc) ** 2)
+        assert abs(e - e_want) <= TOL_EX * abs(e_want) and abs(e - e2_want) <= TOL_EX * abs(e_want)
+        assert np.abs(pb - pb_want).max() <= TOL_EX * abs(e_want)
+        assert np.all(pb[np.asarray(w.occ) == 0] == 0.0) and abs(pb.sum() - e) <= 1e-14 * abs(e)
+        e_again, pb_again = g.energy(pd, w.occ, None)
+        assert e_again == e and np.array_equal(pb_again, pb)
+    assert g.energy(pd, np.zeros(w.nk * nb), None)[0] == 0.0
+    g.close()
+
+
+@pytest.mark.parametrize("name", ["C2", "C3", "C4a", "C5"])
+def test_energy_route_full_size_against_golden(B, name):
+    """At BASELINE's full sizes, in the default launch configuration: E_x and the per-band terms of the pair-density route
+    against the stored oracle values (E1 and E2 of tests/golden/make_golden.py)."""
+    w = W.make(name)
+    gold = json.load(open(os.path.join(GOLD, "exx_%s.json" % name)))
+    g = B.Exx.from_workload(w)
+    psi = w.coefficients(g.npw)
+    pd = g.to_device(psi)
+    e, pb = g.energy(pd, w.occ, None)
+    assert g.get_info(B.EXX_INFO_ENERGY_ROUTE) == 2 and g.get_info(B.EXX_INFO_PATH_USED) == 2
+    nocc = int((np.asarray(w.occ) != 0).sum())
+    assert g.get_info(B.EXX_INFO_PAIRS_ORDERED) == nocc * nocc
+    assert e < 0 and np.all(pb <= 0) and abs(pb.sum() - e) <= 1e-13 * abs(e)
+    for i, (k, n) in enumerate(gold["rows"]):
+        assert abs(pb[k * w.nbands + n] - gold["row_energy"][i]) <= TOL_EX * abs(gold["row_energy"][i]) + 1e-300
+    if "E_x_E1" in gold:
+        assert abs(e - gold["E_x_E1"]) <= TOL_EX * abs(gold["E_x_E1"])
+        assert abs(e - gold["E_x_E2"]) <= TOL_EX * abs(gold["E_x_E2"])
+        assert np.abs(pb - np.array(gold["per_band_energy"])).max() <= TOL_EX * abs(gold["E_x_E1"])
+    # and against this library's own V_x psi route
+    g.set_option(B.EXX_OPT_ENERGY_ROUTE, 1)
+    e1, pb1 = g.energy(pd, w.occ, None)
+    assert g.get_info(B.EXX_INFO_ENERGY_ROUTE) == 1
+    assert abs(e - e1) <= 1e-12 * abs(e1) and np.abs(pb - pb1).max() <= 1e-12 * abs(e1)
+    g.close()
+
+
+def test_energy_route_aliased_grid_generic_fallback_and_mixed_precision(B):
+    # C1: fused kernels on an aliased grid (no pair symmetry): (E1) = (E2) holds on any grid (K' real, Parseval)
+    w = W.make("C1")
+    o, g = _pair(B, w)
+    psi = w.coefficients(o.npw)
+    e_want, pb_want = o.energy(psi, w.occ, o.apply(psi, w.occ))
+    pd = g.to_device(psi)
+    e, pb = g.energy(pd, w.occ, None)
+    assert g.get_info(B.EXX_INFO_ENERGY_ROUTE) == 2 and g.get_info(B.EXX_INFO_SYMMETRY) == 0
+    assert abs(e - e_want) <= TOL_EX * abs(e_want) and np.abs(pb - pb_want).max() <= TOL_EX * abs(e_want)
+    # generic kernels asked for: no pair-density route there, the library falls back to V_x psi + (E1)
+    g.set_option(B.EXX_OPT_PATH, 1)
+    e, _ = g.energy(pd, w.occ, None)
+    assert g.get_info(B.EXX_INFO_ENERGY_ROUTE) == 1 and g.get_info(B.EXX_INFO_PATH_USED) == 1
+    assert abs(e - e_want) <= TOL_EX * abs(e_want)
+    g.close()
+    # mixed precision (not under the fp64 bars): fp32 transforms, fp64 sums
+    w = W.make("C3")
+    g = B.Exx.from_workload(w)
+    pd = g.to_device(w.coefficients(g.npw))
+    e64, _ = g.energy(pd, w.occ, None)
+    g.set_option(B.EXX_OPT_PRECISION, 1)
+    e32, _ = g.energy(pd, w.occ, None)
+    assert g.get_info(B.EXX_INFO_PRECISION) == 1 and g.get_info(B.EXX_INFO_ENERGY_ROUTE) == 2
+    assert 0 < abs(e32 - e64) <= 1e-5 * abs(e64)
+    g.close()

@@ -262,6 +262,24 @@ def run_ours(args, rank, world, local):
         assert abs(ex_f - ex) <= (1e-11 if args.precision == "fp64" else 1e-5) * abs(ex)
         g.set_option(B.EXX_OPT_PRUNE, 1)
 
+    # ---- E_x from psi alone by the pair-density route (EXX_OPT_ENERGY_ROUTE = 0): for information, not the headline
+    energy_only = None
+    if not shard:
+        g.energy(pd, occ, None)
+        sync_all()
+        q0, q1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        q0.record()
+        for _ in range(args.steps):
+            ex_q = g.energy(pd, occ, None)[0]
+        q1.record()
+        sync_all()
+        ms_q = max_over_ranks(q0.elapsed_time(q1), world, dev) / args.steps
+        pq = g.get_info(B.EXX_INFO_PAIRS_ORDERED)
+        energy_only = {"route": {1: "E1 from V_x psi", 2: "E2 pair densities"}.get(g.get_info(B.EXX_INFO_ENERGY_ROUTE)), "ms_per_step": ms_q,
+                       "pairs_ordered": pq, "pairs_executed": g.get_info(B.EXX_INFO_PAIRS_EXECUTED), "value": world * pq / (ms_q * 1e-3), "unit": UNIT,
+                       "gpu_launches": g.get_info(B.EXX_INFO_LAUNCHES), "E_x": ex_q}
+        assert abs(ex_q - ex) <= (1e-11 if args.precision == "fp64" else 1e-5) * abs(ex)
+
     # ---- timed region 3: end to end through exx_apply_host, pinned host buffers, copies inside the timed region
     for _ in range(min(2, args.warmup)):
         step_host()
@@ -295,6 +313,8 @@ def run_ours(args, rank, world, local):
             "gpu_launches": launches * args.steps}
     if full is not None:
         line["full_grid"] = full
+    if energy_only is not None:
+        line["energy_only"] = energy_only
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(w, psi)
     if rank == 0:

@@ -93,6 +93,43 @@ static void emu_pair(const cplx* un, const cplx* um, const double* Knat, double 
         }
 }
 
+// energy route of one pair (pass A, the forward half of pass B, the K' |rho^|^2 sum of p2_x8_energy), tile partials added up
+// in tile order as pair_sum_kernel would see them
+template <int R1>
+static double emu_pair_energy(const cplx* un, const cplx* um, const double* Knat, cplx* W) {
+    typedef FusedCfg<R1> C;
+    constexpr int N = 8 * R1, U = C::U1, NT13 = C::NT1, Z = C::Z, NT2 = C::NT2;
+    constexpr bool TWREG = C::TWREG;
+    std::vector<double> Kp((size_t)N * N * N);
+    permute_ktable(R1, Z, KVW, Knat, Kp.data());
+    std::vector<cplx> S((size_t)U * R1 * N), T(R1 * 8), S2((size_t)N * P2Geo<Z>::PX);
+    for (int k = 0; k < R1; k++)
+        for (int j = 0; j < 8; j++) T[tidx(k, j)] = EXX_TW(R1, j * k);
+    for (int x = 0; x < N; x++)
+        for (int yb = 0; yb < 8 / U; yb++) {
+            for (int t = 0; t < NT13; t++) p1_z1<R1, U, NT13>(t, un, um, x, yb, S.data());
+            for (int t = 0; t < NT13; t++) {
+                cplx twr[8];
+                load_twr<R1>(t, twr);
+                p13_z8<R1, U, NT13, -1, TWREG>(t, S.data(), T.data(), twr);
+            }
+            for (int t = 0; t < NT13; t++) p1_y1<R1, U, NT13>(t, S.data(), W, x, yb);
+        }
+    double e = 0.0;
+    for (int k1y = 0; k1y < R1; k1y++)
+        for (int zb = 0; zb < N / Z; zb++) {
+            const double* Kt = Kp.data() + ((size_t)k1y * (N / Z) + zb) * ((size_t)N * 8 * Z);
+            cplx* Wt = W + ((size_t)k1y * (N / Z) + zb) * ((size_t)N * 8 * Z);
+            p2_copy_rows<R1, Z>(S2.data(), Wt, true);
+            for (int t = 0; t < NT2; t++) p2_y8<R1, Z, NT2, -1>(t, S2.data(), k1y);
+            for (int t = 0; t < NT2; t++) p2_xR<R1, Z, NT2, -1>(t, S2.data());
+            double tile = 0.0;
+            for (int t = 0; t < NT2; t++) tile += p2_x8_energy<R1, Z, NT2>(t, S2.data(), Kt);
+            e += tile;
+        }
+    return e;
+}
+
 // plain 3-D transforms through the fused passes.  sign < 0: natural box `in` -> F-layout box `out`;
 // sign > 0: F-layout box `in` (modified in place by the pass-B half) -> natural box `out`
 template <int R1>
@@ -188,6 +225,18 @@ int exx_emu_pair(int R1, const double* un, const double* um, const double* Knat,
     case 9: emu_pair<9>((const cplx*)un, (const cplx*)um, Knat, wf, (acc_c*)acc, (cplx*)work); return 0;
     case 12: emu_pair<12>((const cplx*)un, (const cplx*)um, Knat, wf, (acc_c*)acc, (cplx*)work); return 0;
     case 16: emu_pair<16>((const cplx*)un, (const cplx*)um, Knat, wf, (acc_c*)acc, (cplx*)work); return 0;
+    default: return -1;
+    }
+}
+
+// sum_g K(g) |FFT[conj(u_m) u_n](g)|^2 through the energy route's phases
+int exx_emu_pair_energy(int R1, const double* un, const double* um, const double* Knat, double* work, double* e_out) {
+    fill_tw();
+    switch (R1) {
+#define EXX_EMU_E(r) \
+    case r: *e_out = emu_pair_energy<r>((const cplx*)un, (const cplx*)um, Knat, (cplx*)work); return 0;
+        EXX_EMU_E(2) EXX_EMU_E(4) EXX_EMU_E(5) EXX_EMU_E(10) EXX_EMU_E(6) EXX_EMU_E(8) EXX_EMU_E(9) EXX_EMU_E(12) EXX_EMU_E(16)
+#undef EXX_EMU_E
     default: return -1;
     }
 }

@@ -23,6 +23,7 @@ def emu(tmp_path_factory):
     L = C.CDLL(so)
     L.exx_emu_dft.argtypes = [C.c_int, C.c_int, dp]
     L.exx_emu_pair.argtypes = [C.c_int, dp, dp, dp, C.c_double, dp, dp]
+    L.exx_emu_pair_energy.argtypes = [C.c_int, dp, dp, dp, dp, dp]
     return L
 
 
@@ -61,6 +62,22 @@ def test_three_passes_equal_definition(emu, R1):
     assert emu.exx_emu_pair(R1, _p(un), _p(um), _p(K), wf, _p(acc), _p(work)) == 0
     want = -wf * um * np.fft.ifftn(K * np.fft.fftn(np.conj(um) * un)) * N ** 3
     assert np.linalg.norm(acc - acc0 - want) <= 1e-14 * np.linalg.norm(want)
+
+
+@pytest.mark.parametrize("R1", [2, 4, 5, 6, 8, 9, 10, 12, 16])
+def test_energy_route_equals_definition(emu, R1):
+    """sum_g K(g) |FFT[conj(u_m) u_n](g)|^2 for one pair (passes A, forward B, p2_x8_energy) against numpy.fft."""
+    N = 8 * R1
+    rng = np.random.default_rng(1000 + R1)
+    shp = (N, N, N)
+    un = rng.standard_normal(shp) + 1j * rng.standard_normal(shp)
+    um = rng.standard_normal(shp) + 1j * rng.standard_normal(shp)
+    K = rng.random(shp)  # asymmetric real table: a mirrored or transposed frequency index changes the sum
+    work = np.zeros(shp, dtype=np.complex128)
+    e = np.zeros(1)
+    assert emu.exx_emu_pair_energy(R1, _p(un), _p(um), _p(K), _p(work), _p(e)) == 0
+    want = float((K * np.abs(np.fft.fftn(np.conj(um) * un)) ** 2).sum())
+    assert abs(e[0] - want) <= 1e-13 * want
 
 
 def test_single_plane_wave_pair(emu):

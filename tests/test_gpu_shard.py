@@ -68,6 +68,16 @@ def test_shards_add_up_to_the_full_apply_and_the_oracle(B, name, P):
         executed.append(g.get_info(B.EXX_INFO_PAIRS_EXECUTED))
         acc = part.clone() if acc is None else acc + part
     assert sum(executed) == total_exec and all(e < total_exec for e in executed)
+    # E_x from psi alone (pair-density route on the fused path, V_x psi + (E1) on the generic one): the shards' partial sums add up
+    e_parts, pb_parts = [], []
+    for r in range(P):
+        g.set_option(B.EXX_OPT_SHARD_RANK, r)
+        e_r, pb_r = g.energy(pd, w.occ, None)
+        assert g.get_info(B.EXX_INFO_ENERGY_ROUTE) == (2 if fused else 1)
+        e_parts.append(e_r)
+        pb_parts.append(pb_r)
+    assert abs(sum(e_parts) - e_want) <= 1e-11 * abs(e_want)
+    assert np.abs(sum(pb_parts) - o.energy(psi, w.occ, want)[1]).max() <= 1e-11 * abs(e_want)
     if fused:
         assert executed == plan.tolist()
     g.set_option(B.EXX_OPT_SHARD_COUNT, 1)

@@ -812,7 +812,7 @@ def test_energy_route_ragged_tiles_occupation_holes_kpoints(B, tile):
     g.close()
 
 
-@pytest.mark.parametrize("name", ["C2", "C3", "C4a", "C5"])
+@pytest.mark.parametrize("name", ["C2", "C3", "C4a", "C4b", "C5"])
 def test_energy_route_full_size_against_golden(B, name):
     """At BASELINE's full sizes, in the default launch configuration: E_x and the per-band terms of the pair-density route
     against the stored oracle values (E1 and E2 of tests/golden/make_golden.py)."""
@@ -832,6 +832,8 @@ def test_energy_route_full_size_against_golden(B, name):
         assert abs(e - gold["E_x_E1"]) <= TOL_EX * abs(gold["E_x_E1"])
         assert abs(e - gold["E_x_E2"]) <= TOL_EX * abs(gold["E_x_E2"])
         assert np.abs(pb - np.array(gold["per_band_energy"])).max() <= TOL_EX * abs(gold["E_x_E1"])
+    e_again, pb_again = g.energy(pd, w.occ, None)       # fixed summation order, no atomics: bit-identical
+    assert e_again == e and np.array_equal(pb_again, pb)
     # and against this library's own V_x psi route
     g.set_option(B.EXX_OPT_ENERGY_ROUTE, 1)
     e1, pb1 = g.energy(pd, w.occ, None)

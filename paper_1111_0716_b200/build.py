@@ -4,6 +4,7 @@
 
 nvcc cross-compiles without a GPU.  The built library sits next to this file so that it travels with the repo.
 """
+import hashlib
 import os
 import subprocess
 import sys
@@ -11,9 +12,10 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libexx.so")
+STAMP = LIB + ".srchash"   # hash of what LIB was built from (git-ignored like the library, travels with it)
 SOURCES = ["exx_api.cu", "exx_kernels.cu", "exx_fused.cu", "exx_subspace.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--fmad=true",
-              "-Xcompiler", "-fPIC,-ffp-contract=off,-Wall,-Wno-unknown-pragmas", "-shared", "-cudart", "shared"]
+              "-Xcompiler", "-fPIC,-ffp-contract=off,-Wall,-Wno-unknown-pragmas", "-shared", "-cudart", "shared", "--threads", "4"]
 
 
 def _nvcc():
@@ -23,12 +25,24 @@ def _nvcc():
     return "nvcc"
 
 
+def _source_hash():
+    """sha256 over the sources, the public header and the compiler flags: what the library was built from."""
+    h = hashlib.sha256(" ".join(NVCC_FLAGS).encode())
+    deps = sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC)) + [os.path.join(os.path.dirname(HERE), "include", "exx.h")]
+    for d in deps:
+        h.update(os.path.basename(d).encode())
+        with open(d, "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()
+
+
 def needs_build():
-    if not os.path.exists(LIB):
+    """Stale iff the library is missing or was built from other sources.  Decided by content (a hash kept beside the library), not
+    by modification times: a copy of the tree (e.g. onto the GPU box) does not keep them, and a needless rebuild costs ~20 s."""
+    if not os.path.exists(LIB) or not os.path.exists(STAMP):
         return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(os.path.dirname(HERE), "include", "exx.h")]
-    return any(os.path.getmtime(d) > t for d in deps)
+    with open(STAMP) as f:
+        return f.read().strip() != _source_hash()
 
 
 def build(force=False, verbose=False, extra=(), out=None):
@@ -40,8 +54,13 @@ def build(force=False, verbose=False, extra=(), out=None):
     cmd = [_nvcc()] + NVCC_FLAGS + list(extra) + ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
     if verbose:
         print(" ".join(cmd))
+    digest = _source_hash()
     subprocess.check_call(cmd)
     os.replace(tmp, target)
+    if out is None and not extra:
+        with open(STAMP + ".tmp.%d" % os.getpid(), "w") as f:
+            f.write(digest + "\n")
+        os.replace(STAMP + ".tmp.%d" % os.getpid(), STAMP)
     return target
 
 

@@ -252,6 +252,27 @@ class Exx:
             all_reduce_sum(out_dev, group)
         return out_dev
 
+    def energy_sharded(self, psi_dev, occ, group=None, rank=None, world=None):
+        """E_x from psi alone with the pair work shared out like apply_sharded: this rank's partial sum through exx_energy
+        (EXX_OPT_SHARD_COUNT / _RANK; pair-density route on the fused path), then ONE all-reduce of nk*nbands + 1 doubles
+        ("E_x is one scalar all-reduce").  Every rank returns the full (E_x, per-band terms)."""
+        import torch.distributed as dist
+        world = dist.get_world_size(group) if world is None else world
+        rank = dist.get_rank(group) if rank is None else rank
+        self.set_option(EXX_OPT_SHARD_COUNT, world)
+        self.set_option(EXX_OPT_SHARD_RANK, rank)
+        try:
+            ex, pb = self.energy(psi_dev, occ, None)
+        finally:
+            self.set_option(EXX_OPT_SHARD_RANK, 0)
+            self.set_option(EXX_OPT_SHARD_COUNT, 1)
+        if world > 1:
+            t = self._torch.from_numpy(np.concatenate([pb, [ex]])).to(psi_dev.device)
+            all_reduce_sum(t, group)
+            r = t.cpu().numpy()
+            ex, pb = float(r[-1]), r[:-1].copy()
+        return ex, pb
+
     def energy(self, psi_dev, occ, vxpsi_dev=None):
         """(E_x, per-band terms).  Without vxpsi_dev the library works from psi alone (EXX_OPT_ENERGY_ROUTE)."""
         occ = self._occ(occ)

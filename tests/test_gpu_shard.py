@@ -130,6 +130,13 @@ def test_apply_sharded_through_nccl_world_of_one(B):
         c = g.apply_sharded(pd, w.occ, world=2, rank=0)
         d = g.apply_sharded(pd, w.occ, world=2, rank=1)
         assert (c + d - a).abs().max().item() <= 1e-13 * a.abs().max().item()
+        # the same for E_x from psi alone: partial sums through the collective
+        e, pb = g.energy(pd, w.occ, None)
+        e1, pb1 = g.energy_sharded(pd, w.occ)
+        assert e1 == e and np.array_equal(pb1, pb)
+        (e_a, pb_a), (e_b, pb_b) = g.energy_sharded(pd, w.occ, world=2, rank=0), g.energy_sharded(pd, w.occ, world=2, rank=1)
+        assert abs(e_a + e_b - e) <= 1e-13 * abs(e) and np.abs(pb_a + pb_b - pb).max() <= 1e-13 * abs(e)
+        assert g.get_option(B.EXX_OPT_SHARD_COUNT) == 1 and g.get_option(B.EXX_OPT_SHARD_RANK) == 0
         g.close()
     finally:
         if created:

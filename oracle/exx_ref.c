@@ -455,6 +455,62 @@ int exx_ref_apply(const exx_ref_ctx *c, const double *psi, const double *occ, do
     return rc;
 }
 
+/* The operator of (D), built from the orbitals psi and their occupations, applied to OTHER vectors phi (same layout as psi:
+ * nb vectors per k-point on sphere(k)) -- what FOCK_ACC does inside an iterative eigensolver, where it acts on the trial
+ * wavefunctions while the occupied orbitals define the operator (blocks of NSIM bands):
+ *   t_ik(r_j)         = sum_{g in sphere(k)} phi_ik(g) exp(+2 pi i sum g_i j_i / N_i)
+ *   rho~(g)           = (1/Ng) sum_j conj(u_mq(r_j)) t_ik(r_j) exp(-...)
+ *   v(r_j)            = (1/Omega) sum_g K(|k-q+G|) rho~(g) exp(+...)
+ *   (V_x t)_ik(r_j)   = - sum_q w_q sum_m f_mq u_mq(r_j) v(r_j),      out_ik(g) = (1/Ng) sum_j (V_x t)_ik(r_j) exp(-...), g in sphere(k)
+ * i.e. (D) with u_nk replaced by t_ik in the co-density only.  Plain loops: rows in parallel, the (q,m) sum of a row serial in
+ * loop order.  Pins (tests/test_oracle_exchange.py): closed-form eigenvalue for plane waves, phi = psi gives exx_ref_apply,
+ * Hermiticity and negativity of <phi_i|V_x phi_j>, linearity in phi. */
+int exx_ref_apply_to(const exx_ref_ctx *c, const double *psi_, const double *occ, const double *phi_, double *out_) {
+    if (!c || !psi_ || !occ || !phi_ || !out_) return EXX_REF_ERR_NULL;
+    int rc = check_occ(c, occ);
+    if (rc) return rc;
+    const cplx *psi = (const cplx *)psi_, *phi = (const cplx *)phi_;
+    cplx *out = (cplx *)out_;
+    const int64_t Ng = c->Ng;
+    cplx **u = all_real(c, psi, occ, NULL); /* the occupied orbitals in real space */
+    if (!u) return EXX_REF_ERR_ALLOC;
+    int fail = 0;
+#pragma omp parallel for schedule(dynamic)
+    for (int i = 0; i < c->nk * c->nb; i++) {
+        int k = i / c->nb, n = i % c->nb;
+        cplx *t = malloc(sizeof(cplx) * (size_t)Ng), *w = malloc(sizeof(cplx) * (size_t)Ng), *acc = calloc((size_t)Ng, sizeof(cplx));
+        double *K = malloc(sizeof(double) * (size_t)Ng);
+        if (!t || !w || !acc || !K) {
+            fail = 1;
+        } else {
+            to_real(c, k, phi + c->off[k] + (int64_t)n * c->npw[k], t);
+            for (int q = 0; q < c->nk; q++) {
+                exx_ref_kernel_table(c, k, q, K);
+                for (int m = 0; m < c->nb; m++) {
+                    double f = occ[q * c->nb + m];
+                    if (f == 0.0) continue;
+                    const cplx *um = u[q * c->nb + m];
+                    for (int64_t j = 0; j < Ng; j++) w[j] = conj(um[j]) * t[j];
+                    fft3d(c->N, -1, w);
+                    for (int64_t g = 0; g < Ng; g++) w[g] = (K[g] * (w[g] / (double)Ng)) / c->omega;
+                    fft3d(c->N, +1, w);
+                    double wf = c->kw[q] * f;
+                    for (int64_t j = 0; j < Ng; j++) acc[j] -= wf * (um[j] * w[j]);
+                }
+            }
+            fft3d(c->N, -1, acc);
+            cplx *o = out + c->off[k] + (int64_t)n * c->npw[k];
+            for (int ig = 0; ig < c->npw[k]; ig++) o[ig] = acc[c->map[k][ig]] / (double)Ng;
+        }
+        free(t);
+        free(w);
+        free(acc);
+        free(K);
+    }
+    free_real(c, u);
+    return fail ? EXX_REF_ERR_ALLOC : EXX_REF_OK;
+}
+
 /* (E1): E_x = 1/2 sum_k w_k sum_n f_nk Re <c_nk | (V_x c)_nk>; per_band (optional) gets the nk*nb terms. */
 int exx_ref_energy(const exx_ref_ctx *c, const double *psi_, const double *occ, const double *vxpsi_, double *ex, double *per_band) {
     if (!c || !psi_ || !occ || !vxpsi_ || !ex) return EXX_REF_ERR_NULL;

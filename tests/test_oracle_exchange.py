@@ -278,3 +278,57 @@ def test_subspace_matrix_pins():
     # a transposed operand or a missing conjugate would fail this: M computed from (psi, out) is not M from (out, psi)^T
     M01 = o.subspace(0, psi, out)
     assert np.abs(o.subspace(0, out, psi) - M01.conj().T).max() < 1e-16
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# exx_ref_apply_to: the operator of (psi, occ) applied to other vectors phi
+def test_apply_to_closed_form_plane_wave_eigenvalues():
+    """Occupied orbitals = plane waves g_m (weights f_m), trial vectors = plane waves g_i (some among the occupied, some not):
+    conj(u_m) t_i is one plane wave, so V_x t_i = lambda_i t_i with lambda_i = -(1/Omega) sum_m f_m K(|G_i - G_m|) (bare kernel, the
+    Q = 0 term dropped; HSE keeps pi/mu^2) -- evaluated here from the lattice, no oracle code."""
+    gm = [(0, 0, 0), (1, 0, 0), (0, 2, 0), (-1, 1, 3), (2, -2, 1)]
+    gi = [(1, 0, 0), (0, 0, 1), (-2, 1, 0), (2, -2, 1), (1, 1, 1)]
+    f = np.array([1.0, 1.0, 0.5, 0.0, 0.25])
+    lat = W.rhombohedral(9.0, 70.0)
+    Bm = 2 * np.pi * np.linalg.inv(lat).T
+    for kind, mu in ((0, 0.0), (1, 0.3)):
+        o = R.RefExx((16,) * 3, lat, np.zeros((1, 3)), [1.0], 6.0, kind, mu, 1.0, nbands=5)
+        psi = _plane_wave_bands(o, [(0, n) for n in range(5)], gm)
+        phi = _plane_wave_bands(o, [(0, n) for n in range(5)], gi)
+        phi *= np.exp(0.3j) * 1.7            # any amplitude
+        out = o.apply_to(psi, f, phi)
+        for i, a in enumerate(gi):
+            lam = 0.0
+            for j, b in enumerate(gm):
+                d = (np.array(a) - np.array(b)) @ Bm
+                q2 = float(d @ d)
+                if q2 > 0:
+                    kq = 4 * np.pi / q2 * (1.0 if kind == 0 else -np.expm1(-q2 / (4 * mu * mu)))
+                else:
+                    kq = 0.0 if kind == 0 else np.pi / mu ** 2
+                lam -= f[j] * kq / o.omega
+            assert np.linalg.norm(o.band(out, 0, i) - lam * o.band(phi, 0, i)) <= 1e-13 * abs(lam) * np.linalg.norm(o.band(phi, 0, i))
+
+
+@pytest.mark.parametrize("kpts", [False, True])
+def test_apply_to_reduces_to_apply_and_operator_identities(kpts):
+    w, o, psi = _small(kpts=kpts, kind=1 if kpts else 0, mu=0.25)
+    occ = w.occ
+    # phi = psi: the pinned function
+    assert np.linalg.norm(o.apply_to(psi, occ, psi) - o.apply(psi, occ)) <= 1e-14 * np.linalg.norm(o.apply(psi, occ))
+    rng = np.random.default_rng(77)
+    phi = rng.standard_normal(o.ncoef) + 1j * rng.standard_normal(o.ncoef)
+    chi = rng.standard_normal(o.ncoef) + 1j * rng.standard_normal(o.ncoef)
+    vphi, vchi = o.apply_to(psi, occ, phi), o.apply_to(psi, occ, chi)
+    # linear in phi (complex coefficients)
+    a, b = 0.7 - 0.2j, -1.3 + 0.5j
+    assert np.linalg.norm(o.apply_to(psi, occ, a * phi + b * chi) - (a * vphi + b * vchi)) <= 1e-13 * np.linalg.norm(vphi)
+    # Hermitian and negative semi-definite within every k-point, for arbitrary vectors
+    for k in range(o.nk):
+        P = np.array([o.band(phi, k, i) for i in range(o.nbands)] + [o.band(chi, k, i) for i in range(o.nbands)])
+        V = np.array([o.band(vphi, k, i) for i in range(o.nbands)] + [o.band(vchi, k, i) for i in range(o.nbands)])
+        M = P.conj() @ V.T
+        assert np.abs(M - M.conj().T).max() <= 1e-13 * np.abs(M).max()
+        assert np.linalg.eigvalsh(0.5 * (M + M.conj().T)).max() <= 1e-13 * np.abs(M).max()
+    # the operator does not depend on the phase of the orbitals that define it
+    assert np.linalg.norm(o.apply_to(psi * np.exp(1.1j), occ, phi) - vphi) <= 1e-13 * np.linalg.norm(vphi)

@@ -25,7 +25,7 @@ EXX_INFO_ENERGY_ROUTE = 16
 SYMBOLS = ("exx_create", "exx_destroy", "exx_npw", "exx_index_map", "exx_psi_offset", "exx_set_option", "exx_get_option",
            "exx_get_info", "exx_get_kernel_time", "exx_kernel_class_name", "exx_apply", "exx_energy", "exx_apply_host",
            "exx_scatter", "exx_gather", "exx_fft3d", "exx_to_real", "exx_kernel_table", "exx_strerror", "exx_last_error",
-           "exx_version", "exx_subspace", "exx_fft3d_fused", "exx_findex", "exx_shard_plan")
+           "exx_version", "exx_subspace", "exx_fft3d_fused", "exx_findex", "exx_shard_plan", "exx_apply_to")
 
 
 class KernelParams(C.Structure):
@@ -75,6 +75,7 @@ def lib():
         L.exx_kernel_class_name.argtypes = [C.c_int]
         L.exx_kernel_class_name.restype = C.c_char_p
         L.exx_apply.argtypes = [vp, vp, dp, vp]
+        L.exx_apply_to.argtypes = [vp, vp, dp, vp, vp]
         L.exx_energy.argtypes = [vp, vp, dp, vp, dp, dp]
         L.exx_apply_host.argtypes = [vp, vp, dp, vp, dp]
         L.exx_subspace.argtypes = [vp, C.c_int, vp, vp, vp]
@@ -232,6 +233,15 @@ class Exx:
         out_dev = self.empty_like_psi() if out_dev is None else out_dev
         occ = self._occ(occ)
         self._chk(lib().exx_apply(self._h, self._dev(psi_dev, self.ncoef), _dp(occ), self._dev(out_dev, self.ncoef)))
+        return out_dev
+
+    def apply_to(self, psi_dev, occ, phi_dev, out_dev=None):
+        """out = V_x[psi, occ] phi: the operator defined by the orbitals psi applied to the vectors phi (layout of psi)."""
+        occ = self._occ(occ)
+        if out_dev is None:
+            out_dev = self.empty_like_psi()
+        self._chk(lib().exx_apply_to(self._h, self._dev(psi_dev, self.ncoef), _dp(occ), self._dev(phi_dev, self.ncoef),
+                                     self._dev(out_dev, self.ncoef)))
         return out_dev
 
     def apply_sharded(self, psi_dev, occ, out_dev=None, group=None, rank=None, world=None):

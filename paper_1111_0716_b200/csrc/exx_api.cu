@@ -102,6 +102,7 @@ static void free_ctx(exx_ctx* c) {
     cudaFree(c->acc_dev);
     cudaFree(c->vx_dev);
     cudaFree(c->psi_stage_dev);
+    cudaFree(c->uphi1_dev);
     cudaFree(c->band_dot_dev);
     cudaFree(c->band_e_dev);
     cudaFree(c->occw_dev);
@@ -593,7 +594,7 @@ static void reset_counters(exx_ctx* c) {
 }
 
 // Generic pipeline, steps S1..S7 as separate kernels.
-static int apply_generic(exx_ctx* c, const double2* psi, const double* occ, double2* out) {
+static int apply_generic(exx_ctx* c, const double2* psi, const double* occ, double2* out, const double2* phi) {
     int rc;
     const int nb = c->nb, nk = c->nk;
     const int64_t Ng = c->Ng;
@@ -612,6 +613,17 @@ static int apply_generic(exx_ctx* c, const double2* psi, const double* occ, doub
                 continue;
             }
             EXX_CUDA(c, cudaMemsetAsync(c->acc_dev, 0, sizeof(double2) * (size_t)Ng, c->stream));
+            // the row's real-space box: u_nk from the cache, or (exx_apply_to) the trial vector phi_nk transformed now
+            const double2* un_base = c->u_dev + (size_t)k * nb * Ng;
+            int un_idx = n;
+            if (phi) {
+                if (!c->uphi1_dev)
+                    if ((rc = dev_alloc(c, &c->uphi1_dev, (size_t)Ng))) return rc;
+                if ((rc = launch_scatter(c, k, phi + c->off[k] + (int64_t)n * c->npw[k], 1, c->uphi1_dev))) return rc;
+                if ((rc = launch_fft3d_generic(c, c->uphi1_dev, 1, +1))) return rc;
+                un_base = c->uphi1_dev;
+                un_idx = 0;
+            }
             for (int q = 0; q < nk; q++) {
                 const double* ktab = c->ktab_dev + (size_t)c->ktab_of[(size_t)k * nk + q] * Ng;
                 const double2* uq = c->u_dev + (size_t)q * nb * Ng;
@@ -624,7 +636,7 @@ static int apply_generic(exx_ctx* c, const double2* psi, const double* occ, doub
                         mt.tm++;
                     }
                     if (mt.tm == tm_max || (m == nb && mt.tm > 0)) {
-                        if ((rc = launch_codensity_tile(c, c->u_dev + (size_t)k * nb * Ng, n, 1, uq, mt, c->work_dev))) return rc;
+                        if ((rc = launch_codensity_tile(c, un_base, un_idx, 1, uq, mt, c->work_dev))) return rc;
                         if ((rc = launch_fft3d_generic(c, c->work_dev, mt.tm, -1))) return rc;
                         if ((rc = launch_kmul(c, ktab, c->work_dev, mt.tm))) return rc;
                         if ((rc = launch_fft3d_generic(c, c->work_dev, mt.tm, +1))) return rc;
@@ -666,7 +678,7 @@ static void counters_from_inner(exx_ctx* c, const exx_ctx* in, int rc) {
     if (rc) c->last_error = in->last_error;
 }
 
-static int apply_impl(exx_ctx* c, const double2* psi, const double* occ, double2* out) {
+static int apply_impl(exx_ctx* c, const double2* psi, const double* occ, double2* out, const double2* phi = nullptr) {
     reset_counters(c);
     if (c->opt_shard_rank >= c->opt_shard_count) return EXX_ERR_BAD_ARG;
     // (an inner grid that was taken only because it has fused kernels is pointless when the generic kernels are asked for)
@@ -674,7 +686,7 @@ static int apply_impl(exx_ctx* c, const double2* psi, const double* occ, double2
         // compact work grid: same spheres, same psi/out layout, every product alias-free on both grids
         exx_ctx* in = c->inner;
         options_to_inner(c, in);
-        int rc = apply_impl(in, psi, occ, out);
+        int rc = apply_impl(in, psi, occ, out, phi);
         counters_from_inner(c, in, rc);
         return rc;
     }
@@ -684,8 +696,8 @@ static int apply_impl(exx_ctx* c, const double2* psi, const double* occ, double2
         if (rc) return rc;
     }
     bool use_fused = fused_supported(c) && c->opt_path != 1;
-    if (use_fused) return fused_apply(c, occ, psi, out);
-    return apply_generic(c, psi, occ, out);
+    if (use_fused) return fused_apply(c, occ, psi, out, phi);
+    return apply_generic(c, psi, occ, out, phi);
 }
 
 int exx_apply(exx_ctx* c, const double* psi_dev, const double* occ_host, double* out_dev) {
@@ -696,6 +708,16 @@ int exx_apply(exx_ctx* c, const double* psi_dev, const double* occ_host, double*
     size_t bytes = sizeof(double2) * (size_t)c->off[c->nk];
     if (p < o + bytes && o < p + bytes) return EXX_ERR_ALIAS;
     return apply_impl(c, (const double2*)psi_dev, occ_host, (double2*)out_dev);
+}
+
+int exx_apply_to(exx_ctx* c, const double* psi_dev, const double* occ_host, const double* phi_dev, double* out_dev) {
+    if (!c || !psi_dev || !occ_host || !phi_dev || !out_dev) return EXX_ERR_NULL;
+    int rc = check_occ(c, occ_host);
+    if (rc) return rc;
+    const char *p = (const char*)psi_dev, *f = (const char*)phi_dev, *o = (const char*)out_dev;
+    size_t bytes = sizeof(double2) * (size_t)c->off[c->nk];
+    if ((p < o + bytes && o < p + bytes) || (f < o + bytes && o < f + bytes)) return EXX_ERR_ALIAS;
+    return apply_impl(c, (const double2*)psi_dev, occ_host, (double2*)out_dev, (const double2*)phi_dev);
 }
 
 static int energy_impl(exx_ctx* c, const double2* psi, const double* occ, const double2* vx, double* ex, double* per_band) {

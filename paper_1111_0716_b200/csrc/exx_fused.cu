@@ -34,6 +34,8 @@ struct FusedState {
     double* epart_dev = nullptr;
     double* pairsum_dev = nullptr;
     double* band_e2_dev = nullptr;
+    // exx_apply_to: real-space boxes of the trial vectors phi (allocated on first use, nk*nb boxes like the u cache)
+    cplx* uphi_dev = nullptr;
 };
 
 #define EXX_DISPATCH_R1(R1v, EXPR)                  \
@@ -129,6 +131,7 @@ void fused_destroy(exx_ctx* c) {
     cudaFree(st->epart_dev);
     cudaFree(st->pairsum_dev);
     cudaFree(st->band_e2_dev);
+    cudaFree(st->uphi_dev);
     delete st;
     c->fused = nullptr;
 }
@@ -219,7 +222,9 @@ struct ModeF {
 
 template <class M>
 static int pair_loop(exx_ctx* c, FusedState* st, const double* occ, const typename M::cplx* u_base, typename M::cplx* work,
-                     const typename M::real* kperm_base, acc_c* acc, bool sym, int ta_max, int tb_max) {
+                     const typename M::real* kperm_base, acc_c* acc, bool sym, int ta_max, int tb_max,
+                     const typename M::cplx* ua_base = nullptr /* a-bands from another set of boxes (exx_apply_to; needs !sym) */) {
+    if (!ua_base) ua_base = u_base;
     int rc;
     const int nb = c->nb, nk = c->nk;
     const size_t Ng = (size_t)c->Ng;
@@ -232,7 +237,7 @@ static int pair_loop(exx_ctx* c, FusedState* st, const double* occ, const typena
         if (blk.shard != (int)c->opt_shard_rank) continue;
         const int k = blk.k, q = blk.q;
         const typename M::real* kperm = kperm_base + (size_t)c->ktab_of[(size_t)k * nk + q] * Ng;
-        const typename M::cplx* ua = u_base + (size_t)k * nb * Ng;
+        const typename M::cplx* ua = ua_base + (size_t)k * nb * Ng;
         const typename M::cplx* ub = u_base + (size_t)q * nb * Ng;
         if (bl_q != q) b_list(nb, occ, q, sym, blist), bl_q = q;
         const int a0 = blk.a0, ta = blk.ta, tb = blk.tb;
@@ -356,7 +361,8 @@ static int pair_loop(exx_ctx* c, FusedState* st, const double* occ, const typena
 }
 
 // S1: sphere coefficients -> F-layout work boxes (scatter) -> inverse transform through passes B/C -> u cache
-static int fused_u_cache(exx_ctx* c, FusedState* st, const double2* psi) {
+static int fused_u_cache(exx_ctx* c, FusedState* st, const double2* psi, cplx* u_out = nullptr) {
+    if (!u_out) u_out = (cplx*)c->u_dev;
     int rc;
     const int nb = c->nb, nk = c->nk;
     const size_t Ng = (size_t)c->Ng;
@@ -365,7 +371,7 @@ static int fused_u_cache(exx_ctx* c, FusedState* st, const double2* psi) {
         for (int n0 = 0; n0 < nb; n0 += bmax) {
             const int bn = std::min(bmax, nb - n0);
             if ((rc = launch_scatter(c, k, psi + c->off[k] + (int64_t)n0 * c->npw[k], bn, (double2*)c->work_dev, st->fmap_dev + c->map_off[k]))) return rc;
-            EXX_DISPATCH_R1(st->R1, rc = L::fft_inverse(c, (cplx*)c->work_dev, bn, (cplx*)c->u_dev + ((size_t)k * nb + n0) * Ng));
+            EXX_DISPATCH_R1(st->R1, rc = L::fft_inverse(c, (cplx*)c->work_dev, bn, u_out + ((size_t)k * nb + n0) * Ng));
             if (rc) return rc;
         }
     }
@@ -429,7 +435,7 @@ static int fused_mode32_ready(exx_ctx* c, FusedState* st) {
 //   symmetry mode: k <= q, and a <= b when k == q; pair evaluated iff f_a != 0 or f_b != 0;
 //                  acc_a -= w_q f_b u_b v   and (unless a == b)   acc_b -= w_k f_a u_a conj(v)
 // using v_{bq,ak} = conj(v_{ak,bq}) (K real and K_{q-k}(g) = K_{k-q}(-g); exact on an alias-free grid).
-int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out) {
+int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out, const double2* phi) {
     FusedState* st = (FusedState*)c->fused;
     if (!st) return EXX_ERR_BAD_ARG;
     int rc;
@@ -438,21 +444,32 @@ int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out)
     c->path_used = 2;
     c->pruned_used = 0;
     if ((rc = fused_u_cache(c, st, psi))) return rc;
+    if (phi) {  // exx_apply_to: the a-bands of every pair are the trial vectors
+        if (!st->uphi_dev) {
+            if (cudaMalloc((void**)&st->uphi_dev, sizeof(cplx) * Ng * (size_t)nk * nb) != cudaSuccess) {
+                cudaGetLastError();
+                return EXX_ERR_ALLOC;
+            }
+            c->dev_bytes += sizeof(cplx) * Ng * (size_t)nk * nb;
+        }
+        if ((rc = fused_u_cache(c, st, phi, st->uphi_dev))) return rc;
+    }
     int ta_max, tb_max;
     bool sym;
     fused_batch_shape(c, &ta_max, &tb_max, &sym);
+    if (phi) sym = false, c->symmetry_used = 0;  // v_{b,a} = conj(v_{a,b}) pairs two bands of ONE set; here a and b come from different sets
     cplx* work = (cplx*)c->work_dev;
     acc_c* acc = (acc_c*)c->acc_dev;  // one accumulator box per (k, band), always fp64
     EXX_CUDA(c, cudaMemsetAsync(acc, 0, sizeof(acc_c) * Ng * (size_t)nk * nb, c->stream));
     c->precision_used = 0;
-    if (c->opt_precision == 1) {
+    if (c->opt_precision == 1 && !phi) {
         // mixed precision (the paper's second mode): pair transforms, kernel multiply and the product with u in fp32;
         // S1, S7 and every accumulator stay fp64
         if ((rc = fused_mode32_ready(c, st))) return rc;
         if ((rc = pair_loop<ModeF>(c, st, occ, st->u32_dev, (exx32::cplx*)c->work_dev, st->kperm32_dev, acc, sym, ta_max, tb_max))) return rc;
         c->precision_used = 1;
     } else {
-        if ((rc = pair_loop<ModeD>(c, st, occ, (const cplx*)c->u_dev, work, st->kperm_dev, acc, sym, ta_max, tb_max))) return rc;
+        if ((rc = pair_loop<ModeD>(c, st, occ, (const cplx*)c->u_dev, work, st->kperm_dev, acc, sym, ta_max, tb_max, phi ? st->uphi_dev : nullptr))) return rc;
     }
     // S7: forward transform of every accumulator through passes A/B (-> F layout), gather onto sphere(k)
     for (int k = 0; k < nk; k++) {

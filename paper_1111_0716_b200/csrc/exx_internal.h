@@ -74,6 +74,7 @@ struct exx_ctx {
     size_t work_boxes = 0, acc_boxes = 0;
     double2* vx_dev = nullptr;        // internal V_x psi buffer (exx_energy with NULL, exx_apply_host)
     double2* psi_stage_dev = nullptr; // exx_apply_host staging
+    double2* uphi1_dev = nullptr;     // exx_apply_to on the generic path: one box, the current trial vector in real space
     double* band_dot_dev = nullptr;   // nk*nb Re<c|Vc>
     double* band_e_dev = nullptr;     // nk*nb + 1: per-band energies, then total
     double* occw_dev = nullptr;       // nk*nb: 1/2 w_k f_nk
@@ -188,7 +189,7 @@ bool fused_supported(const exx_ctx* c);
 void fused_tiles(const exx_ctx* c, int* tn, int* tm);
 int fused_create(exx_ctx* c);
 void fused_destroy(exx_ctx* c);
-int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out);
+int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out, const double2* phi = nullptr);  // phi: exx_apply_to
 int fused_energy(exx_ctx* c, const double* occ, const double2* psi, double* band_e2_host);  // E2 route: per-band sums w f w f K'|rho^|^2
 int fused_fft3d(exx_ctx* c, double2* in, int nbatch, int sign, double2* out);
 int fused_findex(const exx_ctx* c, int32_t* host_out);

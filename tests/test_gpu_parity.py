@@ -868,3 +868,101 @@ def test_energy_route_aliased_grid_generic_fallback_and_mixed_precision(B):
     assert g.get_info(B.EXX_INFO_PRECISION) == 1 and g.get_info(B.EXX_INFO_ENERGY_ROUTE) == 2
     assert 0 < abs(e32 - e64) <= 1e-5 * abs(e64)
     g.close()
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# exx_apply_to: the operator of (psi, occ) applied to other vectors phi (FOCK_ACC on trial wavefunctions)
+def _random_phi(w, npw_total, seed):
+    rng = np.random.default_rng(seed)
+    return rng.standard_normal(npw_total) + 1j * rng.standard_normal(npw_total)
+
+
+@pytest.mark.parametrize("name", ["kpts_frac_occ", "noncubic_hse", "tiny_aliased", "one_band", "mixed_27"])
+def test_apply_to_small_cases_against_oracle(B, name):
+    """Fused kernels on the compact grid, generic kernels (EXX_OPT_PATH = 1, pruning off) and shards: V_x[psi, occ] phi per vector
+    at the 1e-10 bar against the oracle's exx_ref_apply_to."""
+    import torch
+    w = _small(name)
+    o, g = _pair(B, w)
+    psi = w.coefficients(o.npw)
+    phi = _random_phi(w, o.ncoef, 31)
+    want = o.apply_to(psi, w.occ, phi)
+    pd, fd = g.to_device(psi), g.to_device(phi)
+    for path, prune, P in ((0, 1, 1), (1, 0, 1), (0, 1, 2), (0, 0, 3)):
+        g.set_option(B.EXX_OPT_PATH, path)
+        g.set_option(B.EXX_OPT_PRUNE, prune)
+        acc = None
+        for r in range(P):
+            g.set_option(B.EXX_OPT_SHARD_COUNT, P)
+            g.set_option(B.EXX_OPT_SHARD_RANK, r)
+            part = g.apply_to(pd, w.occ, fd).clone()
+            acc = part if acc is None else acc + part
+        g.set_option(B.EXX_OPT_SHARD_COUNT, 1)
+        g.set_option(B.EXX_OPT_SHARD_RANK, 0)
+        assert g.get_info(B.EXX_INFO_SYMMETRY) == 0
+        got = acc.cpu().numpy()
+        for k in range(w.nk):
+            for n in range(w.nbands):
+                assert _rel(o.band(got, k, n), o.band(want, k, n)) < TOL_VX, (name, path, prune, P, k, n)
+    # phi = psi is exx_apply
+    a, b = g.apply(pd, w.occ).clone(), g.apply_to(pd, w.occ, pd)
+    assert (a - b).abs().max().item() <= 1e-13 * a.abs().max().item()
+    with pytest.raises(B.ExxError):
+        g.apply_to(pd, w.occ, fd, fd)      # out may not alias phi
+    g.close()
+
+
+def test_apply_to_fused_kpoints_ragged_tiles(B):
+    nb = 11
+    occ = np.array([1, 0, 1, 0.5, 0, 0, 1, 1, 0.25, 0, 0.75], dtype=float)
+    w = W.custom("to48", 4048, (48, 48, 48), W.rhombohedral(7.5, 66.0), [[0.0, 0.0, 0.0], [0.25, -0.25, 0.5]], [0.4, 0.6], 5.0, nb, occ, 1, 0.2)
+    o, g = _pair(B, w)
+    psi = w.coefficients(o.npw)
+    phi = _random_phi(w, o.ncoef, 32)
+    want = o.apply_to(psi, w.occ, phi)
+    pd, fd = g.to_device(psi), g.to_device(phi)
+    for tile in (0, 3):
+        g.set_option(B.EXX_OPT_TILE_N, tile)
+        g.set_option(B.EXX_OPT_TILE_M, tile)
+        out = g.apply_to(pd, w.occ, fd)
+        assert g.get_info(B.EXX_INFO_PATH_USED) == 2 and g.get_info(B.EXX_INFO_PAIRS_ORDERED) == w.pair_evals
+        got = out.cpu().numpy()
+        for k in range(w.nk):
+            for n in range(nb):
+                assert _rel(o.band(got, k, n), o.band(want, k, n)) < TOL_VX, (tile, k, n)
+        again = g.apply_to(pd, w.occ, fd).cpu().numpy()
+        assert np.array_equal(again.view(np.float64), got.view(np.float64))
+    g.close()
+
+
+def test_apply_to_C3_full_size_properties_and_sampled_rows(B):
+    """BASELINE configs[2] at full size (64 bands, 64^3, HSE): trial vectors = random vectors; two of them against the oracle row by
+    row (the oracle's apply_to on a problem padded with zero vectors would take minutes, so the rows are obtained from
+    exx_ref_apply_rows on an extended orbital set with the trial vector appended at zero occupation), and the operator
+    identities that hold at any size: linearity, Hermiticity of <phi_i|V_x phi_j> (exx_subspace), phi = psi equals exx_apply."""
+    w = W.make("C3")
+    g = B.Exx.from_workload(w)
+    psi = w.coefficients(g.npw)
+    pd = g.to_device(psi)
+    phi = _random_phi(w, g.ncoef, 33)
+    fd = g.to_device(phi)
+    vphi = g.apply_to(pd, w.occ, fd).clone()
+    a = g.apply(pd, w.occ).clone()
+    b = g.apply_to(pd, w.occ, pd)
+    assert (a - b).abs().max().item() <= 1e-13 * a.abs().max().item()
+    lin = g.apply_to(pd, w.occ, 0.5 * fd + (0.25 - 1.0j) * pd)
+    assert (lin - (0.5 * vphi + (0.25 - 1.0j) * a)).abs().max().item() <= 1e-13 * vphi.abs().max().item()
+    M = g.subspace(0, fd, vphi).cpu().numpy()
+    assert np.abs(M - M.conj().T).max() <= 1e-12 * np.abs(M).max()
+    assert np.linalg.eigvalsh(0.5 * (M + M.conj().T)).max() <= 1e-12 * np.abs(M).max()
+    # sampled rows against the oracle: a context with one more band, the trial vector stored there with f = 0 (reading A16:
+    # an empty band still receives V_x, and contributes nothing as m)
+    o = R.RefExx(w.grid, w.lattice, w.kfrac, w.kweight, w.ecut, w.kernel_kind, w.mu, w.scale, w.nbands + 1)
+    got = vphi.cpu().numpy()
+    npw = g.npw[0]
+    for i in (0, 41):
+        ext = np.concatenate([psi, phi[i * npw:(i + 1) * npw]])
+        occ_ext = np.concatenate([w.occ, [0.0]])
+        row = o.apply_rows(ext, occ_ext, [(0, w.nbands)])[0]
+        assert _rel(got[i * npw:(i + 1) * npw], row) < TOL_VX, i
+    g.close()

@@ -1,7 +1,7 @@
 """GPU parity on seeded random problems (-m gpu): cell, grid (fused and generic), k-points and weights, cutoff, kernel, band count,
 occupations that differ from k-point to k-point, and every option that changes how the work is cut up (pair symmetry, compact grid,
 batch tiles, generic kernels, shards).  Each case: V_x psi per band at 1e-10 and E_x / per-band terms at 1e-11 against the oracle,
-for the shards' sum, for (E1) from the summed V_x psi and for the pair-density route from psi alone.
+for the shards' sum, for (E1) from the summed V_x psi and for the pair-density route from psi alone; then exx_apply_to on random trial vectors.
 """
 import numpy as np
 import pytest
@@ -51,6 +51,7 @@ def _case(seed):
 @pytest.mark.parametrize("block", range(6))
 def test_random_problems_against_oracle(B, block):
     ran = 0
+    rng_phi = np.random.default_rng(9000 + block)
     for seed in range(20 * block, 20 * block + 20):
         w, occ, opts = _case(seed)
         o = R.RefExx(w.grid, w.lattice, w.kfrac, w.kweight, w.ecut, w.kernel_kind, w.mu, w.scale, w.nbands)
@@ -87,6 +88,14 @@ def test_random_problems_against_oracle(B, block):
         e, pb = g.energy(pd, occ, acc)
         assert abs(e - e_want) <= tol_e and np.abs(pb - pb_want).max() <= tol_e, (seed, opts)
         assert abs(e_parts - e_want) <= tol_e and np.abs(pb_parts - pb_want).max() <= tol_e, (seed, opts)
+        # the same operator on random trial vectors (exx_apply_to), same options
+        phi = rng_phi.standard_normal(o.ncoef) + 1j * rng_phi.standard_normal(o.ncoef)
+        want_phi = o.apply_to(psi, occ, phi)
+        got_phi = g.apply_to(pd, occ, g.to_device(phi)).cpu().numpy()
+        for k in range(w.nk):
+            for n in range(w.nbands):
+                a, b = o.band(got_phi, k, n), o.band(want_phi, k, n)
+                assert np.linalg.norm(a - b) <= 1e-10 * np.linalg.norm(b) + 1e-300, (seed, opts, "apply_to", k, n)
         g.close()
         ran += 1
     assert ran >= 15

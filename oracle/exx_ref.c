@@ -462,11 +462,13 @@ int exx_ref_apply(const exx_ref_ctx *c, const double *psi, const double *occ, do
  *   rho~(g)           = (1/Ng) sum_j conj(u_mq(r_j)) t_ik(r_j) exp(-...)
  *   v(r_j)            = (1/Omega) sum_g K(|k-q+G|) rho~(g) exp(+...)
  *   (V_x t)_ik(r_j)   = - sum_q w_q sum_m f_mq u_mq(r_j) v(r_j),      out_ik(g) = (1/Ng) sum_j (V_x t)_ik(r_j) exp(-...), g in sphere(k)
- * i.e. (D) with u_nk replaced by t_ik in the co-density only.  Plain loops: rows in parallel, the (q,m) sum of a row serial in
+ * i.e. (D) with u_nk replaced by t_ik in the co-density only.  phi and out hold nphi vectors per k-point (any nphi >= 1), packed like
+ * psi: element (k,i,ig) at nphi * sum_{k'<k} npw(k') + i*npw(k) + ig.  Plain loops: rows in parallel, the (q,m) sum of a row serial in
  * loop order.  Pins (tests/test_oracle_exchange.py): closed-form eigenvalue for plane waves, phi = psi gives exx_ref_apply,
  * Hermiticity and negativity of <phi_i|V_x phi_j>, linearity in phi. */
-int exx_ref_apply_to(const exx_ref_ctx *c, const double *psi_, const double *occ, const double *phi_, double *out_) {
+int exx_ref_apply_to(const exx_ref_ctx *c, const double *psi_, const double *occ, const double *phi_, int nphi, double *out_) {
     if (!c || !psi_ || !occ || !phi_ || !out_) return EXX_REF_ERR_NULL;
+    if (nphi < 1) return EXX_REF_ERR_BAD_ARG;
     int rc = check_occ(c, occ);
     if (rc) return rc;
     const cplx *psi = (const cplx *)psi_, *phi = (const cplx *)phi_;
@@ -476,14 +478,15 @@ int exx_ref_apply_to(const exx_ref_ctx *c, const double *psi_, const double *occ
     if (!u) return EXX_REF_ERR_ALLOC;
     int fail = 0;
 #pragma omp parallel for schedule(dynamic)
-    for (int i = 0; i < c->nk * c->nb; i++) {
-        int k = i / c->nb, n = i % c->nb;
+    for (int i = 0; i < c->nk * nphi; i++) {
+        int k = i / nphi, n = i % nphi;
+        const int64_t offk = (c->off[k] / c->nb) * nphi; /* nphi * sum_{k'<k} npw(k') */
         cplx *t = malloc(sizeof(cplx) * (size_t)Ng), *w = malloc(sizeof(cplx) * (size_t)Ng), *acc = calloc((size_t)Ng, sizeof(cplx));
         double *K = malloc(sizeof(double) * (size_t)Ng);
         if (!t || !w || !acc || !K) {
             fail = 1;
         } else {
-            to_real(c, k, phi + c->off[k] + (int64_t)n * c->npw[k], t);
+            to_real(c, k, phi + offk + (int64_t)n * c->npw[k], t);
             for (int q = 0; q < c->nk; q++) {
                 exx_ref_kernel_table(c, k, q, K);
                 for (int m = 0; m < c->nb; m++) {
@@ -499,7 +502,7 @@ int exx_ref_apply_to(const exx_ref_ctx *c, const double *psi_, const double *occ
                 }
             }
             fft3d(c->N, -1, acc);
-            cplx *o = out + c->off[k] + (int64_t)n * c->npw[k];
+            cplx *o = out + offk + (int64_t)n * c->npw[k];
             for (int ig = 0; ig < c->npw[k]; ig++) o[ig] = acc[c->map[k][ig]] / (double)Ng;
         }
         free(t);

@@ -45,7 +45,7 @@ def lib():
         L.exx_ref_kernel_table.argtypes = [vp, C.c_int, C.c_int, dp]
         L.exx_ref_to_real.argtypes = [vp, C.c_int, dp, dp]
         L.exx_ref_apply.argtypes = [vp, dp, dp, dp]
-        L.exx_ref_apply_to.argtypes = [vp, dp, dp, dp, dp]
+        L.exx_ref_apply_to.argtypes = [vp, dp, dp, dp, C.c_int, dp]
         L.exx_ref_apply_rows.argtypes = [vp, dp, dp, C.c_int, ip, dp]
         L.exx_ref_apply_direct.argtypes = [vp, dp, dp, dp]
         L.exx_ref_energy.argtypes = [vp, dp, dp, dp, dp, dp]
@@ -182,12 +182,14 @@ class RefExx:
         return out
 
     def apply_to(self, psi, occ, phi):
-        """The operator built from (psi, occ) applied to the vectors phi (layout of psi)."""
+        """The operator built from (psi, occ) applied to the vectors phi: nphi vectors per k-point packed like psi
+        (nphi = phi.size / sum_k npw(k))."""
         psi, phi = _c128(psi).reshape(-1), _c128(phi).reshape(-1)
-        assert psi.size == self.ncoef and phi.size == self.ncoef
+        tot = int(sum(self.npw))
+        assert psi.size == self.ncoef and phi.size % tot == 0 and phi.size >= tot
         occ = self._occ(occ)
         out = np.empty_like(phi)
-        _chk(lib().exx_ref_apply_to(self._h, _dp(psi), _dp(occ), _dp(phi), _dp(out)))
+        _chk(lib().exx_ref_apply_to(self._h, _dp(psi), _dp(occ), _dp(phi), phi.size // tot, _dp(out)))
         return out
 
     def apply_rows(self, psi, occ, rows):

@@ -332,3 +332,38 @@ def test_apply_to_reduces_to_apply_and_operator_identities(kpts):
         assert np.linalg.eigvalsh(0.5 * (M + M.conj().T)).max() <= 1e-13 * np.abs(M).max()
     # the operator does not depend on the phase of the orbitals that define it
     assert np.linalg.norm(o.apply_to(psi * np.exp(1.1j), occ, phi) - vphi) <= 1e-13 * np.linalg.norm(vphi)
+
+
+def test_apply_to_block_of_trial_vectors():
+    """Fewer (or more) trial vectors per k-point than orbitals: each vector's result is independent of the block it travels in,
+    and the plane-wave eigenvalue holds for a block of two."""
+    w, o, psi = _small(kpts=True)
+    rng = np.random.default_rng(78)
+    tot = int(sum(o.npw))
+    full = rng.standard_normal(o.ncoef) + 1j * rng.standard_normal(o.ncoef)
+    vfull = o.apply_to(psi, w.occ, full)
+    for nphi in (1, 2, o.nbands + 2):
+        blk = np.concatenate([np.concatenate([o.band(full, k, i % o.nbands) for i in range(nphi)]) for k in range(o.nk)])
+        vblk = o.apply_to(psi, w.occ, blk)
+        assert vblk.size == nphi * tot
+        pos = 0
+        for k in range(o.nk):
+            for i in range(nphi):
+                got = vblk[pos:pos + o.npw[k]]
+                pos += o.npw[k]
+                assert np.linalg.norm(got - o.band(vfull, k, i % o.nbands)) <= 1e-14 * np.linalg.norm(got)
+    gm = [(0, 0, 0), (1, 0, 0), (0, 2, 0)]
+    f = np.array([1.0, 0.5, 0.25])
+    o2 = R.RefExx((16,) * 3, W.cubic(9.0), np.zeros((1, 3)), [1.0], 6.0, nbands=3)
+    psi2 = _plane_wave_bands(o2, [(0, n) for n in range(3)], gm)
+    m = o2.index_map(0)
+    blk = np.zeros(2 * o2.npw[0], complex)
+    gi = [(0, 0, 1), (1, 0, 0)]
+    for i, gv in enumerate(gi):
+        blk[i * o2.npw[0] + np.searchsorted(m, ((gv[0] % 16) * 16 + (gv[1] % 16)) * 16 + (gv[2] % 16))] = 1.0
+    out = o2.apply_to(psi2, f, blk)
+    Bm = 2 * np.pi / 9.0
+    for i, gv in enumerate(gi):
+        lam = -sum(fj * 4 * np.pi / (Bm ** 2 * float((np.array(gv) - np.array(b)) @ (np.array(gv) - np.array(b)))) / o2.omega
+                   for fj, b in zip(f, gm) if tuple(b) != tuple(gv))
+        assert np.linalg.norm(out[i * o2.npw[0]:(i + 1) * o2.npw[0]] - lam * blk[i * o2.npw[0]:(i + 1) * o2.npw[0]]) <= 1e-13 * abs(lam)

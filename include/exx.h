@@ -153,12 +153,14 @@ int exx_apply(exx_ctx* ctx, const double* psi_dev, const double* occ_host, doubl
 
 /* The same operator applied to OTHER vectors: out(k,i,:) = (V_x[psi, occ] phi_ki)(g), g in sphere(k), i.e. definition (D) above with
  * u_nk replaced, in the co-density only, by the real-space image of phi_ki.  This is FOCK_ACC inside an iterative eigensolver
- * (applied to blocks of NSIM bands, L143): the orbitals psi with occupations occ define the operator, the trial
- * vectors phi receive it.  phi_dev / out_dev: the layout of psi (nbands vectors per k-point; pad with zero vectors if fewer are
- * needed), device, 16-byte aligned; out may overlap neither psi nor phi.  phi == psi gives exx_apply's result (without the
- * pair symmetry, which couples two bands of one set: EXX_INFO_SYMMETRY reads 0).  Always fp64 (EXX_OPT_PRECISION is ignored).
- * Shards, tiles, pruning and paths as for exx_apply.  Asynchronous on the stream. */
-int exx_apply_to(exx_ctx* ctx, const double* psi_dev, const double* occ_host, const double* phi_dev, double* out_dev);
+ * (applied to blocks of NSIM bands, L143): the orbitals psi with occupations occ define the operator, a block of
+ * trial vectors phi receives it.  phi_dev / out_dev: nphi >= 1 vectors per k-point (any count, not tied to nbands), packed like
+ * psi: element (k,i,ig) at nphi * sum_{k'<k} npw(k') + i*npw(k) + ig; device, 16-byte aligned; out may overlap neither psi nor
+ * phi.  phi == psi (nphi = nbands) gives exx_apply's result, without the pair symmetry, which couples two bands of one set:
+ * EXX_INFO_SYMMETRY reads 0.  Always fp64 (EXX_OPT_PRECISION is ignored).  Shards, tiles, pruning and paths as for exx_apply.
+ * The first call, and any call with a larger nphi than before, allocates the trial vectors' real-space boxes and accumulators
+ * (2 nk nphi boxes).  Asynchronous on the stream. */
+int exx_apply_to(exx_ctx* ctx, const double* psi_dev, const double* occ_host, const double* phi_dev, int nphi, double* out_dev);
 
 /* E_x = 1/2 sum w_k f_nk Re<c_nk|(V_x c)_nk> (Eq. 2).  If vxpsi_dev_or_null is NULL the library evaluates E_x
  * from psi alone: by the pair-density route (EXX_OPT_ENERGY_ROUTE = 0, fused kernels; the counters of exx_get_info then describe

@@ -75,7 +75,7 @@ def lib():
         L.exx_kernel_class_name.argtypes = [C.c_int]
         L.exx_kernel_class_name.restype = C.c_char_p
         L.exx_apply.argtypes = [vp, vp, dp, vp]
-        L.exx_apply_to.argtypes = [vp, vp, dp, vp, vp]
+        L.exx_apply_to.argtypes = [vp, vp, dp, vp, C.c_int, vp]
         L.exx_energy.argtypes = [vp, vp, dp, vp, dp, dp]
         L.exx_apply_host.argtypes = [vp, vp, dp, vp, dp]
         L.exx_subspace.argtypes = [vp, C.c_int, vp, vp, vp]
@@ -236,12 +236,17 @@ class Exx:
         return out_dev
 
     def apply_to(self, psi_dev, occ, phi_dev, out_dev=None):
-        """out = V_x[psi, occ] phi: the operator defined by the orbitals psi applied to the vectors phi (layout of psi)."""
+        """out = V_x[psi, occ] phi: the operator defined by the orbitals psi applied to a block of trial vectors phi, nphi per
+        k-point packed like psi (nphi = phi.numel() / sum_k npw(k))."""
         occ = self._occ(occ)
+        tot = int(sum(self.npw))
+        n = int(phi_dev.numel())
+        if n % tot or n < tot:
+            raise ValueError("phi must hold a whole number of vectors per k-point (%d elements each set)" % tot)
         if out_dev is None:
-            out_dev = self.empty_like_psi()
-        self._chk(lib().exx_apply_to(self._h, self._dev(psi_dev, self.ncoef), _dp(occ), self._dev(phi_dev, self.ncoef),
-                                     self._dev(out_dev, self.ncoef)))
+            out_dev = self._torch.empty_like(phi_dev)
+        self._chk(lib().exx_apply_to(self._h, self._dev(psi_dev, self.ncoef), _dp(occ), self._dev(phi_dev, n), n // tot,
+                                     self._dev(out_dev, n)))
         return out_dev
 
     def apply_sharded(self, psi_dev, occ, out_dev=None, group=None, rank=None, world=None):

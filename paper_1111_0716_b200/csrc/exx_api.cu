@@ -594,7 +594,7 @@ static void reset_counters(exx_ctx* c) {
 }
 
 // Generic pipeline, steps S1..S7 as separate kernels.
-static int apply_generic(exx_ctx* c, const double2* psi, const double* occ, double2* out, const double2* phi) {
+static int apply_generic(exx_ctx* c, const double2* psi, const double* occ, double2* out, const double2* phi, int nphi) {
     int rc;
     const int nb = c->nb, nk = c->nk;
     const int64_t Ng = c->Ng;
@@ -605,11 +605,13 @@ static int apply_generic(exx_ctx* c, const double2* psi, const double* occ, doub
     if (c->opt_tile_m > 0) tm_max = (int)std::min<int64_t>(tm_max, c->opt_tile_m);
     c->tile_n_used = 1;
     c->tile_m_used = tm_max;
+    const int na = phi ? nphi : nb;  // output rows per k-point
     for (int k = 0; k < nk; k++)
-        for (int n = 0; n < nb; n++) {
-            if ((int64_t)(k * nb + n) % c->opt_shard_count != c->opt_shard_rank) {
+        for (int n = 0; n < na; n++) {
+            double2* out_row = out + c->off[k] / nb * na + (int64_t)n * c->npw[k];
+            if ((int64_t)(k * na + n) % c->opt_shard_count != c->opt_shard_rank) {
                 // another shard's output row: zero here, so that the sum over shards is the full result
-                EXX_CUDA(c, cudaMemsetAsync(out + c->off[k] + (int64_t)n * c->npw[k], 0, sizeof(double2) * (size_t)c->npw[k], c->stream));
+                EXX_CUDA(c, cudaMemsetAsync(out_row, 0, sizeof(double2) * (size_t)c->npw[k], c->stream));
                 continue;
             }
             EXX_CUDA(c, cudaMemsetAsync(c->acc_dev, 0, sizeof(double2) * (size_t)Ng, c->stream));
@@ -619,7 +621,7 @@ static int apply_generic(exx_ctx* c, const double2* psi, const double* occ, doub
             if (phi) {
                 if (!c->uphi1_dev)
                     if ((rc = dev_alloc(c, &c->uphi1_dev, (size_t)Ng))) return rc;
-                if ((rc = launch_scatter(c, k, phi + c->off[k] + (int64_t)n * c->npw[k], 1, c->uphi1_dev))) return rc;
+                if ((rc = launch_scatter(c, k, phi + c->off[k] / nb * na + (int64_t)n * c->npw[k], 1, c->uphi1_dev))) return rc;
                 if ((rc = launch_fft3d_generic(c, c->uphi1_dev, 1, +1))) return rc;
                 un_base = c->uphi1_dev;
                 un_idx = 0;
@@ -649,7 +651,7 @@ static int apply_generic(exx_ctx* c, const double2* psi, const double* occ, doub
             }
             // S7: forward transform of the accumulator, gather onto sphere(k) (the 1/(Omega Ng^2) is inside K')
             if ((rc = launch_fft3d_generic(c, c->acc_dev, 1, -1))) return rc;
-            if ((rc = launch_gather(c, k, c->acc_dev, 1, out + c->off[k] + (int64_t)n * c->npw[k]))) return rc;
+            if ((rc = launch_gather(c, k, c->acc_dev, 1, out_row))) return rc;
         }
     return EXX_OK;
 }
@@ -678,7 +680,7 @@ static void counters_from_inner(exx_ctx* c, const exx_ctx* in, int rc) {
     if (rc) c->last_error = in->last_error;
 }
 
-static int apply_impl(exx_ctx* c, const double2* psi, const double* occ, double2* out, const double2* phi = nullptr) {
+static int apply_impl(exx_ctx* c, const double2* psi, const double* occ, double2* out, const double2* phi = nullptr, int nphi = 0) {
     reset_counters(c);
     if (c->opt_shard_rank >= c->opt_shard_count) return EXX_ERR_BAD_ARG;
     // (an inner grid that was taken only because it has fused kernels is pointless when the generic kernels are asked for)
@@ -686,7 +688,7 @@ static int apply_impl(exx_ctx* c, const double2* psi, const double* occ, double2
         // compact work grid: same spheres, same psi/out layout, every product alias-free on both grids
         exx_ctx* in = c->inner;
         options_to_inner(c, in);
-        int rc = apply_impl(in, psi, occ, out, phi);
+        int rc = apply_impl(in, psi, occ, out, phi, nphi);
         counters_from_inner(c, in, rc);
         return rc;
     }
@@ -696,8 +698,8 @@ static int apply_impl(exx_ctx* c, const double2* psi, const double* occ, double2
         if (rc) return rc;
     }
     bool use_fused = fused_supported(c) && c->opt_path != 1;
-    if (use_fused) return fused_apply(c, occ, psi, out, phi);
-    return apply_generic(c, psi, occ, out, phi);
+    if (use_fused) return fused_apply(c, occ, psi, out, phi, nphi);
+    return apply_generic(c, psi, occ, out, phi, nphi);
 }
 
 int exx_apply(exx_ctx* c, const double* psi_dev, const double* occ_host, double* out_dev) {
@@ -710,14 +712,15 @@ int exx_apply(exx_ctx* c, const double* psi_dev, const double* occ_host, double*
     return apply_impl(c, (const double2*)psi_dev, occ_host, (double2*)out_dev);
 }
 
-int exx_apply_to(exx_ctx* c, const double* psi_dev, const double* occ_host, const double* phi_dev, double* out_dev) {
+int exx_apply_to(exx_ctx* c, const double* psi_dev, const double* occ_host, const double* phi_dev, int nphi, double* out_dev) {
     if (!c || !psi_dev || !occ_host || !phi_dev || !out_dev) return EXX_ERR_NULL;
+    if (nphi < 1 || nphi > 65536) return EXX_ERR_BAD_ARG;
     int rc = check_occ(c, occ_host);
     if (rc) return rc;
     const char *p = (const char*)psi_dev, *f = (const char*)phi_dev, *o = (const char*)out_dev;
-    size_t bytes = sizeof(double2) * (size_t)c->off[c->nk];
-    if ((p < o + bytes && o < p + bytes) || (f < o + bytes && o < f + bytes)) return EXX_ERR_ALIAS;
-    return apply_impl(c, (const double2*)psi_dev, occ_host, (double2*)out_dev, (const double2*)phi_dev);
+    const size_t bytes_psi = sizeof(double2) * (size_t)c->off[c->nk], bytes_phi = bytes_psi / c->nb * nphi;
+    if ((p < o + bytes_phi && o < p + bytes_psi) || (f < o + bytes_phi && o < f + bytes_phi)) return EXX_ERR_ALIAS;
+    return apply_impl(c, (const double2*)psi_dev, occ_host, (double2*)out_dev, (const double2*)phi_dev, nphi);
 }
 
 static int energy_impl(exx_ctx* c, const double2* psi, const double* occ, const double2* vx, double* ex, double* per_band) {

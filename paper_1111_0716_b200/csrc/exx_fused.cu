@@ -36,6 +36,7 @@ struct FusedState {
     double* band_e2_dev = nullptr;
     // exx_apply_to: real-space boxes of the trial vectors phi (allocated on first use, nk*nb boxes like the u cache)
     cplx* uphi_dev = nullptr;
+    size_t uphi_boxes = 0;
 };
 
 #define EXX_DISPATCH_R1(R1v, EXPR)                  \
@@ -223,21 +224,23 @@ struct ModeF {
 template <class M>
 static int pair_loop(exx_ctx* c, FusedState* st, const double* occ, const typename M::cplx* u_base, typename M::cplx* work,
                      const typename M::real* kperm_base, acc_c* acc, bool sym, int ta_max, int tb_max,
-                     const typename M::cplx* ua_base = nullptr /* a-bands from another set of boxes (exx_apply_to; needs !sym) */) {
+                     const typename M::cplx* ua_base = nullptr /* a-bands from another set of boxes (exx_apply_to; needs !sym) */,
+                     int na = -1 /* ... na of them per k-point, boxes (k * na + a) */) {
     if (!ua_base) ua_base = u_base;
+    if (na < 0) na = c->nb;
     int rc;
     const int nb = c->nb, nk = c->nk;
     const size_t Ng = (size_t)c->Ng;
     // the batch list and its owners (exx_shard.h); one shard = the whole list
     std::vector<PairBlock> blocks;
-    plan_blocks(nk, nb, occ, sym, ta_max, tb_max, (int)c->opt_shard_count, blocks);
+    plan_blocks(nk, nb, occ, sym, ta_max, tb_max, (int)c->opt_shard_count, blocks, na);
     std::vector<int> blist;
     int bl_q = -1;
     for (const PairBlock& blk : blocks) {
         if (blk.shard != (int)c->opt_shard_rank) continue;
         const int k = blk.k, q = blk.q;
         const typename M::real* kperm = kperm_base + (size_t)c->ktab_of[(size_t)k * nk + q] * Ng;
-        const typename M::cplx* ua = ua_base + (size_t)k * nb * Ng;
+        const typename M::cplx* ua = ua_base + (size_t)k * na * Ng;
         const typename M::cplx* ub = u_base + (size_t)q * nb * Ng;
         if (bl_q != q) b_list(nb, occ, q, sym, blist), bl_q = q;
         const int a0 = blk.a0, ta = blk.ta, tb = blk.tb;
@@ -250,7 +253,7 @@ static int pair_loop(exx_ctx* c, FusedState* st, const double* occ, const typena
         for (int j = 0; j < tb; j++) aj.b_idx[j] = blist[b0 + j];
         for (int i = 0; i < ta; i++)
             for (int j = 0; j < tb; j++) {
-                const double fa = occ[k * nb + aj.a_idx[i]], fb = occ[q * nb + aj.b_idx[j]];
+                const double fa = aj.a_idx[i] < nb ? occ[k * nb + aj.a_idx[i]] : 0.0, fb = occ[q * nb + aj.b_idx[j]];
                 bool e = pair_evaluated(sym, k, q, aj.a_idx[i], aj.b_idx[j], fa, fb);
                 ev[i][j] = e;
                 if (e) {
@@ -282,7 +285,7 @@ static int pair_loop(exx_ctx* c, FusedState* st, const double* occ, const typena
                     if (ev[i][j] && occ[q * nb + aj.b_idx[j]] != 0.0) cj.col[cj.nr][n++] = (unsigned char)j;
                 if (n) {
                     cj.cnt[cj.nr] = n;
-                    cj.tgt[cj.nr] = k * nb + aj.a_idx[i];
+                    cj.tgt[cj.nr] = k * na + aj.a_idx[i];
                     rowbox[cj.nr] = i;
                     cj.nr++;
                     units += n;
@@ -361,17 +364,21 @@ static int pair_loop(exx_ctx* c, FusedState* st, const double* occ, const typena
 }
 
 // S1: sphere coefficients -> F-layout work boxes (scatter) -> inverse transform through passes B/C -> u cache
-static int fused_u_cache(exx_ctx* c, FusedState* st, const double2* psi, cplx* u_out = nullptr) {
+// nvec vectors per k-point (default nb), packed like psi; box (k, n) goes to u_out[(k * stride + n) * Ng] (stride default nb)
+static int fused_u_cache(exx_ctx* c, FusedState* st, const double2* psi, cplx* u_out = nullptr, int nvec = -1, int stride = -1) {
     if (!u_out) u_out = (cplx*)c->u_dev;
+    if (nvec < 0) nvec = c->nb;
+    if (stride < 0) stride = c->nb;
     int rc;
     const int nb = c->nb, nk = c->nk;
     const size_t Ng = (size_t)c->Ng;
     for (int k = 0; k < nk; k++) {
-        const int bmax = (int)std::min<size_t>(c->work_boxes, (size_t)nb);
-        for (int n0 = 0; n0 < nb; n0 += bmax) {
-            const int bn = std::min(bmax, nb - n0);
-            if ((rc = launch_scatter(c, k, psi + c->off[k] + (int64_t)n0 * c->npw[k], bn, (double2*)c->work_dev, st->fmap_dev + c->map_off[k]))) return rc;
-            EXX_DISPATCH_R1(st->R1, rc = L::fft_inverse(c, (cplx*)c->work_dev, bn, u_out + ((size_t)k * nb + n0) * Ng));
+        const int bmax = (int)std::min<size_t>(c->work_boxes, (size_t)nvec);
+        const int64_t offk = c->off[k] / nb * nvec;
+        for (int n0 = 0; n0 < nvec; n0 += bmax) {
+            const int bn = std::min(bmax, nvec - n0);
+            if ((rc = launch_scatter(c, k, psi + offk + (int64_t)n0 * c->npw[k], bn, (double2*)c->work_dev, st->fmap_dev + c->map_off[k]))) return rc;
+            EXX_DISPATCH_R1(st->R1, rc = L::fft_inverse(c, (cplx*)c->work_dev, bn, u_out + ((size_t)k * stride + n0) * Ng));
             if (rc) return rc;
         }
     }
@@ -435,7 +442,7 @@ static int fused_mode32_ready(exx_ctx* c, FusedState* st) {
 //   symmetry mode: k <= q, and a <= b when k == q; pair evaluated iff f_a != 0 or f_b != 0;
 //                  acc_a -= w_q f_b u_b v   and (unless a == b)   acc_b -= w_k f_a u_a conj(v)
 // using v_{bq,ak} = conj(v_{ak,bq}) (K real and K_{q-k}(g) = K_{k-q}(-g); exact on an alias-free grid).
-int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out, const double2* phi) {
+int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out, const double2* phi, int nphi) {
     FusedState* st = (FusedState*)c->fused;
     if (!st) return EXX_ERR_BAD_ARG;
     int rc;
@@ -445,22 +452,29 @@ int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out,
     c->pruned_used = 0;
     if ((rc = fused_u_cache(c, st, psi))) return rc;
     if (phi) {  // exx_apply_to: the a-bands of every pair are the trial vectors
-        if (!st->uphi_dev) {
-            if (cudaMalloc((void**)&st->uphi_dev, sizeof(cplx) * Ng * (size_t)nk * nb) != cudaSuccess) {
+        if (st->uphi_boxes < (size_t)nk * nphi) {  // grown on demand; accumulators of the trial vectors sit behind their boxes
+            cudaFree(st->uphi_dev);
+            st->uphi_dev = nullptr;
+            c->dev_bytes -= 2 * sizeof(cplx) * Ng * st->uphi_boxes;
+            st->uphi_boxes = 0;
+            if (cudaMalloc((void**)&st->uphi_dev, 2 * sizeof(cplx) * Ng * (size_t)nk * nphi) != cudaSuccess) {
                 cudaGetLastError();
                 return EXX_ERR_ALLOC;
             }
-            c->dev_bytes += sizeof(cplx) * Ng * (size_t)nk * nb;
+            st->uphi_boxes = (size_t)nk * nphi;
+            c->dev_bytes += 2 * sizeof(cplx) * Ng * st->uphi_boxes;
         }
-        if ((rc = fused_u_cache(c, st, phi, st->uphi_dev))) return rc;
+        if ((rc = fused_u_cache(c, st, phi, st->uphi_dev, nphi, nphi))) return rc;
     }
+    const int na = phi ? nphi : nb;  // a-bands per k-point
     int ta_max, tb_max;
     bool sym;
     fused_batch_shape(c, &ta_max, &tb_max, &sym);
     if (phi) sym = false, c->symmetry_used = 0;  // v_{b,a} = conj(v_{a,b}) pairs two bands of ONE set; here a and b come from different sets
     cplx* work = (cplx*)c->work_dev;
-    acc_c* acc = (acc_c*)c->acc_dev;  // one accumulator box per (k, band), always fp64
-    EXX_CUDA(c, cudaMemsetAsync(acc, 0, sizeof(acc_c) * Ng * (size_t)nk * nb, c->stream));
+    // one accumulator box per (k, band), always fp64; exx_apply_to: per (k, trial vector), behind the trial vectors' boxes
+    acc_c* acc = phi ? (acc_c*)(st->uphi_dev + Ng * st->uphi_boxes) : (acc_c*)c->acc_dev;
+    EXX_CUDA(c, cudaMemsetAsync(acc, 0, sizeof(acc_c) * Ng * (size_t)nk * na, c->stream));
     c->precision_used = 0;
     if (c->opt_precision == 1 && !phi) {
         // mixed precision (the paper's second mode): pair transforms, kernel multiply and the product with u in fp32;
@@ -469,16 +483,17 @@ int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out,
         if ((rc = pair_loop<ModeF>(c, st, occ, st->u32_dev, (exx32::cplx*)c->work_dev, st->kperm32_dev, acc, sym, ta_max, tb_max))) return rc;
         c->precision_used = 1;
     } else {
-        if ((rc = pair_loop<ModeD>(c, st, occ, (const cplx*)c->u_dev, work, st->kperm_dev, acc, sym, ta_max, tb_max, phi ? st->uphi_dev : nullptr))) return rc;
+        if ((rc = pair_loop<ModeD>(c, st, occ, (const cplx*)c->u_dev, work, st->kperm_dev, acc, sym, ta_max, tb_max, phi ? st->uphi_dev : nullptr, na))) return rc;
     }
     // S7: forward transform of every accumulator through passes A/B (-> F layout), gather onto sphere(k)
     for (int k = 0; k < nk; k++) {
-        const int bmax = (int)std::min<size_t>(c->work_boxes, (size_t)nb);
-        for (int n0 = 0; n0 < nb; n0 += bmax) {
-            const int bn = std::min(bmax, nb - n0);
-            EXX_DISPATCH_R1(st->R1, rc = L::fft_forward(c, (const cplx*)(acc + ((size_t)k * nb + n0) * Ng), bn, work));
+        const int bmax = (int)std::min<size_t>(c->work_boxes, (size_t)na);
+        const int64_t offk = c->off[k] / nb * na;
+        for (int n0 = 0; n0 < na; n0 += bmax) {
+            const int bn = std::min(bmax, na - n0);
+            EXX_DISPATCH_R1(st->R1, rc = L::fft_forward(c, (const cplx*)(acc + ((size_t)k * na + n0) * Ng), bn, work));
             if (rc) return rc;
-            if ((rc = launch_gather(c, k, (const double2*)work, bn, out + c->off[k] + (int64_t)n0 * c->npw[k], st->fmap_dev + c->map_off[k]))) return rc;
+            if ((rc = launch_gather(c, k, (const double2*)work, bn, out + offk + (int64_t)n0 * c->npw[k], st->fmap_dev + c->map_off[k]))) return rc;
         }
     }
     return EXX_OK;

@@ -189,7 +189,7 @@ bool fused_supported(const exx_ctx* c);
 void fused_tiles(const exx_ctx* c, int* tn, int* tm);
 int fused_create(exx_ctx* c);
 void fused_destroy(exx_ctx* c);
-int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out, const double2* phi = nullptr);  // phi: exx_apply_to
+int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out, const double2* phi = nullptr, int nphi = 0);  // phi, nphi: exx_apply_to
 int fused_energy(exx_ctx* c, const double* occ, const double2* psi, double* band_e2_host);  // E2 route: per-band sums w f w f K'|rho^|^2
 int fused_fft3d(exx_ctx* c, double2* in, int nbatch, int sign, double2* out);
 int fused_findex(const exx_ctx* c, int32_t* host_out);

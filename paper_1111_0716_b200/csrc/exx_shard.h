@@ -40,24 +40,26 @@ inline bool pair_evaluated(bool sym, int k, int q, int a, int b, double fa, doub
 
 // All non-empty batches in loop order, each assigned to a shard: longest-processing-time first (batches sorted by cost,
 // ties in loop order, each to the least loaded shard, ties to the lowest rank) — deterministic, the same on every rank.
-inline void plan_blocks(int nk, int nb, const double* occ, bool sym, int ta_max, int tb_max, int nshards, std::vector<PairBlock>& out) {
+// na: number of a-bands per k-point (default nb; exx_apply_to with a block of na trial vectors: a = 0 .. na-1, needs !sym)
+inline void plan_blocks(int nk, int nb, const double* occ, bool sym, int ta_max, int tb_max, int nshards, std::vector<PairBlock>& out, int na = -1) {
     out.clear();
+    if (na < 0) na = nb;
     std::vector<int> blist;
     for (int k = 0; k < nk; k++)
         for (int q = sym ? k : 0; q < nk; q++) {
             b_list(nb, occ, q, sym, blist);
-            for (int a0 = 0; a0 < nb; a0 += ta_max)
+            for (int a0 = 0; a0 < na; a0 += ta_max)
                 for (size_t b0 = (sym && k == q) ? (size_t)a0 : 0; b0 < blist.size(); b0 += tb_max) {
                     PairBlock p;
                     p.k = k, p.q = q, p.a0 = a0, p.b0 = (int)b0;
-                    p.ta = std::min(ta_max, nb - a0);
+                    p.ta = std::min(ta_max, na - a0);
                     p.tb = (int)std::min<size_t>(tb_max, blist.size() - b0);
                     p.npairs = p.units_a = p.units_b = 0;
                     p.shard = 0;
                     for (int i = 0; i < p.ta; i++)
                         for (int j = 0; j < p.tb; j++) {
                             const int a = a0 + i, b = blist[b0 + j];
-                            const double fa = occ[k * nb + a], fb = occ[q * nb + b];
+                            const double fa = a < nb ? occ[k * nb + a] : 0.0, fb = occ[q * nb + b];  // (fa is used with sym only)
                             if (!pair_evaluated(sym, k, q, a, b, fa, fb)) continue;
                             p.npairs++;
                             if (fb != 0.0) p.units_a++;

@@ -921,6 +921,23 @@ def test_apply_to_fused_kpoints_ragged_tiles(B):
     phi = _random_phi(w, o.ncoef, 32)
     want = o.apply_to(psi, w.occ, phi)
     pd, fd = g.to_device(psi), g.to_device(phi)
+    # blocks of 1, 3 and nb + 2 trial vectors per k-point (FOCK_ACC's NSIM blocks), default and small ragged tiles, generic path
+    tot = int(sum(o.npw))
+    for nphi, tile, path in ((1, 0, 0), (3, 2, 0), (nb + 2, 3, 0), (3, 0, 1)):
+        blk = _random_phi(w, nphi * tot, 40 + nphi)
+        want_b = o.apply_to(psi, w.occ, blk)
+        g.set_option(B.EXX_OPT_TILE_N, tile)
+        g.set_option(B.EXX_OPT_TILE_M, tile)
+        g.set_option(B.EXX_OPT_PATH, path)
+        got_b = g.apply_to(pd, w.occ, g.to_device(blk)).cpu().numpy()
+        assert g.get_info(B.EXX_INFO_PAIRS_ORDERED) == w.nk * w.nk * nphi * w.nocc
+        pos = 0
+        for k in range(w.nk):
+            for i in range(nphi):
+                sl = slice(pos, pos + o.npw[k])
+                pos += o.npw[k]
+                assert _rel(got_b[sl], want_b[sl]) < TOL_VX, (nphi, tile, path, k, i)
+    g.set_option(B.EXX_OPT_PATH, 0)
     for tile in (0, 3):
         g.set_option(B.EXX_OPT_TILE_N, tile)
         g.set_option(B.EXX_OPT_TILE_M, tile)

@@ -84,6 +84,11 @@ enum {
                                apply_sharded does).  Fused path: the pair batches of exx_shard_plan; generic path: output rows
                                (k,n) with (k nbands + n) mod P = rank, the other rows of `out` zero */
     EXX_OPT_SHARD_RANK = 10, /* 0 .. P-1 (default 0); exx_apply returns EXX_ERR_BAD_ARG while rank >= P */
+    EXX_OPT_KEEP_U = 12,    /* 1: the caller promises that psi is the same as in the previous exx_apply / exx_apply_to / exx_energy call on this
+                               context (same work grid): the real-space images u_nk(r) kept from that call are used and S1 of psi is
+                               skipped (fused path; the generic kernels ignore it).  For an eigensolver that calls exx_apply_to on many
+                               blocks of trial vectors between two updates of the orbitals.  0 (default): S1 of psi in every call.
+                               Set it back to 0 for the first call after psi changes */
     EXX_OPT_ENERGY_ROUTE = 11 /* what exx_energy does when it is given no V_x psi.  0 (default): the pair-density route
                                E_x = -1/2 sum w_k w_q f_nk f_mq sum_g K'_{k-q}(g) |rho^_{nk,mq}(g)|^2 (form (E2) of DESIGN.md section 2:
                                Eq. 2 of PAPER.md, L127-130, written in reciprocal space) wherever the fused kernels run: the co-density

@@ -484,6 +484,9 @@ int exx_set_option(exx_ctx* c, int option, int64_t value) {
         if (value != 0 && value != 1) return EXX_ERR_BAD_ARG;
         c->opt_energy_route = value;
         return EXX_OK;
+    case EXX_OPT_KEEP_U:
+        c->opt_keep_u = value ? 1 : 0;
+        return EXX_OK;
     default: return EXX_ERR_BAD_ARG;
     }
 }
@@ -500,6 +503,7 @@ int exx_get_option(const exx_ctx* c, int option, int64_t* value) {
     case EXX_OPT_SHARD_COUNT: *value = c->opt_shard_count; return EXX_OK;
     case EXX_OPT_SHARD_RANK: *value = c->opt_shard_rank; return EXX_OK;
     case EXX_OPT_ENERGY_ROUTE: *value = c->opt_energy_route; return EXX_OK;
+    case EXX_OPT_KEEP_U: *value = c->opt_keep_u; return EXX_OK;
     default: return EXX_ERR_BAD_ARG;
     }
 }
@@ -600,6 +604,7 @@ static int apply_generic(exx_ctx* c, const double2* psi, const double* occ, doub
     const int64_t Ng = c->Ng;
     c->path_used = 1;
     c->pruned_used = 0;
+    c->u_valid = false;  // EXX_OPT_KEEP_U is a promise about the fused path's cache only
     if ((rc = compute_u_cache(c, psi))) return rc;
     int tm_max = (int)std::min<size_t>(c->work_boxes, 32);
     if (c->opt_tile_m > 0) tm_max = (int)std::min<int64_t>(tm_max, c->opt_tile_m);
@@ -663,6 +668,7 @@ static void options_to_inner(const exx_ctx* c, exx_ctx* in) {
     in->opt_profile = c->opt_profile;
     in->opt_symmetry = c->opt_symmetry;
     in->opt_precision = c->opt_precision;
+    in->opt_keep_u = c->opt_keep_u;
     in->opt_shard_count = c->opt_shard_count;
     in->opt_shard_rank = c->opt_shard_rank;
 }

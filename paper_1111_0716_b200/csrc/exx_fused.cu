@@ -450,7 +450,10 @@ int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out,
     const size_t Ng = (size_t)c->Ng;
     c->path_used = 2;
     c->pruned_used = 0;
-    if ((rc = fused_u_cache(c, st, psi))) return rc;
+    if (!(c->opt_keep_u && c->u_valid)) {  // EXX_OPT_KEEP_U: psi unchanged since the previous call, its real-space boxes still stand
+        if ((rc = fused_u_cache(c, st, psi))) return rc;
+        c->u_valid = true;
+    }
     if (phi) {  // exx_apply_to: the a-bands of every pair are the trial vectors
         if (st->uphi_boxes < (size_t)nk * nphi) {  // grown on demand; accumulators of the trial vectors sit behind their boxes
             cudaFree(st->uphi_dev);
@@ -559,7 +562,10 @@ int fused_energy(exx_ctx* c, const double* occ, const double2* psi, double* band
     const int nb = c->nb, nk = c->nk;
     c->path_used = 2;
     c->pruned_used = 0;
-    if ((rc = fused_u_cache(c, st, psi))) return rc;
+    if (!(c->opt_keep_u && c->u_valid)) {  // EXX_OPT_KEEP_U: psi unchanged since the previous call, its real-space boxes still stand
+        if ((rc = fused_u_cache(c, st, psi))) return rc;
+        c->u_valid = true;
+    }
     int ta_max, tb_max;
     bool sym;
     fused_batch_shape(c, &ta_max, &tb_max, &sym);

@@ -100,6 +100,8 @@ struct exx_ctx {
 
     // options
     int64_t opt_path = 0, opt_tile_n = 0, opt_tile_m = 0, opt_prune = 1, opt_profile = 0, opt_symmetry = 1, opt_precision = 0;
+    int64_t opt_keep_u = 0;        // 1: the caller promises psi is unchanged since the previous call: S1 of psi is skipped (fused path)
+    bool u_valid = false;          // the u cache holds S1 of the psi of the previous call (fused path)
     int64_t opt_energy_route = 0;  // 0 auto (pair-density route E2 where the fused path runs), 1 always E1 from V_x psi
     int64_t energy_route_used = 0;
     int64_t opt_shard_count = 1, opt_shard_rank = 0;  // S8(f)-4: this context runs shard rank of count (exx_shard.h)

@@ -938,6 +938,20 @@ def test_apply_to_fused_kpoints_ragged_tiles(B):
                 pos += o.npw[k]
                 assert _rel(got_b[sl], want_b[sl]) < TOL_VX, (nphi, tile, path, k, i)
     g.set_option(B.EXX_OPT_PATH, 0)
+    # EXX_OPT_KEEP_U: psi unchanged between calls -> S1 of psi skipped, same bits; a changed psi with the option off is picked up
+    g.set_option(B.EXX_OPT_TILE_N, 0)
+    g.set_option(B.EXX_OPT_TILE_M, 0)
+    blk = g.to_device(_random_phi(w, 2 * tot, 50))
+    first = g.apply_to(pd, w.occ, blk).clone()
+    n_first = g.get_info(B.EXX_INFO_LAUNCHES)
+    g.set_option(B.EXX_OPT_KEEP_U, 1)
+    kept = g.apply_to(pd, w.occ, blk)
+    assert g.get_info(B.EXX_INFO_LAUNCHES) < n_first and bool((kept == first).all())
+    e_keep, _ = g.energy(pd, w.occ, None)
+    g.set_option(B.EXX_OPT_KEEP_U, 0)
+    assert e_keep == g.energy(pd, w.occ, None)[0]
+    other = g.apply_to(pd * (0.5 + 0.5j), w.occ, blk)       # |0.5 + 0.5i|^2 = 1/2: the operator is quadratic in the orbitals
+    assert (other - 0.5 * first).abs().max().item() <= 1e-13 * first.abs().max().item()
     for tile in (0, 3):
         g.set_option(B.EXX_OPT_TILE_N, tile)
         g.set_option(B.EXX_OPT_TILE_M, tile)

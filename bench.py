@@ -280,6 +280,29 @@ def run_ours(args, rank, world, local):
                        "gpu_launches": g.get_info(B.EXX_INFO_LAUNCHES), "E_x": ex_q}
         assert abs(ex_q - ex) <= (1e-11 if args.precision == "fp64" else 1e-5) * abs(ex)
 
+    # ---- the operator applied to a block of trial vectors (exx_apply_to; FOCK_ACC's NSIM block): for information
+    apply_to = None
+    if not shard and args.precision == "fp64":
+        nphi = min(8, w.nbands)
+        tot = int(sum(g.npw))
+        gen = torch.Generator(device="cuda").manual_seed(1234)
+        blk = torch.view_as_complex(torch.randn(nphi * tot, 2, dtype=torch.float64, device="cuda", generator=gen))
+        blk_out = torch.empty_like(blk)
+        g.set_option(B.EXX_OPT_KEEP_U, 1)          # psi does not change between these calls
+        g.apply_to(pd, occ, blk, blk_out)
+        sync_all()
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0.record()
+        for _ in range(args.steps):
+            g.apply_to(pd, occ, blk, blk_out)
+        a1.record()
+        sync_all()
+        g.set_option(B.EXX_OPT_KEEP_U, 0)
+        ms_a = max_over_ranks(a0.elapsed_time(a1), world, dev) / args.steps
+        pa = g.get_info(B.EXX_INFO_PAIRS_EXECUTED)
+        apply_to = {"nphi_per_k": nphi, "ms_per_call": ms_a, "pairs_executed": pa, "us_per_pair": 1e3 * ms_a / max(1, pa),
+                    "value": world * pa / (ms_a * 1e-3), "unit": UNIT, "gpu_launches": g.get_info(B.EXX_INFO_LAUNCHES), "keep_u": 1}
+
     # ---- timed region 3: end to end through exx_apply_host, pinned host buffers, copies inside the timed region
     for _ in range(min(2, args.warmup)):
         step_host()
@@ -315,6 +338,8 @@ def run_ours(args, rank, world, local):
         line["full_grid"] = full
     if energy_only is not None:
         line["energy_only"] = energy_only
+    if apply_to is not None:
+        line["apply_to"] = apply_to
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"] = cpu_baseline(w, psi)
     if rank == 0:

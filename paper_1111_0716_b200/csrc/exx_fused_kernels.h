@@ -188,8 +188,11 @@ __global__ void pair_sum_kernel(const double* __restrict__ epart, int ntiles, do
 }
 // band_e2[band] += (w f)_band * sum over the band's pairs of (w f)_partner * pairsum: one thread per band and side, pairs in list
 // order, side a before side b (a diagonal block has the same bands on both sides), launches serial on the stream: deterministic.
-__global__ void band_energy_kernel(AJob job, EJob ej, const double* __restrict__ pairsum, double* __restrict__ band_e2) {
+__global__ void band_energy_kernel(AJob job, EJob ej, const double* __restrict__ pairsum_g, double* __restrict__ band_e2) {
     const int t = threadIdx.x;
+    __shared__ double pairsum[TMAX * TMAX];  // staged once: the serial loops below then run at shared-memory latency
+    for (int p = t; p < job.npairs; p += blockDim.x) pairsum[p] = pairsum_g[p];
+    __syncthreads();
     if (t < TMAX) {
         double s = 0.0;
         bool any = false;

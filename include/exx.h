@@ -182,6 +182,11 @@ int exx_energy(exx_ctx* ctx, const double* psi_dev, const double* occ_host, cons
  * Asynchronous on the stream.  Hermitian when vxpsi = V_x psi and every band is occupied. */
 int exx_subspace(exx_ctx* ctx, int ik, const double* psi_dev, const double* vxpsi_dev, double* m_dev);
 
+/* The same matrix for a block of trial vectors (the layout of exx_apply_to: nphi vectors per k-point in phi_dev and vphi_dev):
+ * m_dev[i*nphi + j] = sum_g conj(phi_i(g)) vphi_j(g) within k-point ik, nphi x nphi complex128, row-major, device — the projected
+ * operator <phi_i|V_x|phi_j> an iterative eigensolver builds from exx_apply_to's output.  Asynchronous. */
+int exx_subspace_block(exx_ctx* ctx, int ik, const double* phi_dev, const double* vphi_dev, int nphi, double* m_dev);
+
 /* Same as exx_apply (+ exx_energy when ex_host_or_null != NULL) on HOST buffers: copies psi to the device, applies,
  * copies out back; synchronises.  Pinned host memory makes the copies asynchronous, pageable memory works too. */
 int exx_apply_host(exx_ctx* ctx, const double* psi_host, const double* occ_host, double* out_host, double* ex_host_or_null);

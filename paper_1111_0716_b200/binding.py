@@ -26,7 +26,7 @@ EXX_INFO_ENERGY_ROUTE = 16
 SYMBOLS = ("exx_create", "exx_destroy", "exx_npw", "exx_index_map", "exx_psi_offset", "exx_set_option", "exx_get_option",
            "exx_get_info", "exx_get_kernel_time", "exx_kernel_class_name", "exx_apply", "exx_energy", "exx_apply_host",
            "exx_scatter", "exx_gather", "exx_fft3d", "exx_to_real", "exx_kernel_table", "exx_strerror", "exx_last_error",
-           "exx_version", "exx_subspace", "exx_fft3d_fused", "exx_findex", "exx_shard_plan", "exx_apply_to")
+           "exx_version", "exx_subspace", "exx_fft3d_fused", "exx_findex", "exx_shard_plan", "exx_apply_to", "exx_subspace_block")
 
 
 class KernelParams(C.Structure):
@@ -77,6 +77,7 @@ def lib():
         L.exx_kernel_class_name.restype = C.c_char_p
         L.exx_apply.argtypes = [vp, vp, dp, vp]
         L.exx_apply_to.argtypes = [vp, vp, dp, vp, C.c_int, vp]
+        L.exx_subspace_block.argtypes = [vp, C.c_int, vp, vp, C.c_int, vp]
         L.exx_energy.argtypes = [vp, vp, dp, vp, dp, dp]
         L.exx_apply_host.argtypes = [vp, vp, dp, vp, dp]
         L.exx_subspace.argtypes = [vp, C.c_int, vp, vp, vp]
@@ -305,6 +306,17 @@ class Exx:
             m_dev = self._torch.empty((self.nbands, self.nbands), dtype=self._torch.complex128, device="cuda")
         self._chk(lib().exx_subspace(self._h, ik, self._dev(psi_dev, self.ncoef), self._dev(vxpsi_dev, self.ncoef),
                                      self._dev(m_dev, self.nbands * self.nbands)))
+        return m_dev
+
+    def subspace_block(self, ik, phi_dev, vphi_dev, m_dev=None):
+        """M[i, j] = <phi_i | vphi_j> within k-point ik for blocks of nphi vectors per k-point (layout of apply_to)."""
+        tot = int(sum(self.npw))
+        n = int(phi_dev.numel())
+        nphi = n // tot
+        if m_dev is None:
+            m_dev = self._torch.empty((nphi, nphi), dtype=self._torch.complex128, device="cuda")
+        self._chk(lib().exx_subspace_block(self._h, ik, self._dev(phi_dev, nphi * tot), self._dev(vphi_dev, nphi * tot), nphi,
+                                           self._dev(m_dev, nphi * nphi)))
         return m_dev
 
     def apply_host(self, psi_host, occ, out_host=None, want_energy=True):

@@ -826,6 +826,12 @@ int exx_subspace(exx_ctx* c, int ik, const double* psi_dev, const double* vxpsi_
     return launch_subspace(c, ik, (const double2*)psi_dev, (const double2*)vxpsi_dev, (double2*)m_dev);
 }
 
+int exx_subspace_block(exx_ctx* c, int ik, const double* phi_dev, const double* vphi_dev, int nphi, double* m_dev) {
+    if (!c || !phi_dev || !vphi_dev || !m_dev) return EXX_ERR_NULL;
+    if (ik < 0 || ik >= c->nk || nphi < 1 || nphi > 65536) return EXX_ERR_BAD_ARG;
+    return launch_subspace(c, ik, (const double2*)phi_dev, (const double2*)vphi_dev, (double2*)m_dev, nphi);
+}
+
 int exx_apply_host(exx_ctx* c, const double* psi_host, const double* occ_host, double* out_host, double* ex_host_or_null) {
     if (!c || !psi_host || !occ_host || !out_host) return EXX_ERR_NULL;
     int rc = check_occ(c, occ_host);

@@ -183,7 +183,7 @@ int launch_codensity_tile(exx_ctx* c, const double2* un_base, int n0, int tn, co
 int launch_kmul(exx_ctx* c, const double* ktab, double2* work, int nboxes);
 int launch_accumulate_tile(exx_ctx* c, const double2* uq_base, const MTile& mt, int tn, const double2* work, double2* acc);
 int launch_energy(exx_ctx* c, const double2* psi, const double2* vx);
-int launch_subspace(exx_ctx* c, int ik, const double2* psi, const double2* vx, double2* M);  // exx_subspace.cu
+int launch_subspace(exx_ctx* c, int ik, const double2* psi, const double2* vx, double2* M, int nvec = -1);  // exx_subspace.cu
 int compute_u_cache(exx_ctx* c, const double2* psi);  // exx_api.cu: S1 for every band
 
 // ---- fused path (exx_fused.cu) ----

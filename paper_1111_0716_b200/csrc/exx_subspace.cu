@@ -62,8 +62,10 @@ __global__ void subspace_reduce_kernel(const double2* __restrict__ partial, int 
     M[e] = s;
 }
 
-int launch_subspace(exx_ctx* c, int ik, const double2* psi, const double2* vx, double2* M) {
-    const int nb = c->nb, npw = c->npw[ik];
+// nvec vectors per k-point in psi / vx (default: the context's nbands), M is nvec x nvec
+int launch_subspace(exx_ctx* c, int ik, const double2* psi, const double2* vx, double2* M, int nvec) {
+    const int nb = nvec > 0 ? nvec : c->nb, npw = c->npw[ik];
+    const int64_t offk = c->off[ik] / c->nb * nb;
     const int tiles = (nb + 7) / 8;
     // slices: enough warps to fill the machine, chunks a multiple of 4 plane waves
     int nslices = std::max(1, std::min(64, (148 * 16 * 4) / std::max(1, tiles * tiles)));
@@ -84,7 +86,7 @@ int launch_subspace(exx_ctx* c, int ik, const double2* psi, const double2* vx, d
     {
         LaunchScope ls(c, KC_SUBSPACE, 1);
         dim3 grid((tiles * tiles + 3) / 4, nslices);
-        subspace_partial_kernel<<<grid, 128, 0, c->stream>>>(psi + c->off[ik], vx + c->off[ik], nb, npw, chunk, (double2*)c->subspace_dev);
+        subspace_partial_kernel<<<grid, 128, 0, c->stream>>>(psi + offk, vx + offk, nb, npw, chunk, (double2*)c->subspace_dev);
     }
     {
         LaunchScope ls(c, KC_SUBSPACE, 0);

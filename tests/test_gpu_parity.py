@@ -937,6 +937,17 @@ def test_apply_to_fused_kpoints_ragged_tiles(B):
                 sl = slice(pos, pos + o.npw[k])
                 pos += o.npw[k]
                 assert _rel(got_b[sl], want_b[sl]) < TOL_VX, (nphi, tile, path, k, i)
+        # the projected operator <phi_i|V_x phi_j> of the block (exx_subspace_block, DMMA) against numpy on the oracle's vectors
+        vd = g.to_device(want_b)
+        pos = 0
+        for k in range(w.nk):
+            P = blk[pos:pos + nphi * o.npw[k]].reshape(nphi, o.npw[k])
+            V = want_b[pos:pos + nphi * o.npw[k]].reshape(nphi, o.npw[k])
+            pos += nphi * o.npw[k]
+            M = g.subspace_block(k, g.to_device(blk), vd).cpu().numpy()
+            Mw = P.conj() @ V.T
+            assert np.abs(M - Mw).max() <= 1e-13 * np.abs(Mw).max(), (nphi, k)
+            assert np.abs(Mw - Mw.conj().T).max() <= 1e-12 * np.abs(Mw).max()
     g.set_option(B.EXX_OPT_PATH, 0)
     # EXX_OPT_KEEP_U: psi unchanged between calls -> S1 of psi skipped, same bits; a changed psi with the option off is picked up
     g.set_option(B.EXX_OPT_TILE_N, 0)

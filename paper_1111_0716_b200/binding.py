@@ -50,14 +50,17 @@ def lib():
     global _lib
     if _lib is None:
         if not os.environ.get("EXX_LIB"):
-            # compile (or re-compile after a source change) the CUDA library in-tree; compiling is not a fallback path:
-            # if nvcc or the sources are missing this raises, and nothing else can compute
+            # compile (or re-compile after a source change) the CUDA library in-tree; compiling is not a fallback path.  A build
+            # error is re-raised even when an older libexx.so is still on disk: only a library whose source stamp matches the
+            # sources is ever loaded, so tests and bench.py cannot report numbers for code that was never built.
+            from . import build as _build
             try:
-                from . import build as _build
                 _build.build()
             except Exception as e:  # noqa: BLE001
-                if not os.path.exists(LIB_PATH):
-                    raise RuntimeError("libexx.so is missing and could not be built (%s); there is no CPU fallback" % e)
+                raise RuntimeError("libexx.so could not be built from the current sources (%s); refusing to load a stale "
+                                   "library (set EXX_LIB to load a specific build); there is no CPU fallback" % e) from e
+            if _build.needs_build():
+                raise RuntimeError("libexx.so does not match the sources after the build step; there is no CPU fallback")
         if not os.path.exists(LIB_PATH):
             raise RuntimeError("libexx.so not found at %s: build it with `python -m paper_1111_0716_b200.build` "
                                "(there is no CPU fallback)" % LIB_PATH)

@@ -46,7 +46,9 @@ def needs_build():
 
 
 def build(force=False, verbose=False, extra=(), out=None):
-    """Build libexx.so (or `out`, e.g. a tuning variant compiled with extra -D flags)."""
+    """Build libexx.so (or `out`, e.g. a variant compiled with extra flags; such a variant never replaces libexx.so itself)."""
+    if extra and out is None and any(not str(x).startswith("-Xptxas") and str(x) != "-v" for x in extra):
+        raise ValueError("build(extra=...) needs out=...: libexx.so is only ever built with the stamped flags")
     if out is None and not force and not needs_build():
         return LIB
     target = out or LIB
@@ -57,7 +59,7 @@ def build(force=False, verbose=False, extra=(), out=None):
     digest = _source_hash()
     subprocess.check_call(cmd)
     os.replace(tmp, target)
-    if out is None and not extra:
+    if out is None:   # extra can only be ptxas verbosity here (checked above): same code
         with open(STAMP + ".tmp.%d" % os.getpid(), "w") as f:
             f.write(digest + "\n")
         os.replace(STAMP + ".tmp.%d" % os.getpid(), STAMP)

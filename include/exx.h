@@ -89,6 +89,11 @@ enum {
                                skipped (fused path; the generic kernels ignore it).  For an eigensolver that calls exx_apply_to on many
                                blocks of trial vectors between two updates of the orbitals.  0 (default): S1 of psi in every call.
                                Set it back to 0 for the first call after psi changes */
+    EXX_OPT_DUAL_SWEEP = 13, /* pair symmetry only.  1 (default): the last pass transforms every pair box back ONCE and feeds both
+                               accumulations (acc_a -= w_q f_b u_b v on chip, acc_b -= w_k f_a u_a conj(v) through one partial box per
+                               (row group, column) that a small reduction kernel adds in a fixed order); 0: two sweeps of the last
+                               pass, the second repeating the inverse y/z steps (grids without a dual kernel always do this).
+                               Results differ by rounding order only; both are deterministic */
     EXX_OPT_ENERGY_ROUTE = 11 /* what exx_energy does when it is given no V_x psi.  0 (default): the pair-density route
                                E_x = -1/2 sum w_k w_q f_nk f_mq sum_g K'_{k-q}(g) |rho^_{nk,mq}(g)|^2 (form (E2) of DESIGN.md section 2:
                                Eq. 2 of PAPER.md, L127-130, written in reciprocal space) wherever the fused kernels run: the co-density

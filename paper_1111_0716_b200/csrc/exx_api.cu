@@ -48,7 +48,8 @@ LaunchScope::~LaunchScope() {
 }
 
 static const char* kclass_names[KC_COUNT] = {"scatter", "gather", "fft_axis_generic", "codensity", "kernel_multiply",
-                                             "accumulate", "energy", "fused_pass_a", "fused_pass_b", "fused_pass_c", "subspace_zgemm", "fused_fft_pass"};
+                                             "accumulate", "energy", "fused_pass_a", "fused_pass_b", "fused_pass_c", "subspace_zgemm", "fused_fft_pass",
+                                             "fused_pass_r"};
 
 // ---- host arithmetic of S0 (index maps, kernel tables).  Evaluation order of |t.B|^2 is fixed (A11). ----
 static inline int fold(int j, int n) { return (2 * j < n) ? j : j - n; }
@@ -487,6 +488,9 @@ int exx_set_option(exx_ctx* c, int option, int64_t value) {
     case EXX_OPT_KEEP_U:
         c->opt_keep_u = value ? 1 : 0;
         return EXX_OK;
+    case EXX_OPT_DUAL_SWEEP:
+        c->opt_dual = value ? 1 : 0;
+        return EXX_OK;
     default: return EXX_ERR_BAD_ARG;
     }
 }
@@ -504,6 +508,7 @@ int exx_get_option(const exx_ctx* c, int option, int64_t* value) {
     case EXX_OPT_SHARD_RANK: *value = c->opt_shard_rank; return EXX_OK;
     case EXX_OPT_ENERGY_ROUTE: *value = c->opt_energy_route; return EXX_OK;
     case EXX_OPT_KEEP_U: *value = c->opt_keep_u; return EXX_OK;
+    case EXX_OPT_DUAL_SWEEP: *value = c->opt_dual; return EXX_OK;
     default: return EXX_ERR_BAD_ARG;
     }
 }
@@ -669,6 +674,7 @@ static void options_to_inner(const exx_ctx* c, exx_ctx* in) {
     in->opt_symmetry = c->opt_symmetry;
     in->opt_precision = c->opt_precision;
     in->opt_keep_u = c->opt_keep_u;
+    in->opt_dual = c->opt_dual;
     in->opt_shard_count = c->opt_shard_count;
     in->opt_shard_rank = c->opt_shard_rank;
 }

@@ -37,6 +37,9 @@ struct FusedState {
     // exx_apply_to: real-space boxes of the trial vectors phi (allocated on first use, nk*nb boxes like the u cache)
     cplx* uphi_dev = nullptr;
     size_t uphi_boxes = 0;
+    // dual sweep of pass C (pair symmetry): partial boxes of the second side, one per (row group, column) of a batch
+    cplx* part_dev = nullptr;
+    size_t part_boxes = 0;
 };
 
 #define EXX_DISPATCH_R1(R1v, EXPR)                  \
@@ -117,6 +120,18 @@ int fused_create(exx_ctx* c) {
         }
         c->dev_bytes += sizeof(double) * (TMAX * TMAX * (tiles2 + 1) + (size_t)c->nk * c->nb);
     }
+    int rg = 0;
+    EXX_DISPATCH_R1(st->R1, rg = L::RG);
+    if (rg > 0 && c->alias_free) {  // the pair symmetry (and with it the dual sweep) only ever runs on alias-free grids
+        int tn, tm;
+        fused_tiles(c, &tn, &tm);
+        st->part_boxes = (size_t)((tn + rg - 1) / rg) * tm;
+        if (cudaMalloc((void**)&st->part_dev, sizeof(cplx) * Ng * st->part_boxes) != cudaSuccess) {
+            cudaGetLastError();
+            return EXX_ERR_ALLOC;
+        }
+        c->dev_bytes += sizeof(cplx) * Ng * st->part_boxes;
+    }
     int rc = EXX_OK;
     EXX_DISPATCH_R1(st->R1, rc = L::init(c));
     return rc;
@@ -133,6 +148,7 @@ void fused_destroy(exx_ctx* c) {
     cudaFree(st->pairsum_dev);
     cudaFree(st->band_e2_dev);
     cudaFree(st->uphi_dev);
+    cudaFree(st->part_dev);
     delete st;
     c->fused = nullptr;
 }
@@ -266,6 +282,55 @@ static int pair_loop(exx_ctx* c, FusedState* st, const double* occ, const typena
         EXX_DISPATCH_M(st->R1, rc = L::pass_ab(c, ua, ub, aj, kperm, work));
         if (rc) return rc;
         c->pairs_executed += aj.npairs;
+        int dual_rg = 0;
+        EXX_DISPATCH_M(st->R1, dual_rg = L::RG);
+        if (sym && dual_rg > 0 && c->opt_dual && st->part_dev && (size_t)((ta + dual_rg - 1) / dual_rg) * tb <= st->part_boxes) {
+            // dual sweep: every pair box is transformed back ONCE; side a accumulates on chip per row, side b goes
+            // through one partial box per (row group, column), added to the b-bands' accumulators by pass R in row-group order
+            DJob dj;
+            RJob rj;
+            dj.ta = ta, dj.tb = tb, dj.nrg = (ta + dual_rg - 1) / dual_rg, dj.amask = 0u;
+            rj.ncol = tb, rj.tb = tb, rj.nrg = dj.nrg;
+            int64_t units_a = 0, units_b = 0, boxes = 0, parts = 0;
+            for (int j = 0; j < tb; j++) {
+                dj.b_src[j] = aj.b_idx[j];
+                dj.coef_b[j] = c->kw[q] * occ[q * nb + aj.b_idx[j]];
+                if (occ[q * nb + aj.b_idx[j]] != 0.0) dj.amask |= 1u << j;
+                rj.tgt[j] = q * nb + aj.b_idx[j];
+                rj.gmask[j] = 0u;
+            }
+            for (int i = 0; i < ta; i++) {
+                const double fa = occ[k * nb + aj.a_idx[i]];
+                dj.a_tgt[i] = k * na + aj.a_idx[i];
+                dj.a_src[i] = aj.a_idx[i];
+                dj.coef_a[i] = c->kw[k] * fa;
+                dj.ev[i] = dj.bside[i] = 0u;
+                for (int j = 0; j < tb; j++) {
+                    if (!ev[i][j]) continue;
+                    const bool sa = (dj.amask >> j & 1u) != 0, sb = fa != 0.0 && !(k == q && aj.a_idx[i] == aj.b_idx[j]);
+                    if (!sa && !sb) continue;
+                    dj.ev[i] |= 1u << j;
+                    boxes++;
+                    if (sa) units_a++;
+                    if (sb) {
+                        dj.bside[i] |= 1u << j, units_b++;
+                        if (!(rj.gmask[j] >> (i / dual_rg) & 1u)) rj.gmask[j] |= 1u << (i / dual_rg), parts++;
+                    }
+                }
+            }
+            for (int i = ta; i < TMAX; i++) dj.ev[i] = dj.bside[i] = 0u, dj.a_tgt[i] = dj.a_src[i] = 0, dj.coef_a[i] = 0.0;
+            for (int j = tb; j < TMAX; j++) dj.b_src[j] = 0, dj.coef_b[j] = 0.0, rj.tgt[j] = 0, rj.gmask[j] = 0u;
+            if (boxes) {
+                EXX_DISPATCH_M(st->R1, rc = L::pass_c_dual(c, ua, ub, dj, boxes, work, acc, (typename M::cplx*)st->part_dev));
+                if (rc) return rc;
+            }
+            if (parts) {
+                EXX_DISPATCH_M(st->R1, rc = L::pass_r(c, rj, parts, (const typename M::cplx*)st->part_dev, acc));
+                if (rc) return rc;
+            }
+            c->pairs_ordered += units_a + units_b;
+            continue;
+        }
         // side a: rows = a-bands, columns = b-bands with f_b != 0
         {
             CJob cj;

@@ -7,6 +7,9 @@ namespace EXX_NS {
 #ifdef EXX_SECOND_MODE  // names of exx_internal.h that the first mode (namespace exx) sees directly
 using ::exx::AJob;
 using ::exx::CJob;
+using ::exx::DJob;
+using ::exx::RJob;
+using ::exx::KC_PASS_R;
 using ::exx::LaunchScope;
 using ::exx::KC_PASS_A;
 using ::exx::KC_PASS_B;
@@ -285,6 +288,122 @@ __global__ void __launch_bounds__(FusedCfg<R1>::NT3, FusedCfg<R1>::MINB3) pass_c
     }
 }
 
+
+// ---- dual sweep (pair symmetry): one inverse transform per pair, both accumulations ----------------------------------------
+// CTA = (tile, row group): RG warp groups of NT3 threads, group wg owns row g*RG + wg of the batch: its tile S, its staging
+// slots G (next column's work-box elements), its slots UA ((-w_k f_a) u_a of the row, loaded once) and its register accumulators.
+// The column's u_b elements are staged once per CTA (G2).  Per column: [y step] group barrier [8-point z step] CTA barrier
+// [last z step; side a into registers; side b = P written over the thread's own elements of S] CTA barrier [P tiles of the groups
+// added in group order -> partial box (row group, column)] CTA barrier.  Every sum has a fixed order: deterministic.
+__device__ __forceinline__ void group_barrier(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
+
+template <int R1>
+struct DualGeo {
+    static constexpr int N = 8 * R1, U = FusedCfg<R1>::U3, NT = FusedCfg<R1>::NT3, RG = FusedCfg<R1>::RG > 0 ? FusedCfg<R1>::RG : 1;
+    static constexpr int TILE = U * R1 * N;
+    static constexpr int ITS = (U * N + NT - 1) / NT, ITU = (U * R1 * 8 + NT - 1) / NT;
+    static constexpr int GS = ITS * R1 * NT, US = ITU * R1 * NT;  // slots per group: work-box elements, u elements
+    static constexpr size_t smem = sizeof(cplx) * ((size_t)RG * (TILE + GS + US) + US + R1 * 8);
+};
+
+template <int R1>
+__global__ void __launch_bounds__(DualGeo<R1>::RG * DualGeo<R1>::NT, 1) pass_c_dual_kernel(const cplx* __restrict__ work, const cplx* __restrict__ ua_base,
+                                                                                        const cplx* __restrict__ ub_base, DJob job,
+                                                                                        acc_c* __restrict__ acc_base, cplx* __restrict__ part_base) {
+    typedef DualGeo<R1> D;
+    constexpr int N = D::N, U = D::U, NT = D::NT, RG = D::RG, TILE = D::TILE, GS = D::GS, US = D::US, ITU = D::ITU;
+    constexpr size_t Ng = (size_t)N * N * N;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    cplx* S0 = reinterpret_cast<cplx*>(smem_raw);
+    cplx* G0 = S0 + RG * TILE;
+    cplx* UA0 = G0 + RG * GS;
+    cplx* G2 = UA0 + RG * US;
+    cplx* T = G2 + US;
+    const int tid_cta = threadIdx.x;
+    const int wg = tid_cta / NT, tid = tid_cta - wg * NT;
+    cplx* S = S0 + wg * TILE;
+    cplx* G = G0 + wg * GS;
+    cplx* UA = UA0 + wg * US;
+    const unsigned bid = blockIdx.x;
+    const int g = bid % job.nrg;
+    const int tile = bid / job.nrg;
+    const int x = tile / (8 / U), yb = tile % (8 / U);
+    const int row = g * RG + wg;
+    const bool rowok = row < job.ta;
+    const unsigned ev = rowok ? job.ev[row] : 0u, bs = rowok ? job.bside[row] : 0u;
+    unsigned cta_ev = 0u;
+#pragma unroll
+    for (int w = 0; w < RG; w++)
+        if (g * RG + w < job.ta) cta_ev |= job.ev[g * RG + w];
+    for (int i = tid_cta; i < R1 * 8; i += RG * NT) T[tidx(i >> 3, i & 7)] = c_tw[TwOff<R1>::v + (i >> 3) * (i & 7)];
+    cplx twr[8];  // (TWREG is not used by the dual sweep)
+    acc_c accr[ITU * R1];
+#pragma unroll
+    for (int i = 0; i < ITU * R1; i++) accr[i] = mka(0.0, 0.0);
+    const size_t rowbox = (size_t)row * job.tb;
+    if (bs) p3_stage_u<R1, U, NT>(tid, ua_base + (size_t)job.a_src[rowok ? row : 0] * Ng, x, yb, UA);
+    stage_commit();
+    unsigned rem = cta_ev;
+    if (rem) {
+        const int c0 = __ffs(rem) - 1;
+        if (ev >> c0 & 1u) p3_stage<R1, U, NT>(tid, work + (rowbox + c0) * Ng, x, yb, G);
+    }
+    stage_commit();
+    stage_wait<1>();  // the row's u_a elements have landed (the first column's work-box elements may still be in flight)
+    if (bs) p3_scale_slots<R1, U, NT>(tid, UA, (real)(-job.coef_a[row]));
+    __syncthreads();  // twiddle table
+    while (rem) {
+        const int c = __ffs(rem) - 1;
+        rem &= rem - 1;
+        const bool act = ev >> c & 1u;
+        const bool col_a = job.amask >> c & 1u;
+        stage_wait<0>();
+        if (act) p3_y2inv_staged<R1, U, NT>(tid, G, S);
+        if (col_a) p3_stage_u_share<R1, U, NT, RG>(wg, tid, ub_base + (size_t)job.b_src[c] * Ng, x, yb, G2);
+        stage_commit();  // group 1: this thread's share of the column's u_b elements
+        if (rem) {
+            const int cn = __ffs(rem) - 1;
+            if (ev >> cn & 1u) p3_stage<R1, U, NT>(tid, work + (rowbox + cn) * Ng, x, yb, G);
+        }
+        stage_commit();  // group 2 (possibly empty): the next column's work-box elements
+        group_barrier(1 + wg, NT);
+        if (act) p13_z8<R1, U, NT, +1, false>(tid, S, T, twr);
+        stage_wait<1>();
+        __syncthreads();  // S of the group is complete; every thread's share of u_b has landed
+        if (act) p3_zinv2_dual<R1, U, NT>(tid, S, G2, UA, job.coef_b[c], col_a, bs >> c & 1u, accr);
+        unsigned gm = 0u;
+#pragma unroll
+        for (int w = 0; w < RG; w++)
+            if (g * RG + w < job.ta && (job.bside[g * RG + w] >> c & 1u)) gm |= 1u << w;
+        if (gm) {
+            __syncthreads();
+            p3_reduce_b<R1, U, NT, RG>(wg, tid, S0, TILE, gm, part_base + ((size_t)g * job.tb + c) * Ng, x, yb);
+        }
+        __syncthreads();  // S and G2 are free for the next column
+    }
+    if (ev & job.amask) p3_flush_reg<R1, U, NT>(tid, accr, acc_base + (size_t)job.a_tgt[row] * Ng, x, yb);
+}
+
+// pass R: acc[tgt[col]] += sum_g partial[g*tb + col] over the row groups that wrote one, in group order (fixed: deterministic)
+template <int DUMMY>
+__global__ void __launch_bounds__(256) pass_r_kernel(const cplx* __restrict__ part, RJob job, acc_c* __restrict__ acc_base, size_t Ng) {
+    const int col = blockIdx.y;
+    const unsigned gm = job.gmask[col];
+    if (!gm) return;
+    acc_c* acc = acc_base + (size_t)job.tgt[col] * Ng;
+    for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < Ng; p += (size_t)gridDim.x * blockDim.x) {
+        double sx = 0.0, sy = 0.0;
+        for (int g = 0; g < job.nrg; g++)
+            if (gm >> g & 1u) {
+                cplx v = part[((size_t)g * job.tb + col) * Ng + p];
+                sx += (double)v.x;
+                sy += (double)v.y;
+            }
+        acc_c a = acc[p];
+        acc[p] = mka(a.x + sx, a.y + sy);
+    }
+}
+
 // ---- plain 3-D transforms through the same passes (S1, S7; F layout, see exx_fused_phases.h) ------------------------
 // forward first half: natural box p of in_base -> work box p (z transform, first y step)
 template <int R1>
@@ -384,7 +503,11 @@ struct Launch {
     static constexpr size_t smem_c3 = smem_c + sizeof(cplx) * (size_t)((STAGE3 ? IT3S : 0) + (STAGEU ? IT3U : 0)) * R1 * FusedCfg<R1>::NT3;  // pass_c_kernel
     static constexpr size_t smem_b = sizeof(cplx) * ((size_t)N * P2Geo<Z>::PX);
 
+    static constexpr int RG = FusedCfg<R1>::RG;  // dual sweep: rows per CTA (0: not built for this grid)
+    static constexpr size_t smem_d = DualGeo<R1>::smem;
+
     static int init(exx_ctx* c) {
+        if (RG > 0) EXX_CUDA(c, cudaFuncSetAttribute(pass_c_dual_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_d));
         EXX_CUDA(c, cudaFuncSetAttribute(pass_a_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_a));
         EXX_CUDA(c, cudaFuncSetAttribute(pass_b_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_b));
         EXX_CUDA(c, cudaFuncSetAttribute(pass_c_kernel<R1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_c3));
@@ -464,6 +587,22 @@ struct Launch {
             int j = nat[i];
             out[i] = (int32_t)findex<R1>(j / (N * N), (j / N) % N, j % N);
         }
+    }
+    // the dual sweep (pair symmetry) and the reduction of its partial boxes
+    static int pass_c_dual(exx_ctx* c, const cplx* ua_base, const cplx* ub_base, const DJob& job, int64_t units, const cplx* work, acc_c* acc_base,
+                           cplx* part) {
+        const unsigned tiles3 = N * (8 / U3);
+        LaunchScope ls(c, KC_PASS_C, units);
+        pass_c_dual_kernel<R1><<<tiles3 * job.nrg, DualGeo<R1>::RG * FusedCfg<R1>::NT3, smem_d, c->stream>>>(work, ua_base, ub_base, job, acc_base, part);
+        EXX_CUDA(c, cudaGetLastError());
+        return EXX_OK;
+    }
+    static int pass_r(exx_ctx* c, const RJob& job, int64_t units, const cplx* part, acc_c* acc_base) {
+        LaunchScope ls(c, KC_PASS_R, units);
+        const size_t Ng = (size_t)N * N * N;
+        pass_r_kernel<0><<<dim3((unsigned)((Ng + 511) / 512), job.ncol), 256, 0, c->stream>>>(part, job, acc_base, Ng);
+        EXX_CUDA(c, cudaGetLastError());
+        return EXX_OK;
     }
     // one accumulation sweep (pass C)
     static int pass_c(exx_ctx* c, const cplx* usrc_base, const CJob& job, int64_t units, const cplx* work, acc_c* acc_base) {

@@ -69,6 +69,13 @@ constexpr int s3(int dflt) {
     return dflt;
 #endif
 }
+constexpr int rg(int dflt) {
+#ifdef EXX_DUAL_RG_ALL  // tuning builds: one value for every grid (0 switches the dual sweep off)
+    return EXX_DUAL_RG_ALL;
+#else
+    return dflt;
+#endif
+}
 template <int R1>
 struct FusedCfgBase;
 template <>
@@ -77,6 +84,7 @@ struct FusedCfgBase<2> {
     static constexpr bool TWREG = false, ACCREG = false;
     static constexpr int STAGE3 = s3(0);
     static constexpr int MINB1 = 1, MINB2 = 1, MINB3 = 1;
+    static constexpr int RG = rg(4);  // warp groups (rows) per CTA of the dual sweep; 0: two single sweeps instead
 };
 template <>
 struct FusedCfgBase<4> {
@@ -84,6 +92,7 @@ struct FusedCfgBase<4> {
     static constexpr bool TWREG = false, ACCREG = false;
     static constexpr int STAGE3 = s3(2);
     static constexpr int MINB1 = 1, MINB2 = 6, MINB3 = 1;
+    static constexpr int RG = rg(4);  // warp groups (rows) per CTA of the dual sweep; 0: two single sweeps instead
 };
 template <>
 struct FusedCfgBase<5> {
@@ -91,6 +100,7 @@ struct FusedCfgBase<5> {
     static constexpr bool TWREG = false, ACCREG = true;
     static constexpr int STAGE3 = s3(2);
     static constexpr int MINB1 = 1, MINB2 = 6, MINB3 = 1;
+    static constexpr int RG = rg(2);  // warp groups (rows) per CTA of the dual sweep; 0: two single sweeps instead
 };
 template <>
 struct FusedCfgBase<10> {
@@ -98,6 +108,7 @@ struct FusedCfgBase<10> {
     static constexpr bool TWREG = false, ACCREG = false;
     static constexpr int STAGE3 = s3(1);
     static constexpr int MINB1 = 1, MINB2 = 4, MINB3 = 1;
+    static constexpr int RG = rg(2);  // warp groups (rows) per CTA of the dual sweep; 0: two single sweeps instead
 };
 template <>
 struct FusedCfgBase<6> {
@@ -105,6 +116,7 @@ struct FusedCfgBase<6> {
     static constexpr bool TWREG = false, ACCREG = false;
     static constexpr int STAGE3 = s3(2);
     static constexpr int MINB1 = 1, MINB2 = 6, MINB3 = 1;  // min CTAs per SM asked of the compiler (register cap)
+    static constexpr int RG = rg(4);  // warp groups (rows) per CTA of the dual sweep; 0: two single sweeps instead
 };
 template <>
 struct FusedCfgBase<8> {
@@ -112,6 +124,7 @@ struct FusedCfgBase<8> {
     static constexpr bool TWREG = false, ACCREG = true;
     static constexpr int STAGE3 = s3(2);
     static constexpr int MINB1 = 1, MINB2 = 6, MINB3 = 1;
+    static constexpr int RG = rg(2);  // warp groups (rows) per CTA of the dual sweep; 0: two single sweeps instead
 };
 template <>
 struct FusedCfgBase<9> {
@@ -119,6 +132,7 @@ struct FusedCfgBase<9> {
     static constexpr bool TWREG = false, ACCREG = true;
     static constexpr int STAGE3 = s3(2);
     static constexpr int MINB1 = 1, MINB2 = 5, MINB3 = 1;
+    static constexpr int RG = rg(4);  // warp groups (rows) per CTA of the dual sweep; 0: two single sweeps instead
 };
 template <>
 struct FusedCfgBase<12> {
@@ -126,6 +140,7 @@ struct FusedCfgBase<12> {
     static constexpr bool TWREG = false, ACCREG = false;
     static constexpr int STAGE3 = s3(1);
     static constexpr int MINB1 = 1, MINB2 = 4, MINB3 = 1;
+    static constexpr int RG = rg(2);  // warp groups (rows) per CTA of the dual sweep; 0: two single sweeps instead
 };
 template <>
 struct FusedCfgBase<16> {
@@ -133,6 +148,7 @@ struct FusedCfgBase<16> {
     static constexpr bool TWREG = false, ACCREG = false;
     static constexpr int STAGE3 = s3(1);
     static constexpr int MINB1 = 1, MINB2 = 2, MINB3 = 1;
+    static constexpr int RG = rg(0);  // warp groups (rows) per CTA of the dual sweep; 0: two single sweeps instead
 };
 template <int R1>
 struct FusedCfg : FusedCfgBase<R1> {};
@@ -178,6 +194,7 @@ struct FusedCfg<EXX_TUNE_R1> {
     static constexpr bool TWREG = EXX_TUNE_TWREG, ACCREG = EXX_TUNE_ACCREG;
     static constexpr int STAGE3 = EXX_TUNE_STAGE3;
     static constexpr int MINB1 = EXX_TUNE_MINB1, MINB2 = EXX_TUNE_MINB2, MINB3 = EXX_TUNE_MINB3;
+    static constexpr int RG = FusedCfgBase<EXX_TUNE_R1>::RG;
 };
 #endif
 
@@ -640,6 +657,98 @@ EXX_HD void p3_flush_reg(int tid, const acc_c* acc, acc_c* __restrict__ accg, in
             size_t base = ((size_t)x * N + (n1y * 8 + yb * U + u)) * N + n2z;
 #pragma unroll
             for (int j = 0; j < R1; j++) accg[base + j * 8] = mka(accg[base + j * 8].x + acc[i * R1 + j].x, accg[base + j * 8].y + acc[i * R1 + j].y);
+        }
+    }
+}
+
+// ---- dual sweep (pair symmetry): ONE inverse transform of a pair's box feeds both accumulations --------------------------
+// A CTA of RG warp groups (NT threads each) owns RG rows (a-bands) of the batch for one tile and walks the columns (b-bands) in
+// lockstep.  Group wg transforms box (row, column) in its own tile S and, in the last step, adds
+//     side a:  acc_a -= (w_q f_b) u_b v                 into its register accumulators (flushed once after the loop), and writes
+//     side b:  P = (-w_k f_a) u_a conj(v)               over its own elements of S (each thread owns the elements it read),
+// UA holding (-w_k f_a) u_a of the group's row and UB the column's u_b, both in per-thread slots (element j of item tid + i NT at
+// slot (i R1 + j) NT + tid).  After a barrier p3_reduce_b adds the P tiles of the contributing groups in group order and stores
+// the sum to the column's partial box; pass_r_kernel later adds the partial boxes of a column, in row-group order, to acc_b.
+template <int R1, int U, int NT>
+EXX_HD void p3_zinv2_dual(int tid, cplx* S, const cplx* UB, const cplx* UA, double wfb, bool do_a, bool do_b, acc_c* acc) {
+    constexpr int NI = U * R1 * 8, IT = (NI + NT - 1) / NT;
+#pragma unroll
+    for (int i = 0; i < IT; i++) {
+        int it = tid + i * NT;
+        if (it < NI) {
+            int row = it >> 3, n2z = it & 7;
+            int u = row / R1, n1y = row - u * R1;
+            cplx v[R1];
+#pragma unroll
+            for (int j = 0; j < R1; j++) v[j] = S[sidx<R1>(u, n1y, j, n2z)];
+            dft<R1, +1>(v);
+            if (do_a) {
+#pragma unroll
+                for (int j = 0; j < R1; j++) {
+                    cplx p = UB[(i * R1 + j) * NT + tid] * v[j];
+                    acc[i * R1 + j] = mka(acc[i * R1 + j].x - wfb * p.x, acc[i * R1 + j].y - wfb * p.y);
+                }
+            }
+            if (do_b) {
+#pragma unroll
+                for (int j = 0; j < R1; j++) S[sidx<R1>(u, n1y, j, n2z)] = mul_conj_b(UA[(i * R1 + j) * NT + tid], v[j]);
+            }
+        }
+    }
+}
+
+// UA slots <- coef * u (this thread's elements of the group's row; the slots are private to the thread)
+template <int R1, int U, int NT>
+EXX_HD void p3_scale_slots(int tid, cplx* UA, real coef) {
+    constexpr int NI = U * R1 * 8, IT = (NI + NT - 1) / NT;
+#pragma unroll
+    for (int i = 0; i < IT; i++)
+        if (tid + i * NT < NI) {
+#pragma unroll
+            for (int j = 0; j < R1; j++) UA[(i * R1 + j) * NT + tid] = scale(coef, UA[(i * R1 + j) * NT + tid]);
+        }
+}
+
+// the column's u_b elements, staged ONCE per CTA: group wg copies the elements j = wg, wg + RG, ... of every item into the shared
+// slots, every group reads all of them after the next CTA barrier
+template <int R1, int U, int NT, int RG>
+EXX_HD void p3_stage_u_share(int wg, int tid, const cplx* __restrict__ um, int x, int yb, cplx* G2) {
+    constexpr int N = 8 * R1, NI = U * R1 * 8, IT = (NI + NT - 1) / NT;
+#pragma unroll
+    for (int i = 0; i < IT; i++) {
+        int it = tid + i * NT;
+        if (it < NI) {
+            int row = it >> 3, n2z = it & 7;
+            int u = row / R1, n1y = row - u * R1;
+            size_t base = ((size_t)x * N + (n1y * 8 + yb * U + u)) * N + n2z;
+#pragma unroll
+            for (int j = 0; j < R1; j++)
+                if (j % RG == wg) stage_elem(G2 + (i * R1 + j) * NT + tid, um + base + j * 8);
+        }
+    }
+}
+
+// partial box of (row group, column) <- sum over the contributing groups (bit g of gmask), in group order, of their P tiles;
+// thread (wg, tid) handles the elements j = wg, wg + RG, ... of its item.  tile_stride = elements between the groups' S tiles.
+template <int R1, int U, int NT, int RG>
+EXX_HD void p3_reduce_b(int wg, int tid, const cplx* S0, int tile_stride, unsigned gmask, cplx* __restrict__ part, int x, int yb) {
+    constexpr int N = 8 * R1, NI = U * R1 * 8, IT = (NI + NT - 1) / NT;
+#pragma unroll
+    for (int i = 0; i < IT; i++) {
+        int it = tid + i * NT;
+        if (it < NI) {
+            int row = it >> 3, n2z = it & 7;
+            int u = row / R1, n1y = row - u * R1;
+            size_t base = ((size_t)x * N + (n1y * 8 + yb * U + u)) * N + n2z;
+#pragma unroll
+            for (int j = 0; j < R1; j++)
+                if (j % RG == wg) {
+                    cplx s = mk(EXX_RC(0.0), EXX_RC(0.0));
+#pragma unroll
+                    for (int g = 0; g < RG; g++)
+                        if (gmask >> g & 1u) s = s + S0[g * tile_stride + sidx<R1>(u, n1y, j, n2z)];
+                    part[base + j * 8] = s;
+                }
         }
     }
 }

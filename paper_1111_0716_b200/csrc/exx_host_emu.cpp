@@ -93,6 +93,130 @@ static void emu_pair(const cplx* un, const cplx* um, const double* Knat, double 
         }
 }
 
+
+// passes A and B of one pair into its work box W (Kp: permuted table)
+template <int R1>
+static void emu_ab(const cplx* un, const cplx* um, const double* Kp, cplx* W) {
+    typedef FusedCfg<R1> C;
+    constexpr int N = 8 * R1, U = C::U1, NT13 = C::NT1, Z = C::Z, NT2 = C::NT2;
+    constexpr bool TWREG = C::TWREG;
+    std::vector<cplx> S((size_t)U * R1 * N), T(R1 * 8), S2((size_t)N * P2Geo<Z>::PX);
+    for (int k = 0; k < R1; k++)
+        for (int j = 0; j < 8; j++) T[tidx(k, j)] = EXX_TW(R1, j * k);
+    for (int x = 0; x < N; x++)
+        for (int yb = 0; yb < 8 / U; yb++) {
+            for (int t = 0; t < NT13; t++) p1_z1<R1, U, NT13>(t, un, um, x, yb, S.data());
+            for (int t = 0; t < NT13; t++) {
+                cplx twr[8];
+                load_twr<R1>(t, twr);
+                p13_z8<R1, U, NT13, -1, TWREG>(t, S.data(), T.data(), twr);
+            }
+            for (int t = 0; t < NT13; t++) p1_y1<R1, U, NT13>(t, S.data(), W, x, yb);
+        }
+    for (int k1y = 0; k1y < R1; k1y++)
+        for (int zb = 0; zb < N / Z; zb++) {
+            const double* Kt = Kp + ((size_t)k1y * (N / Z) + zb) * ((size_t)N * 8 * Z);
+            cplx* Wt = W + ((size_t)k1y * (N / Z) + zb) * ((size_t)N * 8 * Z);
+            p2_copy_rows<R1, Z>(S2.data(), Wt, true);
+            for (int t = 0; t < NT2; t++) p2_y8<R1, Z, NT2, -1>(t, S2.data(), k1y);
+            for (int t = 0; t < NT2; t++) p2_xR<R1, Z, NT2, -1>(t, S2.data());
+            for (int t = 0; t < NT2; t++) p2_x8<R1, Z, NT2>(t, S2.data(), Kt);
+            for (int t = 0; t < NT2; t++) p2_xR<R1, Z, NT2, +1>(t, S2.data());
+            for (int t = 0; t < NT2; t++) p2_y8<R1, Z, NT2, +1>(t, S2.data(), k1y);
+            p2_copy_rows<R1, Z>(S2.data(), Wt, false);
+        }
+}
+
+// The dual sweep of a ta x tb batch exactly as pass_c_dual_kernel + pass_r_kernel schedule it (RG warp groups per CTA, columns
+// in lockstep, side a in per-thread accumulators, side b through the P tiles and one partial box per (row group, column)).
+// ua: ta boxes, ub: tb boxes, ev/bside: per-row column masks, amask: columns with side a; acc_a: ta boxes, acc_b: tb boxes (+=).
+template <int R1>
+static void emu_dual(int ta, int tb, const cplx* ua, const cplx* ub, const double* Knat, const double* coef_a, const double* coef_b,
+                     const unsigned* ev, const unsigned* bside, unsigned amask, acc_c* acc_a, acc_c* acc_b) {
+    typedef FusedCfg<R1> C;
+    constexpr int N = 8 * R1, U = C::U3, NT = C::NT3, Z = C::Z, RG = C::RG > 0 ? C::RG : 1;
+    constexpr int TILE = U * R1 * N, ITS = (U * N + NT - 1) / NT, ITU = (U * R1 * 8 + NT - 1) / NT, GS = ITS * R1 * NT, US = ITU * R1 * NT;
+    const size_t Ng = (size_t)N * N * N;
+    std::vector<double> Kp(Ng);
+    permute_ktable(R1, Z, KVW, Knat, Kp.data());
+    std::vector<cplx> work((size_t)ta * tb * Ng);
+    for (int i = 0; i < ta; i++)
+        for (int j = 0; j < tb; j++)
+            if (ev[i] >> j & 1u) emu_ab<R1>(ua + i * Ng, ub + j * Ng, Kp.data(), work.data() + ((size_t)i * tb + j) * Ng);
+    const int nrg = (ta + RG - 1) / RG;
+    std::vector<cplx> part((size_t)nrg * tb * Ng);
+    std::vector<cplx> S((size_t)RG * TILE), G((size_t)RG * GS), UA((size_t)RG * US), G2(US), T(R1 * 8);
+    std::vector<acc_c> accr((size_t)RG * NT * ITU * R1);
+    for (int k = 0; k < R1; k++)
+        for (int j = 0; j < 8; j++) T[tidx(k, j)] = EXX_TW(R1, j * k);
+    for (int x = 0; x < N; x++)
+        for (int yb = 0; yb < 8 / U; yb++)
+            for (int g = 0; g < nrg; g++) {
+                unsigned cta_ev = 0;
+                for (int w = 0; w < RG; w++)
+                    if (g * RG + w < ta) cta_ev |= ev[g * RG + w];
+                for (auto& a : accr) a = mka(0.0, 0.0);
+                for (int w = 0; w < RG; w++) {
+                    const int row = g * RG + w;
+                    if (row >= ta || !bside[row]) continue;
+                    for (int t = 0; t < NT; t++) p3_stage_u<R1, U, NT>(t, ua + row * Ng, x, yb, UA.data() + w * US);
+                    for (int t = 0; t < NT; t++) p3_scale_slots<R1, U, NT>(t, UA.data() + w * US, -coef_a[row]);
+                }
+                for (int c = 0; c < tb; c++) {
+                    if (!(cta_ev >> c & 1u)) continue;
+                    const bool col_a = amask >> c & 1u;
+                    unsigned gm = 0;
+                    for (int w = 0; w < RG; w++) {
+                        const int row = g * RG + w;
+                        const bool act = row < ta && (ev[row] >> c & 1u);
+                        if (row < ta && (bside[row] >> c & 1u)) gm |= 1u << w;
+                        if (act) {
+                            const cplx* W = work.data() + ((size_t)row * tb + c) * Ng;
+                            for (int t = 0; t < NT; t++) p3_stage<R1, U, NT>(t, W, x, yb, G.data() + w * GS);
+                            for (int t = 0; t < NT; t++) p3_y2inv_staged<R1, U, NT>(t, G.data() + w * GS, S.data() + w * TILE);
+                        }
+                        if (col_a)
+                            for (int t = 0; t < NT; t++) p3_stage_u_share<R1, U, NT, RG>(w, t, ub + c * Ng, x, yb, G2.data());
+                    }
+                    for (int w = 0; w < RG; w++) {
+                        const int row = g * RG + w;
+                        if (!(row < ta && (ev[row] >> c & 1u))) continue;
+                        for (int t = 0; t < NT; t++) {
+                            cplx twr[8];
+                            p13_z8<R1, U, NT, +1, false>(t, S.data() + w * TILE, T.data(), twr);
+                        }
+                    }
+                    for (int w = 0; w < RG; w++) {
+                        const int row = g * RG + w;
+                        if (!(row < ta && (ev[row] >> c & 1u))) continue;
+                        for (int t = 0; t < NT; t++)
+                            p3_zinv2_dual<R1, U, NT>(t, S.data() + w * TILE, G2.data(), UA.data() + w * US, coef_b[c], col_a, bside[row] >> c & 1u,
+                                                     accr.data() + ((size_t)w * NT + t) * ITU * R1);
+                    }
+                    if (gm)
+                        for (int w = 0; w < RG; w++)
+                            for (int t = 0; t < NT; t++)
+                                p3_reduce_b<R1, U, NT, RG>(w, t, S.data(), TILE, gm, part.data() + ((size_t)g * tb + c) * Ng, x, yb);
+                }
+                for (int w = 0; w < RG; w++) {
+                    const int row = g * RG + w;
+                    if (row < ta && (ev[row] & amask))
+                        for (int t = 0; t < NT; t++) p3_flush_reg<R1, U, NT>(t, accr.data() + ((size_t)w * NT + t) * ITU * R1, acc_a + row * Ng, x, yb);
+                }
+            }
+    for (int c = 0; c < tb; c++)  // pass R
+        for (int g = 0; g < nrg; g++) {
+            bool any = false;
+            for (int w = 0; w < RG; w++)
+                if (g * RG + w < ta && (bside[g * RG + w] >> c & 1u)) any = true;
+            if (!any) continue;
+            for (size_t p = 0; p < Ng; p++) {
+                cplx v = part[((size_t)g * tb + c) * Ng + p];
+                acc_b[c * Ng + p] = mka(acc_b[c * Ng + p].x + v.x, acc_b[c * Ng + p].y + v.y);
+            }
+        }
+}
+
 // energy route of one pair (pass A, the forward half of pass B, the K' |rho^|^2 sum of p2_x8_energy), tile partials added up
 // in tile order as pair_sum_kernel would see them
 template <int R1>
@@ -225,6 +349,22 @@ int exx_emu_pair(int R1, const double* un, const double* um, const double* Knat,
     case 9: emu_pair<9>((const cplx*)un, (const cplx*)um, Knat, wf, (acc_c*)acc, (cplx*)work); return 0;
     case 12: emu_pair<12>((const cplx*)un, (const cplx*)um, Knat, wf, (acc_c*)acc, (cplx*)work); return 0;
     case 16: emu_pair<16>((const cplx*)un, (const cplx*)um, Knat, wf, (acc_c*)acc, (cplx*)work); return 0;
+    default: return -1;
+    }
+}
+
+// the dual sweep of a ta x tb batch (see emu_dual); returns -2 where the grid has no dual kernel (RG = 0)
+int exx_emu_dual(int R1, int ta, int tb, const double* ua, const double* ub, const double* Knat, const double* coef_a, const double* coef_b,
+                 const unsigned* ev, const unsigned* bside, unsigned amask, double* acc_a, double* acc_b) {
+    fill_tw();
+    switch (R1) {
+#define EXX_EMU_D(r)                                                                                                             \
+    case r:                                                                                                                      \
+        if (FusedCfg<r>::RG == 0) return -2;                                                                                     \
+        emu_dual<r>(ta, tb, (const cplx*)ua, (const cplx*)ub, Knat, coef_a, coef_b, ev, bside, amask, (acc_c*)acc_a, (acc_c*)acc_b); \
+        return 0;
+        EXX_EMU_D(2) EXX_EMU_D(4) EXX_EMU_D(5) EXX_EMU_D(10) EXX_EMU_D(6) EXX_EMU_D(8) EXX_EMU_D(9) EXX_EMU_D(12) EXX_EMU_D(16)
+#undef EXX_EMU_D
     default: return -1;
     }
 }

@@ -26,7 +26,8 @@ enum KClass {
     KC_PASS_C = 9,       // fused: inverse (y,z)-plane transform, times f_m u_m, accumulate
     KC_SUBSPACE = 10,    // subspace ZGEMM (DMMA) + its slice reduction
     KC_FFT_FUSED = 11,   // plain 3-D transforms (S1, S7) through the fused passes; unit = one box pass
-    KC_COUNT = 12
+    KC_PASS_R = 12,      // fused, pair symmetry: partial boxes of the dual sweep's second side added to the accumulators
+    KC_COUNT = 13
 };
 
 struct Plan1D {
@@ -104,6 +105,7 @@ struct exx_ctx {
     bool u_valid = false;          // the u cache holds S1 of the psi of the previous call (fused path)
     int64_t opt_energy_route = 0;  // 0 auto (pair-density route E2 where the fused path runs), 1 always E1 from V_x psi
     int64_t energy_route_used = 0;
+    int64_t opt_dual = 1;          // pair symmetry: 1 = one dual sweep of pass C per batch (default), 0 = two single sweeps
     int64_t opt_shard_count = 1, opt_shard_rank = 0;  // S8(f)-4: this context runs shard rank of count (exx_shard.h)
 
     // counters of the last apply
@@ -168,6 +170,23 @@ struct CJob {
     int tgt[TMAX], cnt[TMAX], src[TMAX];
     double coef[TMAX];
     unsigned char col[TMAX][TMAX];
+};
+// the dual sweep of pass C (pair symmetry): CTA (tile, row group) walks the columns; row i (a-band) x column j
+// (b-band), work box i*tb + j.  ev[i] bit j: the pair was transformed; side a (acc_a -= coef_b[j] u_b v) runs where amask has bit
+// j (f_b != 0); side b (acc_b -= coef_a[i] u_a conj v) where bside[i] has bit j (f_a != 0 and not the diagonal pair).
+struct DJob {
+    int ta, tb, nrg;
+    int a_tgt[TMAX];            // accumulator box of row i
+    int a_src[TMAX], b_src[TMAX];  // u boxes of row i / column j (within ua_base / ub_base)
+    double coef_a[TMAX], coef_b[TMAX];
+    unsigned ev[TMAX], bside[TMAX];
+    unsigned amask;
+};
+// pass R: acc[tgt[j]] += sum over the row groups g with bit g of gmask[j] of partial box g*tb + j, in group order
+struct RJob {
+    int ncol, tb, nrg;
+    int tgt[TMAX];
+    unsigned gmask[TMAX];
 };
 // weights of one batch on the energy route: band (a,k) gets  wa[i] * sum_j wb[j] S_ij,  band (b,q) (pair symmetry) the mirror image
 struct EJob {

@@ -34,8 +34,8 @@ def test_strerror_and_class_names(L):
     for code in range(0, -11, -1):
         assert L.exx_strerror(code)
     assert L.exx_strerror(-99) == b"unknown error"
-    names = [L.exx_kernel_class_name(k) for k in range(12)]
-    assert all(names) and L.exx_kernel_class_name(12) is None and L.exx_kernel_class_name(-1) is None
+    names = [L.exx_kernel_class_name(k) for k in range(13)]
+    assert all(names) and L.exx_kernel_class_name(13) is None and L.exx_kernel_class_name(-1) is None
 
 
 def test_create_rejects_bad_arguments_before_touching_the_gpu(L):

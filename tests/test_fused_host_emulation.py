@@ -24,6 +24,8 @@ def emu(tmp_path_factory):
     L.exx_emu_dft.argtypes = [C.c_int, C.c_int, dp]
     L.exx_emu_pair.argtypes = [C.c_int, dp, dp, dp, C.c_double, dp, dp]
     L.exx_emu_pair_energy.argtypes = [C.c_int, dp, dp, dp, dp, dp]
+    up = C.POINTER(C.c_uint32)
+    L.exx_emu_dual.argtypes = [C.c_int, C.c_int, C.c_int, dp, dp, dp, dp, dp, up, up, C.c_uint32, dp, dp]
     return L
 
 
@@ -118,3 +120,53 @@ def test_plain_transforms_through_the_passes(emu, R1):
     assert emu.exx_emu_fft(R1, +1, _p(f), _p(back), None) == 0
     want = np.fft.ifftn(y).reshape(-1) * N ** 3
     assert np.linalg.norm(back - want) <= 1e-14 * np.linalg.norm(want)
+
+
+@pytest.mark.parametrize("R1,ta,tb", [(2, 5, 3), (4, 6, 4), (5, 3, 3), (6, 5, 2), (9, 5, 2)])
+def test_dual_sweep_equals_definition(emu, R1, ta, tb):
+    """The dual sweep of pass C (pair symmetry) on a ragged ta x tb batch with holes: rows get
+    acc_a -= sum_j coef_b[j] u_b[j] v_ij, columns get acc_b -= sum_i coef_a[i] u_a[i] conj(v_ij), v_ij = IFFT[K FFT[conj(u_b[j]) u_a[i]]],
+    against numpy.fft.  Masks as the host builds them: a pair may be skipped altogether, feed one side only, or both."""
+    N = 8 * R1
+    rng = np.random.default_rng(7000 + R1)
+    shp = (N, N, N)
+    ua = rng.standard_normal((ta,) + shp) + 1j * rng.standard_normal((ta,) + shp)
+    ub = rng.standard_normal((tb,) + shp) + 1j * rng.standard_normal((tb,) + shp)
+    K = rng.random(shp)
+    coef_a, coef_b = rng.random(ta) + 0.1, rng.random(tb) + 0.1
+    coef_b[tb - 1] = 0.0                                   # an empty b-band: no side a for that column
+    coef_a[1] = 0.0                                        # an empty a-band: no side b for that row
+    ev = np.zeros(ta, dtype=np.uint32)
+    bside = np.zeros(ta, dtype=np.uint32)
+    amask = 0
+    for j in range(tb):
+        if coef_b[j] != 0.0:
+            amask |= 1 << j
+    for i in range(ta):
+        for j in range(tb):
+            if (i, j) == (2, 0):
+                continue                                   # a pair that is not evaluated at all
+            sa, sb = coef_b[j] != 0.0, coef_a[i] != 0.0 and (i, j) != (0, 1)   # (0, 1): a "diagonal" pair, side a only
+            if sa or sb:
+                ev[i] |= 1 << j
+            if sb:
+                bside[i] |= 1 << j
+    acc_a0 = rng.standard_normal((ta,) + shp) + 1j * rng.standard_normal((ta,) + shp)
+    acc_b0 = rng.standard_normal((tb,) + shp) + 1j * rng.standard_normal((tb,) + shp)
+    acc_a, acc_b = acc_a0.copy(), acc_b0.copy()
+    up = C.POINTER(C.c_uint32)
+    rc = emu.exx_emu_dual(R1, ta, tb, _p(ua), _p(ub), _p(K), _p(coef_a), _p(coef_b), ev.ctypes.data_as(up), bside.ctypes.data_as(up),
+                          amask, _p(acc_a), _p(acc_b))
+    assert rc == 0
+    want_a, want_b = np.zeros_like(acc_a), np.zeros_like(acc_b)
+    for i in range(ta):
+        for j in range(tb):
+            if not (ev[i] >> j) & 1:
+                continue
+            v = np.fft.ifftn(K * np.fft.fftn(np.conj(ub[j]) * ua[i])) * N ** 3
+            if (amask >> j) & 1:
+                want_a[i] -= coef_b[j] * ub[j] * v
+            if (bside[i] >> j) & 1:
+                want_b[j] -= coef_a[i] * ua[i] * np.conj(v)
+    assert np.linalg.norm(acc_a - acc_a0 - want_a) <= 1e-14 * np.linalg.norm(want_a)
+    assert np.linalg.norm(acc_b - acc_b0 - want_b) <= 1e-14 * np.linalg.norm(want_b)

@@ -231,7 +231,7 @@ __global__ void __launch_bounds__(FusedCfg<R1>::NT3, FusedCfg<R1>::MINB3) pass_c
     acc_c* A = reinterpret_cast<acc_c*>(S + U * R1 * N);  // fp64 accumulator tile; unused when ACCREG
     cplx* T = reinterpret_cast<cplx*>(A + (ACCREG ? 0 : U * R1 * N));
     cplx* G = T + (TWREG ? 0 : R1 * 8);  // STAGE3: per-thread slots for the next column's work-box elements
-    cplx* G2 = G + ((U * N + NT - 1) / NT) * R1 * NT;  // ... and for this column's u elements
+    cplx* G2 = G + Slots<R1, U, NT>::COUNT;  // ... and for this column's u elements
     const int tid = threadIdx.x;
     const unsigned bid = blockIdx.x;
     const int r = bid % job.nr;
@@ -290,20 +290,21 @@ __global__ void __launch_bounds__(FusedCfg<R1>::NT3, FusedCfg<R1>::MINB3) pass_c
 
 
 // ---- dual sweep (pair symmetry): one inverse transform per pair, both accumulations ----------------------------------------
-// CTA = (tile, row group): RG warp groups of NT3 threads, group wg owns row g*RG + wg of the batch: its tile S, its staging
-// slots G (next column's work-box elements), its slots UA ((-w_k f_a) u_a of the row, loaded once) and its register accumulators.
-// The column's u_b elements are staged once per CTA (G2).  Per column: [y step] group barrier [8-point z step] CTA barrier
-// [last z step; side a into registers; side b = P written over the thread's own elements of S] CTA barrier [P tiles of the groups
-// added in group order -> partial box (row group, column)] CTA barrier.  Every sum has a fixed order: deterministic.
+// CTA = (tile, row group): RG warp groups of NT3 threads, group wg owns row g*RG + wg of the batch: its two tiles S (columns
+// alternate between them), its staging slots G (next column's work-box elements), its slots UA ((-w_k f_a) u_a of the row, loaded
+// once) and its register accumulators.  The column's u_b elements are staged once per CTA, one column ahead, into G2[column parity].
+// Per column: [y step] group barrier [8-point z step] group barrier [last z step; side a into registers; side b = P written over
+// the thread's own elements of S] CTA barrier [P tiles of the groups added in group order -> partial box (row group, column)].
+// The one CTA barrier also hands over the next column's u_b slots; the reduction reads the tiles the next column does not write.
+// Every sum has a fixed order: deterministic.
 __device__ __forceinline__ void group_barrier(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
 
 template <int R1>
 struct DualGeo {
     static constexpr int N = 8 * R1, U = FusedCfg<R1>::U3, NT = FusedCfg<R1>::NT3, RG = FusedCfg<R1>::RG > 0 ? FusedCfg<R1>::RG : 1;
     static constexpr int TILE = U * R1 * N;
-    static constexpr int ITS = (U * N + NT - 1) / NT, ITU = (U * R1 * 8 + NT - 1) / NT;
-    static constexpr int GS = ITS * R1 * NT, US = ITU * R1 * NT;  // slots per group: work-box elements, u elements
-    static constexpr size_t smem = sizeof(cplx) * ((size_t)RG * (TILE + GS + US) + US + R1 * 8);
+    static constexpr int SL = Slots<R1, U, NT>::COUNT;  // slots of one step of one group
+    static constexpr size_t smem = sizeof(cplx) * ((size_t)RG * (2 * TILE + 2 * SL) + 2 * SL + R1 * 8);
 };
 
 template <int R1>
@@ -311,19 +312,19 @@ __global__ void __launch_bounds__(DualGeo<R1>::RG * DualGeo<R1>::NT, 1) pass_c_d
                                                                                         const cplx* __restrict__ ub_base, DJob job,
                                                                                         acc_c* __restrict__ acc_base, cplx* __restrict__ part_base) {
     typedef DualGeo<R1> D;
-    constexpr int N = D::N, U = D::U, NT = D::NT, RG = D::RG, TILE = D::TILE, GS = D::GS, US = D::US, ITU = D::ITU;
+    constexpr int N = D::N, U = D::U, NT = D::NT, RG = D::RG, TILE = D::TILE, SL = D::SL;
+    constexpr int ITU = (U * R1 * 8 + NT - 1) / NT;
     constexpr size_t Ng = (size_t)N * N * N;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    cplx* S0 = reinterpret_cast<cplx*>(smem_raw);
-    cplx* G0 = S0 + RG * TILE;
-    cplx* UA0 = G0 + RG * GS;
-    cplx* G2 = UA0 + RG * US;
-    cplx* T = G2 + US;
+    cplx* S0 = reinterpret_cast<cplx*>(smem_raw);  // [parity][group][TILE]
+    cplx* G0 = S0 + 2 * RG * TILE;
+    cplx* UA0 = G0 + RG * SL;
+    cplx* G2 = UA0 + RG * SL;  // [parity][SL]
+    cplx* T = G2 + 2 * SL;
     const int tid_cta = threadIdx.x;
     const int wg = tid_cta / NT, tid = tid_cta - wg * NT;
-    cplx* S = S0 + wg * TILE;
-    cplx* G = G0 + wg * GS;
-    cplx* UA = UA0 + wg * US;
+    cplx* G = G0 + wg * SL;
+    cplx* UA = UA0 + wg * SL;
     const unsigned bid = blockIdx.x;
     const int g = bid % job.nrg;
     const int tile = bid / job.nrg;
@@ -341,45 +342,42 @@ __global__ void __launch_bounds__(DualGeo<R1>::RG * DualGeo<R1>::NT, 1) pass_c_d
 #pragma unroll
     for (int i = 0; i < ITU * R1; i++) accr[i] = mka(0.0, 0.0);
     const size_t rowbox = (size_t)row * job.tb;
-    if (bs) p3_stage_u<R1, U, NT>(tid, ua_base + (size_t)job.a_src[rowok ? row : 0] * Ng, x, yb, UA);
-    stage_commit();
     unsigned rem = cta_ev;
+    if (bs) p3_stage_u<R1, U, NT>(tid, ua_base + (size_t)job.a_src[rowok ? row : 0] * Ng, x, yb, UA);
     if (rem) {
         const int c0 = __ffs(rem) - 1;
         if (ev >> c0 & 1u) p3_stage<R1, U, NT>(tid, work + (rowbox + c0) * Ng, x, yb, G);
+        if (job.amask >> c0 & 1u) p3_stage_u_share<R1, U, NT, RG>(wg, tid, ub_base + (size_t)job.b_src[c0] * Ng, x, yb, G2);
     }
     stage_commit();
-    stage_wait<1>();  // the row's u_a elements have landed (the first column's work-box elements may still be in flight)
+    stage_wait<0>();
     if (bs) p3_scale_slots<R1, U, NT>(tid, UA, (real)(-job.coef_a[row]));
-    __syncthreads();  // twiddle table
+    __syncthreads();  // twiddle table; the first column's u_b slots
+    int par = 0;
     while (rem) {
         const int c = __ffs(rem) - 1;
         rem &= rem - 1;
         const bool act = ev >> c & 1u;
-        const bool col_a = job.amask >> c & 1u;
-        stage_wait<0>();
+        cplx* S = S0 + (par * RG + wg) * TILE;
         if (act) p3_y2inv_staged<R1, U, NT>(tid, G, S);
-        if (col_a) p3_stage_u_share<R1, U, NT, RG>(wg, tid, ub_base + (size_t)job.b_src[c] * Ng, x, yb, G2);
-        stage_commit();  // group 1: this thread's share of the column's u_b elements
-        if (rem) {
+        if (rem) {  // the next column's work-box elements (this group's row) and this thread's share of its u_b elements
             const int cn = __ffs(rem) - 1;
             if (ev >> cn & 1u) p3_stage<R1, U, NT>(tid, work + (rowbox + cn) * Ng, x, yb, G);
+            if (job.amask >> cn & 1u) p3_stage_u_share<R1, U, NT, RG>(wg, tid, ub_base + (size_t)job.b_src[cn] * Ng, x, yb, G2 + (par ^ 1) * SL);
         }
-        stage_commit();  // group 2 (possibly empty): the next column's work-box elements
+        stage_commit();
         group_barrier(1 + wg, NT);
         if (act) p13_z8<R1, U, NT, +1, false>(tid, S, T, twr);
-        stage_wait<1>();
-        __syncthreads();  // S of the group is complete; every thread's share of u_b has landed
-        if (act) p3_zinv2_dual<R1, U, NT>(tid, S, G2, UA, job.coef_b[c], col_a, bs >> c & 1u, accr);
+        group_barrier(1 + wg, NT);
+        if (act) p3_zinv2_dual<R1, U, NT>(tid, S, G2 + par * SL, UA, job.coef_b[c], job.amask >> c & 1u, bs >> c & 1u, accr);
         unsigned gm = 0u;
 #pragma unroll
         for (int w = 0; w < RG; w++)
             if (g * RG + w < job.ta && (job.bside[g * RG + w] >> c & 1u)) gm |= 1u << w;
-        if (gm) {
-            __syncthreads();
-            p3_reduce_b<R1, U, NT, RG>(wg, tid, S0, TILE, gm, part_base + ((size_t)g * job.tb + c) * Ng, x, yb);
-        }
-        __syncthreads();  // S and G2 are free for the next column
+        stage_wait<0>();
+        __syncthreads();  // P tiles complete; the next column's u_b slots complete; this column's u_b slots free
+        if (gm) p3_reduce_b<R1, U, NT, RG>(wg, tid, S0 + par * RG * TILE, TILE, gm, part_base + ((size_t)g * job.tb + c) * Ng, x, yb);
+        par ^= 1;
     }
     if (ev & job.amask) p3_flush_reg<R1, U, NT>(tid, accr, acc_base + (size_t)job.a_tgt[row] * Ng, x, yb);
 }
@@ -500,7 +498,7 @@ struct Launch {
     static constexpr size_t smem_a = sizeof(cplx) * ((size_t)U1 * R1 * N + (TWREG ? 0 : R1 * 8));
     static constexpr size_t smem_c = sizeof(cplx) * ((size_t)U3 * R1 * N + (TWREG ? 0 : R1 * 8)) + sizeof(acc_c) * (ACCREG ? 0 : (size_t)U3 * R1 * N);
     static constexpr int IT3U = (U3 * R1 * 8 + FusedCfg<R1>::NT3 - 1) / FusedCfg<R1>::NT3;  // ... and in its last step
-    static constexpr size_t smem_c3 = smem_c + sizeof(cplx) * (size_t)((STAGE3 ? IT3S : 0) + (STAGEU ? IT3U : 0)) * R1 * FusedCfg<R1>::NT3;  // pass_c_kernel
+    static constexpr size_t smem_c3 = smem_c + sizeof(cplx) * (size_t)((STAGE3 ? 1 : 0) + (STAGEU ? 1 : 0)) * Slots<R1, FusedCfg<R1>::U3, FusedCfg<R1>::NT3>::COUNT;  // pass_c_kernel
     static constexpr size_t smem_b = sizeof(cplx) * ((size_t)N * P2Geo<Z>::PX);
 
     static constexpr int RG = FusedCfg<R1>::RG;  // dual sweep: rows per CTA (0: not built for this grid)

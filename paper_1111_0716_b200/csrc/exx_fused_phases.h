@@ -84,7 +84,7 @@ struct FusedCfgBase<2> {
     static constexpr bool TWREG = false, ACCREG = false;
     static constexpr int STAGE3 = s3(0);
     static constexpr int MINB1 = 1, MINB2 = 1, MINB3 = 1;
-    static constexpr int RG = rg(4);  // warp groups (rows) per CTA of the dual sweep; 0: two single sweeps instead
+    static constexpr int RG = rg(4);  // rows per CTA of the dual sweep (5.4b); 0: two single sweeps (measured faster at 40^3 and 64^3)
 };
 template <>
 struct FusedCfgBase<4> {
@@ -92,7 +92,7 @@ struct FusedCfgBase<4> {
     static constexpr bool TWREG = false, ACCREG = false;
     static constexpr int STAGE3 = s3(2);
     static constexpr int MINB1 = 1, MINB2 = 6, MINB3 = 1;
-    static constexpr int RG = rg(4);  // warp groups (rows) per CTA of the dual sweep; 0: two single sweeps instead
+    static constexpr int RG = rg(4);  // rows per CTA of the dual sweep (5.4b); 0: two single sweeps (measured faster at 40^3 and 64^3)
 };
 template <>
 struct FusedCfgBase<5> {
@@ -100,7 +100,7 @@ struct FusedCfgBase<5> {
     static constexpr bool TWREG = false, ACCREG = true;
     static constexpr int STAGE3 = s3(2);
     static constexpr int MINB1 = 1, MINB2 = 6, MINB3 = 1;
-    static constexpr int RG = rg(2);  // warp groups (rows) per CTA of the dual sweep; 0: two single sweeps instead
+    static constexpr int RG = rg(0);  // rows per CTA of the dual sweep (5.4b); 0: two single sweeps (measured faster at 40^3 and 64^3)
 };
 template <>
 struct FusedCfgBase<10> {
@@ -108,7 +108,7 @@ struct FusedCfgBase<10> {
     static constexpr bool TWREG = false, ACCREG = false;
     static constexpr int STAGE3 = s3(1);
     static constexpr int MINB1 = 1, MINB2 = 4, MINB3 = 1;
-    static constexpr int RG = rg(2);  // warp groups (rows) per CTA of the dual sweep; 0: two single sweeps instead
+    static constexpr int RG = rg(2);  // rows per CTA of the dual sweep (5.4b); 0: two single sweeps (measured faster at 40^3 and 64^3)
 };
 template <>
 struct FusedCfgBase<6> {
@@ -116,7 +116,7 @@ struct FusedCfgBase<6> {
     static constexpr bool TWREG = false, ACCREG = false;
     static constexpr int STAGE3 = s3(2);
     static constexpr int MINB1 = 1, MINB2 = 6, MINB3 = 1;  // min CTAs per SM asked of the compiler (register cap)
-    static constexpr int RG = rg(4);  // warp groups (rows) per CTA of the dual sweep; 0: two single sweeps instead
+    static constexpr int RG = rg(4);  // rows per CTA of the dual sweep (5.4b); 0: two single sweeps (measured faster at 40^3 and 64^3)
 };
 template <>
 struct FusedCfgBase<8> {
@@ -124,7 +124,7 @@ struct FusedCfgBase<8> {
     static constexpr bool TWREG = false, ACCREG = true;
     static constexpr int STAGE3 = s3(2);
     static constexpr int MINB1 = 1, MINB2 = 6, MINB3 = 1;
-    static constexpr int RG = rg(2);  // warp groups (rows) per CTA of the dual sweep; 0: two single sweeps instead
+    static constexpr int RG = rg(0);  // rows per CTA of the dual sweep (5.4b); 0: two single sweeps (measured faster at 40^3 and 64^3)
 };
 template <>
 struct FusedCfgBase<9> {
@@ -132,7 +132,7 @@ struct FusedCfgBase<9> {
     static constexpr bool TWREG = false, ACCREG = true;
     static constexpr int STAGE3 = s3(2);
     static constexpr int MINB1 = 1, MINB2 = 5, MINB3 = 1;
-    static constexpr int RG = rg(4);  // warp groups (rows) per CTA of the dual sweep; 0: two single sweeps instead
+    static constexpr int RG = rg(4);  // rows per CTA of the dual sweep (5.4b); 0: two single sweeps (measured faster at 40^3 and 64^3)
 };
 template <>
 struct FusedCfgBase<12> {
@@ -140,7 +140,7 @@ struct FusedCfgBase<12> {
     static constexpr bool TWREG = false, ACCREG = false;
     static constexpr int STAGE3 = s3(1);
     static constexpr int MINB1 = 1, MINB2 = 4, MINB3 = 1;
-    static constexpr int RG = rg(2);  // warp groups (rows) per CTA of the dual sweep; 0: two single sweeps instead
+    static constexpr int RG = rg(2);  // rows per CTA of the dual sweep (5.4b); 0: two single sweeps (measured faster at 40^3 and 64^3)
 };
 template <>
 struct FusedCfgBase<16> {
@@ -148,7 +148,7 @@ struct FusedCfgBase<16> {
     static constexpr bool TWREG = false, ACCREG = false;
     static constexpr int STAGE3 = s3(1);
     static constexpr int MINB1 = 1, MINB2 = 2, MINB3 = 1;
-    static constexpr int RG = rg(0);  // warp groups (rows) per CTA of the dual sweep; 0: two single sweeps instead
+    static constexpr int RG = rg(0);  // rows per CTA of the dual sweep (5.4b); 0: two single sweeps (measured faster at 40^3 and 64^3)
 };
 template <int R1>
 struct FusedCfg : FusedCfgBase<R1> {};
@@ -496,6 +496,13 @@ EXX_HD void p3_y2inv(int tid, const cplx* __restrict__ W, int x, int yb, cplx* S
 // STAGE3: the same step with the work-box elements fetched ahead of time.  Element j of item tid + i NT lives in the slot
 // G[(i R1 + j) NT + tid], written and read by this thread only (no barrier needed): p3_stage copies them there (cp.async on the
 // device, one element each, so the thread does not wait for them; a plain copy on the host), p3_y2inv_staged consumes them.
+// slot of element j of item tid + i NT: (i R1 + j) slot_stride + tid; a step has U N = 8 U R1 items, and when they fit one round
+// (NT >= items) the idle threads get no slots
+template <int R1, int U, int NT>
+struct Slots {
+    static constexpr int IT = (8 * U * R1 + NT - 1) / NT, STRIDE = IT == 1 ? 8 * U * R1 : NT;
+    static constexpr int COUNT = IT * R1 * STRIDE;  // slots of one step: work-box elements of the first step or u elements of the last one
+};
 EXX_HD void stage_elem(cplx* dst, const cplx* src) {
 #if defined(__CUDA_ARCH__)
     if (sizeof(cplx) == 16)
@@ -530,7 +537,7 @@ EXX_HD void p3_stage(int tid, const cplx* __restrict__ W, int x, int yb, cplx* G
             int kzl = it & 3, u = (it >> 2) % U, kzpos = (it / (4 * U)) * 4 + kzl;
             size_t base = widx<R1>(0, kzpos, x, yb * U + u);
 #pragma unroll
-            for (int j = 0; j < R1; j++) stage_elem(G + (i * R1 + j) * NT + tid, W + base + (size_t)j * (N / 4) * N * 32);
+            for (int j = 0; j < R1; j++) stage_elem(G + (i * R1 + j) * Slots<R1, U, NT>::STRIDE + tid, W + base + (size_t)j * (N / 4) * N * 32);
         }
     }
 }
@@ -546,7 +553,7 @@ EXX_HD void p3_stage_u(int tid, const cplx* __restrict__ um, int x, int yb, cplx
             int u = row / R1, n1y = row - u * R1;
             size_t base = ((size_t)x * N + (n1y * 8 + yb * U + u)) * N + n2z;
 #pragma unroll
-            for (int j = 0; j < R1; j++) stage_elem(G2 + (i * R1 + j) * NT + tid, um + base + j * 8);
+            for (int j = 0; j < R1; j++) stage_elem(G2 + (i * R1 + j) * Slots<R1, U, NT>::STRIDE + tid, um + base + j * 8);
         }
     }
 }
@@ -560,7 +567,7 @@ EXX_HD void p3_y2inv_staged(int tid, const cplx* G, cplx* S) {
             int kzl = it & 3, u = (it >> 2) % U, kzpos = (it / (4 * U)) * 4 + kzl;
             cplx v[R1];
 #pragma unroll
-            for (int j = 0; j < R1; j++) v[j] = G[(i * R1 + j) * NT + tid];
+            for (int j = 0; j < R1; j++) v[j] = G[(i * R1 + j) * Slots<R1, U, NT>::STRIDE + tid];
             dft<R1, +1>(v);
 #pragma unroll
             for (int j = 0; j < R1; j++) S[sidx<R1>(u, j, kzpos >> 3, kzpos & 7)] = v[j];
@@ -582,7 +589,7 @@ EXX_HD void p3_zinv2(int tid, const cplx* S, const cplx* __restrict__ um, double
             size_t base = ((size_t)x * N + (n1y * 8 + yb * U + u)) * N + n2z;
             cplx b[R1], v[R1];
 #pragma unroll
-            for (int j = 0; j < R1; j++) b[j] = USTG ? G2[(i * R1 + j) * NT + tid] : um[base + j * 8];
+            for (int j = 0; j < R1; j++) b[j] = USTG ? G2[(i * R1 + j) * Slots<R1, U, NT>::STRIDE + tid] : um[base + j * 8];
 #pragma unroll
             for (int j = 0; j < R1; j++) v[j] = S[sidx<R1>(u, n1y, j, n2z)];
             dft<R1, +1>(v);
@@ -632,7 +639,7 @@ EXX_HD void p3_zinv2_reg(int tid, const cplx* S, const cplx* __restrict__ um, do
             size_t base = ((size_t)x * N + (n1y * 8 + yb * U + u)) * N + n2z;
             cplx b[R1], v[R1];
 #pragma unroll
-            for (int j = 0; j < R1; j++) b[j] = USTG ? G2[(i * R1 + j) * NT + tid] : um[base + j * 8];
+            for (int j = 0; j < R1; j++) b[j] = USTG ? G2[(i * R1 + j) * Slots<R1, U, NT>::STRIDE + tid] : um[base + j * 8];
 #pragma unroll
             for (int j = 0; j < R1; j++) v[j] = S[sidx<R1>(u, n1y, j, n2z)];
             dft<R1, +1>(v);
@@ -685,13 +692,13 @@ EXX_HD void p3_zinv2_dual(int tid, cplx* S, const cplx* UB, const cplx* UA, doub
             if (do_a) {
 #pragma unroll
                 for (int j = 0; j < R1; j++) {
-                    cplx p = UB[(i * R1 + j) * NT + tid] * v[j];
+                    cplx p = UB[(i * R1 + j) * Slots<R1, U, NT>::STRIDE + tid] * v[j];
                     acc[i * R1 + j] = mka(acc[i * R1 + j].x - wfb * p.x, acc[i * R1 + j].y - wfb * p.y);
                 }
             }
             if (do_b) {
 #pragma unroll
-                for (int j = 0; j < R1; j++) S[sidx<R1>(u, n1y, j, n2z)] = mul_conj_b(UA[(i * R1 + j) * NT + tid], v[j]);
+                for (int j = 0; j < R1; j++) S[sidx<R1>(u, n1y, j, n2z)] = mul_conj_b(UA[(i * R1 + j) * Slots<R1, U, NT>::STRIDE + tid], v[j]);
             }
         }
     }
@@ -705,7 +712,7 @@ EXX_HD void p3_scale_slots(int tid, cplx* UA, real coef) {
     for (int i = 0; i < IT; i++)
         if (tid + i * NT < NI) {
 #pragma unroll
-            for (int j = 0; j < R1; j++) UA[(i * R1 + j) * NT + tid] = scale(coef, UA[(i * R1 + j) * NT + tid]);
+            for (int j = 0; j < R1; j++) UA[(i * R1 + j) * Slots<R1, U, NT>::STRIDE + tid] = scale(coef, UA[(i * R1 + j) * Slots<R1, U, NT>::STRIDE + tid]);
         }
 }
 
@@ -723,7 +730,7 @@ EXX_HD void p3_stage_u_share(int wg, int tid, const cplx* __restrict__ um, int x
             size_t base = ((size_t)x * N + (n1y * 8 + yb * U + u)) * N + n2z;
 #pragma unroll
             for (int j = 0; j < R1; j++)
-                if (j % RG == wg) stage_elem(G2 + (i * R1 + j) * NT + tid, um + base + j * 8);
+                if (j % RG == wg) stage_elem(G2 + (i * R1 + j) * Slots<R1, U, NT>::STRIDE + tid, um + base + j * 8);
         }
     }
 }

@@ -63,9 +63,9 @@ static void emu_pair(const cplx* un, const cplx* um, const double* Knat, double 
     for (int x = 0; x < N; x++)
         for (int yb = 0; yb < 8 / U3; yb++) {
             for (auto& a : accr) a = mka(0.0, 0.0);
-            std::vector<cplx> G2((size_t)IT3 * R1 * NT3);
+            std::vector<cplx> G2((size_t)Slots<R1, U3, NT3>::COUNT);
             if (STAGE3) {  // per-thread staging slots, as pass_c_kernel uses them
-                std::vector<cplx> G((size_t)((U3 * N + NT3 - 1) / NT3) * R1 * NT3);
+                std::vector<cplx> G((size_t)Slots<R1, U3, NT3>::COUNT);
                 for (int t = 0; t < NT3; t++) p3_stage<R1, U3, NT3>(t, W, x, yb, G.data());
                 for (int t = 0; t < NT3; t++) p3_y2inv_staged<R1, U3, NT3>(t, G.data(), S.data());
                 if (STAGEU)
@@ -135,7 +135,7 @@ static void emu_dual(int ta, int tb, const cplx* ua, const cplx* ub, const doubl
                      const unsigned* ev, const unsigned* bside, unsigned amask, acc_c* acc_a, acc_c* acc_b) {
     typedef FusedCfg<R1> C;
     constexpr int N = 8 * R1, U = C::U3, NT = C::NT3, Z = C::Z, RG = C::RG > 0 ? C::RG : 1;
-    constexpr int TILE = U * R1 * N, ITS = (U * N + NT - 1) / NT, ITU = (U * R1 * 8 + NT - 1) / NT, GS = ITS * R1 * NT, US = ITU * R1 * NT;
+    constexpr int TILE = U * R1 * N, ITU = (U * R1 * 8 + NT - 1) / NT, GS = Slots<R1, U, NT>::COUNT, US = GS;
     const size_t Ng = (size_t)N * N * N;
     std::vector<double> Kp(Ng);
     permute_ktable(R1, Z, KVW, Knat, Kp.data());

@@ -215,6 +215,12 @@ int exx_findex(const exx_ctx* ctx, int32_t* host_out /* Ng entries */);
 /* K'_{k-q}(g) as the library tabulated it (host_out: Ng doubles, C order). */
 int exx_kernel_table(const exx_ctx* ctx, int ik, int iq, double* host_out);
 
+/* Measurement aid ("report both fractions"): the fp64 vector-pipe peak of the current device, measured by a
+ * chain-free DFMA loop (8 independent accumulators per thread, 2 flops per DFMA, every SM filled; CUDA events, best of 3).
+ * *gflops_host receives GFLOP/s.  Not on the hot path; synchronises the stream.  The fused passes are plain fp64 FMA/ADD/MUL code
+ * (tcgen05 has no fp64 kind), so this is the ALU roofline bench.py quotes beside the HBM one. */
+int exx_measure_fp64_peak(void* cuda_stream, double* gflops_host);
+
 const char* exx_strerror(int code);
 const char* exx_last_error(const exx_ctx* ctx_or_null); /* detail of the last EXX_ERR_CUDA (thread-local if ctx NULL) */
 int exx_version(void);

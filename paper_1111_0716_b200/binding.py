@@ -27,7 +27,7 @@ EXX_INFO_ENERGY_ROUTE = 16
 SYMBOLS = ("exx_create", "exx_destroy", "exx_npw", "exx_index_map", "exx_psi_offset", "exx_set_option", "exx_get_option",
            "exx_get_info", "exx_get_kernel_time", "exx_kernel_class_name", "exx_apply", "exx_energy", "exx_apply_host",
            "exx_scatter", "exx_gather", "exx_fft3d", "exx_to_real", "exx_kernel_table", "exx_strerror", "exx_last_error",
-           "exx_version", "exx_subspace", "exx_fft3d_fused", "exx_findex", "exx_shard_plan", "exx_apply_to", "exx_subspace_block")
+           "exx_version", "exx_subspace", "exx_fft3d_fused", "exx_findex", "exx_shard_plan", "exx_apply_to", "exx_subspace_block", "exx_measure_fp64_peak")
 
 
 class KernelParams(C.Structure):
@@ -98,6 +98,7 @@ def lib():
         L.exx_last_error.argtypes = [vp]
         L.exx_last_error.restype = C.c_char_p
         L.exx_version.restype = C.c_int
+        L.exx_measure_fp64_peak.argtypes = [vp, dp]
         _lib = L
     return _lib
 
@@ -117,6 +118,17 @@ def shard_plan(nk, nbands, occ, symmetry=True, tile=0, nshards=1):
     if rc:
         raise ExxError(rc)
     return pairs, passes
+
+
+def measure_fp64_peak(stream=None):
+    """exx_measure_fp64_peak: the device's fp64 vector-pipe peak in GFLOP/s from a DFMA loop (measurement aid for bench.py)."""
+    import torch
+    g = C.c_double()
+    st = stream if stream is not None else torch.cuda.current_stream().cuda_stream
+    rc = lib().exx_measure_fp64_peak(C.c_void_p(st), C.cast(C.byref(g), C.POINTER(C.c_double)))
+    if rc:
+        raise ExxError(rc)
+    return g.value
 
 
 def all_reduce_sum(t, group=None):

@@ -348,3 +348,56 @@ int launch_energy(exx_ctx* c, const double2* psi, const double2* vx) {
 }
 
 }  // namespace exx
+
+// ---- fp64 pipe peak (exx_measure_fp64_peak): 8 independent DFMA chains per thread, no memory traffic ------------------------
+namespace exx {
+__global__ void __launch_bounds__(256) fp64_peak_kernel(double* out, int iters, double a, double b) {
+    double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+    for (int i = 0; i < iters; i++) {
+#pragma unroll
+        for (int r = 0; r < 8; r++) {
+            x0 = fma(x0, a, b), x1 = fma(x1, a, b), x2 = fma(x2, a, b), x3 = fma(x3, a, b);
+            x4 = fma(x4, a, b), x5 = fma(x5, a, b), x6 = fma(x6, a, b), x7 = fma(x7, a, b);
+        }
+    }
+    double s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+    if (s == 12345.678) out[blockIdx.x * blockDim.x + threadIdx.x] = s;  // never true: keeps the chains alive without a store
+}
+}  // namespace exx
+
+extern "C" int exx_measure_fp64_peak(void* cuda_stream, double* gflops_host) {
+    if (!gflops_host) return EXX_ERR_NULL;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return EXX_ERR_CUDA;
+    }
+    double* out = nullptr;
+    const int blocks = sms * 8, threads = 256, iters = 4096;
+    if (cudaMalloc((void**)&out, sizeof(double) * blocks * threads) != cudaSuccess) {
+        cudaGetLastError();
+        return EXX_ERR_ALLOC;
+    }
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    float best = 0.f;
+    int rc = EXX_OK;
+    for (int rep = 0; rep < 4 && rc == EXX_OK; rep++) {  // first repetition = warm-up
+        cudaEventRecord(e0, st);
+        exx::fp64_peak_kernel<<<blocks, threads, 0, st>>>(out, iters, 0.999999, 1e-9);
+        cudaEventRecord(e1, st);
+        if (cudaEventSynchronize(e1) != cudaSuccess || cudaGetLastError() != cudaSuccess) rc = EXX_ERR_CUDA;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (rep > 0 && ms > 0.f && (best == 0.f || ms < best)) best = ms;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(out);
+    if (rc != EXX_OK || best <= 0.f) return EXX_ERR_CUDA;
+    const double flops = 2.0 * 64.0 * (double)iters * (double)blocks * (double)threads;  // 64 DFMA per thread per iteration
+    *gflops_host = flops / (best * 1e-3) / 1e9;
+    return EXX_OK;
+}

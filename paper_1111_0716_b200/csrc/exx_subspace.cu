@@ -6,7 +6,7 @@
 // M = A^H B with A = psi (nb x npw, row-major, npw contiguous) and B = V_x psi (same layout):
 //   Re M_ij = sum_g (ar_ig br_jg + ai_ig bi_jg),   Im M_ij = sum_g (ar_ig bi_jg - ai_ig br_jg)
 // i.e. four real m8n8k4 products per 4 plane waves.  A warp owns one 8 x 8 tile of M over one slice of the plane waves
-// (split-K); the slices are added in a fixed order by a second kernel, so the result is deterministic.
+// (split-K; 32 x 32 per warp, see the kernel); the slices are added in a fixed order by a second kernel, so the result is deterministic.
 #include "exx_internal.h"
 
 namespace exx {
@@ -15,39 +15,68 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-// partial[s][i][j] (complex) for slice s: plane waves [s*chunk, min(npw, (s+1)*chunk)); chunk is a multiple of 4
+// partial[s][i][j] (complex) for slice s: plane waves [s*chunk, min(npw, (s+1)*chunk)); chunk is a multiple of 4.
+// A warp owns a (8 MI) x (8 NJ) tile of M for one slice: per 4 plane waves it loads MI + NJ complex fragments (one element per
+// lane each) and issues 4 MI NJ DMMAs, so every fragment is reused NJ (MI) times from registers; the 4 warps of a CTA take 4
+// consecutive slices of the same tile (their rows are shared in L1/L2).
+template <int MI, int NJ>
 __global__ void __launch_bounds__(128) subspace_partial_kernel(const double2* __restrict__ A, const double2* __restrict__ Bm, int nb, int npw, int chunk,
-                                                                double2* __restrict__ partial) {
+                                                                int nslices, double2* __restrict__ partial) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int tiles = (nb + 7) / 8;
-    const int tile = blockIdx.x * 4 + warp;
-    if (tile >= tiles * tiles) return;
-    const int ti = tile / tiles, tj = tile % tiles, s = blockIdx.y;
+    const int tj_n = (nb + 8 * NJ - 1) / (8 * NJ);
+    const int ti = blockIdx.x / tj_n, tj = blockIdx.x % tj_n, s = blockIdx.y * 4 + warp;
+    if (s >= nslices) return;
     const int row = lane >> 2, kk = lane & 3;        // fragment coordinates: A (row, kk), B (kk, col = row)
-    const int i = ti * 8 + row, j = tj * 8 + row;
     const int g0 = s * chunk, g1 = min(npw, g0 + chunk);
-    const double2* a = A + (size_t)min(i, nb - 1) * npw;
-    const double2* b = Bm + (size_t)min(j, nb - 1) * npw;
-    const bool ia = i < nb, jb = j < nb;
-    double cr0 = 0.0, cr1 = 0.0, ci0 = 0.0, ci1 = 0.0;
+    const double2* a[MI];
+    const double2* b[NJ];
+    bool ia[MI], jb[NJ];
+#pragma unroll
+    for (int m = 0; m < MI; m++) {
+        const int i = (ti * MI + m) * 8 + row;
+        ia[m] = i < nb;
+        a[m] = A + (size_t)min(i, nb - 1) * npw;
+    }
+#pragma unroll
+    for (int n = 0; n < NJ; n++) {
+        const int j = (tj * NJ + n) * 8 + row;
+        jb[n] = j < nb;
+        b[n] = Bm + (size_t)min(j, nb - 1) * npw;
+    }
+    double cr[MI][NJ][2], ci[MI][NJ][2];
+#pragma unroll
+    for (int m = 0; m < MI; m++)
+#pragma unroll
+        for (int n = 0; n < NJ; n++) cr[m][n][0] = cr[m][n][1] = ci[m][n][0] = ci[m][n][1] = 0.0;
     for (int g = g0 + kk; g < g1 + kk; g += 4) {     // every lane makes the same number of trips (mma.sync is warp-wide)
-        double2 x = make_double2(0.0, 0.0), y = make_double2(0.0, 0.0);
-        if (g < g1) {
-            if (ia) x = a[g];
-            if (jb) y = b[g];
-        }
-        dmma884(cr0, cr1, x.x, y.x);
-        dmma884(cr0, cr1, x.y, y.y);
-        dmma884(ci0, ci1, x.x, y.y);
-        dmma884(ci0, ci1, -x.y, y.x);
+        double2 x[MI], y[NJ];
+        const bool in = g < g1;
+#pragma unroll
+        for (int m = 0; m < MI; m++) x[m] = (in && ia[m]) ? a[m][g] : make_double2(0.0, 0.0);
+#pragma unroll
+        for (int n = 0; n < NJ; n++) y[n] = (in && jb[n]) ? b[n][g] : make_double2(0.0, 0.0);
+#pragma unroll
+        for (int m = 0; m < MI; m++)
+#pragma unroll
+            for (int n = 0; n < NJ; n++) {
+                dmma884(cr[m][n][0], cr[m][n][1], x[m].x, y[n].x);
+                dmma884(cr[m][n][0], cr[m][n][1], x[m].y, y[n].y);
+                dmma884(ci[m][n][0], ci[m][n][1], x[m].x, y[n].y);
+                dmma884(ci[m][n][0], ci[m][n][1], -x[m].y, y[n].x);
+            }
     }
     // accumulator fragment: row = lane / 4, columns 2 (lane % 4) and 2 (lane % 4) + 1
-    const int oi = ti * 8 + row, oj = tj * 8 + 2 * kk;
     double2* p = partial + (size_t)s * nb * nb;
-    if (oi < nb) {
-        if (oj < nb) p[(size_t)oi * nb + oj] = make_double2(cr0, ci0);
-        if (oj + 1 < nb) p[(size_t)oi * nb + oj + 1] = make_double2(cr1, ci1);
-    }
+#pragma unroll
+    for (int m = 0; m < MI; m++)
+#pragma unroll
+        for (int n = 0; n < NJ; n++) {
+            const int oi = (ti * MI + m) * 8 + row, oj = (tj * NJ + n) * 8 + 2 * kk;
+            if (oi < nb) {
+                if (oj < nb) p[(size_t)oi * nb + oj] = make_double2(cr[m][n][0], ci[m][n][0]);
+                if (oj + 1 < nb) p[(size_t)oi * nb + oj + 1] = make_double2(cr[m][n][1], ci[m][n][1]);
+            }
+        }
 }
 
 __global__ void subspace_reduce_kernel(const double2* __restrict__ partial, int n2, int nslices, double2* __restrict__ M) {
@@ -66,9 +95,12 @@ __global__ void subspace_reduce_kernel(const double2* __restrict__ partial, int 
 int launch_subspace(exx_ctx* c, int ik, const double2* psi, const double2* vx, double2* M, int nvec) {
     const int nb = nvec > 0 ? nvec : c->nb, npw = c->npw[ik];
     const int64_t offk = c->off[ik] / c->nb * nb;
-    const int tiles = (nb + 7) / 8;
-    // slices: enough warps to fill the machine, chunks a multiple of 4 plane waves
-    int nslices = std::max(1, std::min(64, (148 * 16 * 4) / std::max(1, tiles * tiles)));
+    constexpr int MI = 4, NJ = 4;  // 32 x 32 tile of M per warp
+    const int tiles = ((nb + 8 * MI - 1) / (8 * MI)) * ((nb + 8 * NJ - 1) / (8 * NJ));
+    int dev = 0, sms = 148;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    // slices: about 8 warps per SM over the whole machine, chunks a multiple of 4 plane waves
+    int nslices = std::max(1, std::min(256, (sms * 8 + tiles - 1) / tiles));
     int chunk = ((npw + nslices - 1) / nslices + 3) / 4 * 4;
     nslices = (npw + chunk - 1) / chunk;
     const size_t need = sizeof(double2) * (size_t)nslices * nb * nb;
@@ -85,8 +117,8 @@ int launch_subspace(exx_ctx* c, int ik, const double2* psi, const double2* vx, d
     }
     {
         LaunchScope ls(c, KC_SUBSPACE, 1);
-        dim3 grid((tiles * tiles + 3) / 4, nslices);
-        subspace_partial_kernel<<<grid, 128, 0, c->stream>>>(psi + offk, vx + offk, nb, npw, chunk, (double2*)c->subspace_dev);
+        dim3 grid(tiles, (nslices + 3) / 4);
+        subspace_partial_kernel<MI, NJ><<<grid, 128, 0, c->stream>>>(psi + offk, vx + offk, nb, npw, chunk, nslices, (double2*)c->subspace_dev);
     }
     {
         LaunchScope ls(c, KC_SUBSPACE, 0);

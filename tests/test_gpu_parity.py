@@ -9,12 +9,16 @@ import os
 import numpy as np
 import pytest
 
+import sys
+
 from oracle import exx_ref as R
 from paper_1111_0716_b200 import workloads as W
 
 pytestmark = pytest.mark.gpu
 
 GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+sys.path.insert(0, GOLD)
+from probe import probe_vector  # noqa: E402  (seeded probe vectors of the stored per-band functional)
 TOL_VX = 1e-10
 TOL_EX = 1e-11
 
@@ -176,7 +180,7 @@ def test_apply_C1_full_parity(B):
     assert abs(e - gold["E_x_E1"]) < 1e-15
 
 
-def _check_golden(B, name, live_rows=0, prune=1, symmetry=1):
+def _check_golden(B, name, live_rows=0, prune=1, symmetry=1, dual=1):
     """Big configs: the GPU applies V_x in full; rows, per-band energies and E_x are compared with stored oracle
     results (tests/golden/make_golden.py) and, for `live_rows` rows, with the oracle run now."""
     import torch
@@ -192,6 +196,7 @@ def _check_golden(B, name, live_rows=0, prune=1, symmetry=1):
     pd = g.to_device(psi)
     g.set_option(B.EXX_OPT_PRUNE, prune)
     g.set_option(B.EXX_OPT_SYMMETRY, symmetry)
+    g.set_option(B.EXX_OPT_DUAL_SWEEP, dual)
     out = g.apply(pd, w.occ)
     assert g.get_info(B.EXX_INFO_SYMMETRY) == symmetry
     assert g.get_info(B.EXX_INFO_PAIRS_EXECUTED) == (w.pair_evals if not symmetry else g.get_info(B.EXX_INFO_PAIRS_EXECUTED))
@@ -209,6 +214,14 @@ def _check_golden(B, name, live_rows=0, prune=1, symmetry=1):
         assert np.abs(pb - np.array(gold["per_band_energy"])).max() <= TOL_EX * abs(gold["E_x_E1"])
         norms = np.array([np.linalg.norm(g.band(got, k, n)) for k in range(w.nk) for n in range(w.nbands)])
         assert np.abs(norms / np.array(gold["per_band_norm"]) - 1).max() < TOL_VX
+        if "per_band_probe" in gold:
+            # every band's row against the oracle through a third functional, <z_k | V_x c_nk> with a seeded unit probe vector:
+            # |<z|got> - <z|want>| <= |got - want| (Cauchy-Schwarz), so the rel-L2 bar of the rows applies to it unchanged
+            for k in range(w.nk):
+                z = probe_vector(w.seed, k, g.npw[k])
+                for n in range(w.nbands):
+                    pr = gold["per_band_probe"][k * w.nbands + n]
+                    assert abs(np.vdot(z, g.band(got, k, n)) - complex(pr[0], pr[1])) <= TOL_VX * gold["per_band_norm"][k * w.nbands + n], (name, k, n)
     # properties that hold at any size
     assert e < 0 and abs(pb.sum() - e) <= 1e-13 * abs(e) and np.all(pb <= 0)
     assert g.get_info(B.EXX_INFO_PAIRS_ORDERED) == w.pair_evals
@@ -229,7 +242,16 @@ def test_apply_C3_parity(B):
 
 
 def test_apply_C4a_parity(B):
+    """The benchmarked configuration against the FULL oracle result: E_x by (E1) and (E2), all 160 per-band energies, norms and
+    probe functionals, and 8 complete rows (tile edges 0/31/32/159, interiors 40/95/128, a half-occupied band 158)."""
+    gold = json.load(open(os.path.join(GOLD, "exx_C4a.json")))
+    assert "E_x_E1" in gold and "E_x_E2" in gold and len(gold["per_band_energy"]) == 160 and len(gold["rows"]) >= 8
     _check_golden(B, "C4a")
+
+
+def test_apply_C4a_two_sweeps_parity(B):
+    """EXX_OPT_DUAL_SWEEP = 0 (two sweeps of the last pass instead of the dual sweep) against the same oracle values."""
+    _check_golden(B, "C4a", dual=0)
 
 
 def test_apply_C5_parity(B):

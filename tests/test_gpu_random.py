@@ -1,5 +1,5 @@
 """GPU parity on seeded random problems (-m gpu): cell, grid (fused and generic), k-points and weights, cutoff, kernel, band count,
-occupations that differ from k-point to k-point, and every option that changes how the work is cut up (pair symmetry, compact grid,
+occupations that differ from k-point to k-point, and every option that changes how the work is cut up (pair symmetry, dual sweep, compact grid,
 batch tiles, generic kernels, shards).  Each case: V_x psi per band at 1e-10 and E_x / per-band terms at 1e-11 against the oracle,
 for the shards' sum, for (E1) from the summed V_x psi and for the pair-density route from psi alone; then exx_apply_to on random trial vectors.
 """
@@ -45,6 +45,7 @@ def _case(seed):
         occ[:] = 0
     opts = dict(sym=int(rng.integers(0, 2)), prune=int(rng.integers(0, 2)), tn=int(rng.choice([0, 1, 2, 3, 5, 8])),
                 tm=int(rng.choice([0, 1, 2, 3, 5, 8])), path=int(rng.choice([0, 0, 0, 1])), P=int(rng.choice([1, 1, 2, 3])))
+    opts["dual"] = int(rng.integers(0, 2))   # drawn last: the cases of the earlier options are unchanged
     return w, occ, opts
 
 
@@ -70,6 +71,7 @@ def test_random_problems_against_oracle(B, block):
         g.set_option(B.EXX_OPT_TILE_N, opts["tn"])
         g.set_option(B.EXX_OPT_TILE_M, opts["tm"])
         g.set_option(B.EXX_OPT_PATH, opts["path"])
+        g.set_option(B.EXX_OPT_DUAL_SWEEP, opts["dual"])
         acc, e_parts, pb_parts = None, 0.0, 0.0
         for r in range(opts["P"]):
             g.set_option(B.EXX_OPT_SHARD_COUNT, opts["P"])

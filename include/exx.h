@@ -94,6 +94,10 @@ enum {
                                (row group, column) that a small reduction kernel adds in a fixed order); 0: two sweeps of the last
                                pass, the second repeating the inverse y/z steps (grids without a dual kernel always do this).
                                Results differ by rounding order only; both are deterministic */
+    EXX_OPT_PRUNE_SPHERE = 14, /* fused path, S1 and S7 ("the sphere is ~2 % of the box").  1 (default): the inverse
+                               transform of the bands reads, and the forward transform of the accumulators writes, only the
+                               x rows of the frequency box with |g_x| <= max |g_x| of the spheres (46 % of the rows at C4a); the
+                               scatter clears only those.  0: whole boxes.  Bit-identical results */
     EXX_OPT_ENERGY_ROUTE = 11 /* what exx_energy does when it is given no V_x psi.  0 (default): the pair-density route
                                E_x = -1/2 sum w_k w_q f_nk f_mq sum_g K'_{k-q}(g) |rho^_{nk,mq}(g)|^2 (form (E2) of DESIGN.md section 2:
                                Eq. 2 of PAPER.md, L127-130, written in reciprocal space) wherever the fused kernels run: the co-density

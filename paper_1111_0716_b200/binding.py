@@ -17,6 +17,7 @@ EXX_OPT_SHARD_COUNT, EXX_OPT_SHARD_RANK = 9, 10
 EXX_OPT_ENERGY_ROUTE = 11
 EXX_OPT_KEEP_U = 12
 EXX_OPT_DUAL_SWEEP = 13
+EXX_OPT_PRUNE_SPHERE = 14
 (EXX_INFO_LAUNCHES, EXX_INFO_PAIRS_ORDERED, EXX_INFO_PAIRS_EXECUTED, EXX_INFO_PATH_USED, EXX_INFO_WORKSPACE_BYTES,
  EXX_INFO_NCOEF, EXX_INFO_TILE_N, EXX_INFO_TILE_M, EXX_INFO_PRUNED, EXX_INFO_NUM_KERNEL_CLASSES, EXX_INFO_WORK_GRID,
  EXX_INFO_COMPACT_GRID, EXX_INFO_SYMMETRY) = range(1, 14)

@@ -491,6 +491,9 @@ int exx_set_option(exx_ctx* c, int option, int64_t value) {
     case EXX_OPT_DUAL_SWEEP:
         c->opt_dual = value ? 1 : 0;
         return EXX_OK;
+    case EXX_OPT_PRUNE_SPHERE:
+        c->opt_prune_rows = value ? 1 : 0;
+        return EXX_OK;
     default: return EXX_ERR_BAD_ARG;
     }
 }
@@ -509,6 +512,7 @@ int exx_get_option(const exx_ctx* c, int option, int64_t* value) {
     case EXX_OPT_ENERGY_ROUTE: *value = c->opt_energy_route; return EXX_OK;
     case EXX_OPT_KEEP_U: *value = c->opt_keep_u; return EXX_OK;
     case EXX_OPT_DUAL_SWEEP: *value = c->opt_dual; return EXX_OK;
+    case EXX_OPT_PRUNE_SPHERE: *value = c->opt_prune_rows; return EXX_OK;
     default: return EXX_ERR_BAD_ARG;
     }
 }
@@ -675,6 +679,7 @@ static void options_to_inner(const exx_ctx* c, exx_ctx* in) {
     in->opt_precision = c->opt_precision;
     in->opt_keep_u = c->opt_keep_u;
     in->opt_dual = c->opt_dual;
+    in->opt_prune_rows = c->opt_prune_rows;
     in->opt_shard_count = c->opt_shard_count;
     in->opt_shard_rank = c->opt_shard_rank;
 }

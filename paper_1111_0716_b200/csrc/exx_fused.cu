@@ -442,8 +442,18 @@ static int fused_u_cache(exx_ctx* c, FusedState* st, const double2* psi, cplx* u
         const int64_t offk = c->off[k] / nb * nvec;
         for (int n0 = 0; n0 < nvec; n0 += bmax) {
             const int bn = std::min(bmax, nvec - n0);
-            if ((rc = launch_scatter(c, k, psi + offk + (int64_t)n0 * c->npw[k], bn, (double2*)c->work_dev, st->fmap_dev + c->map_off[k]))) return rc;
-            EXX_DISPATCH_R1(st->R1, rc = L::fft_inverse(c, (cplx*)c->work_dev, bn, u_out + ((size_t)k * stride + n0) * Ng));
+            if (c->opt_prune_rows) {
+                // sphere pruning: only the x rows with |kx| <= gmax are cleared, scattered into and read by the inverse transform
+                RowMask rows;
+                EXX_DISPATCH_R1(st->R1, rows = L::sphere_rows(c->gmax[0]));
+                EXX_DISPATCH_R1(st->R1, rc = L::zero_rows(c, (cplx*)c->work_dev, bn, rows));
+                if (rc) return rc;
+                if ((rc = launch_scatter(c, k, psi + offk + (int64_t)n0 * c->npw[k], bn, (double2*)c->work_dev, st->fmap_dev + c->map_off[k], false))) return rc;
+                EXX_DISPATCH_R1(st->R1, rc = L::fft_inverse(c, (cplx*)c->work_dev, bn, u_out + ((size_t)k * stride + n0) * Ng, rows));
+            } else {
+                if ((rc = launch_scatter(c, k, psi + offk + (int64_t)n0 * c->npw[k], bn, (double2*)c->work_dev, st->fmap_dev + c->map_off[k]))) return rc;
+                EXX_DISPATCH_R1(st->R1, rc = L::fft_inverse(c, (cplx*)c->work_dev, bn, u_out + ((size_t)k * stride + n0) * Ng));
+            }
             if (rc) return rc;
         }
     }
@@ -559,7 +569,13 @@ int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out,
         const int64_t offk = c->off[k] / nb * na;
         for (int n0 = 0; n0 < na; n0 += bmax) {
             const int bn = std::min(bmax, na - n0);
-            EXX_DISPATCH_R1(st->R1, rc = L::fft_forward(c, (const cplx*)(acc + ((size_t)k * na + n0) * Ng), bn, work));
+            if (c->opt_prune_rows) {  // the gather reads sphere points only: rows with |kx| > gmax are not written back
+                RowMask rows;
+                EXX_DISPATCH_R1(st->R1, rows = L::sphere_rows(c->gmax[0]));
+                EXX_DISPATCH_R1(st->R1, rc = L::fft_forward(c, (const cplx*)(acc + ((size_t)k * na + n0) * Ng), bn, work, rows));
+            } else {
+                EXX_DISPATCH_R1(st->R1, rc = L::fft_forward(c, (const cplx*)(acc + ((size_t)k * na + n0) * Ng), bn, work));
+            }
             if (rc) return rc;
             if ((rc = launch_gather(c, k, (const double2*)work, bn, out + offk + (int64_t)n0 * c->npw[k], st->fmap_dev + c->map_off[k]))) return rc;
         }

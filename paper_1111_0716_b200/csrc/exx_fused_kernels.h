@@ -9,7 +9,9 @@ using ::exx::AJob;
 using ::exx::CJob;
 using ::exx::DJob;
 using ::exx::RJob;
+using ::exx::RowMask;
 using ::exx::KC_PASS_R;
+using ::exx::KC_SCATTER;
 using ::exx::LaunchScope;
 using ::exx::KC_PASS_A;
 using ::exx::KC_PASS_B;
@@ -428,9 +430,12 @@ __global__ void __launch_bounds__(FusedCfg<R1>::NT1, FusedCfg<R1>::MINB1) fft_a_
 }
 
 // the pass-B half, in place on work box p.  SIGN < 0: second y step, forward x (-> F layout); SIGN > 0: inverse x, first
-// inverse y step (F layout ->)
+// inverse y step (F layout ->).  Sphere pruning (S1/S7): bit x of `rows` says whether F-layout x row x can hold a
+// sphere coefficient (|kx| <= gmax).  The inverse (S1) bulk-copies only those rows in and zero-fills the others on chip (they are
+// never read from the box, so the scatter need not clear them); the forward (S7) writes only those rows back (the gather reads
+// no other).  All ones = plain transform.
 template <int R1, int SIGN>
-__global__ void __launch_bounds__(FusedCfg<R1>::NT2, FusedCfg<R1>::MINB2) fft_b_kernel(cplx* __restrict__ work, int nbox) {
+__global__ void __launch_bounds__(FusedCfg<R1>::NT2, FusedCfg<R1>::MINB2) fft_b_kernel(cplx* __restrict__ work, int nbox, RowMask rows) {
     constexpr int N = 8 * R1, Z = FusedCfg<R1>::Z, NT = FusedCfg<R1>::NT2, PX = P2Geo<Z>::PX;
     constexpr size_t Ng = (size_t)N * N * N;
     constexpr uint32_t ROWB = 8 * Z * sizeof(cplx);
@@ -443,9 +448,26 @@ __global__ void __launch_bounds__(FusedCfg<R1>::NT2, FusedCfg<R1>::MINB2) fft_b_
     cplx* Wt = work + (size_t)p * Ng + (size_t)tile * ((size_t)N * 8 * Z);
     if (tid == 0) mbar_init(&bar, 1);
     __syncthreads();
-    if (tid == 0) mbar_arrive_expect_tx(&bar, ROWB * N);
-    for (int x = tid; x < N; x += NT) bulk_g2s(S + x * PX, Wt + x * 8 * Z, ROWB, &bar);
-    mbar_wait(&bar, 0);
+    if (SIGN > 0) {
+        int nrows = 0;
+#pragma unroll
+        for (int i = 0; i < 4; i++) nrows += __popc(rows.w[i]);
+        if (tid == 0) mbar_arrive_expect_tx(&bar, ROWB * (uint32_t)nrows);
+        for (int x = tid; x < N; x += NT)
+            if (rows.w[x >> 5] >> (x & 31) & 1u) bulk_g2s(S + x * PX, Wt + x * 8 * Z, ROWB, &bar);
+        if (nrows < N) {
+            for (int e = tid; e < N * 8 * Z; e += NT) {
+                const int x = e / (8 * Z);
+                if (!(rows.w[x >> 5] >> (x & 31) & 1u)) S[x * PX + (e - x * 8 * Z)] = mk(EXX_RC(0.0), EXX_RC(0.0));
+            }
+        }
+        mbar_wait(&bar, 0);
+        if (nrows < N) __syncthreads();  // the zero rows were written by other threads
+    } else {
+        if (tid == 0) mbar_arrive_expect_tx(&bar, ROWB * N);
+        for (int x = tid; x < N; x += NT) bulk_g2s(S + x * PX, Wt + x * 8 * Z, ROWB, &bar);
+        mbar_wait(&bar, 0);
+    }
     if (SIGN < 0) {
         p2_y8<R1, Z, NT, -1>(tid, S, k1y);
         __syncthreads();
@@ -461,8 +483,22 @@ __global__ void __launch_bounds__(FusedCfg<R1>::NT2, FusedCfg<R1>::MINB2) fft_b_
     }
     fence_proxy_async_smem();
     __syncthreads();
-    for (int x = tid; x < N; x += NT) bulk_s2g(Wt + x * 8 * Z, S + x * PX, ROWB);
+    for (int x = tid; x < N; x += NT)
+        if (SIGN > 0 || (rows.w[x >> 5] >> (x & 31) & 1u)) bulk_s2g(Wt + x * 8 * Z, S + x * PX, ROWB);
     bulk_commit_wait_all();
+}
+
+// clears the F-layout x rows of `rows` in nbox work boxes (the only rows the pruned inverse transform reads): S1's scatter target
+template <int R1>
+__global__ void __launch_bounds__(256) zero_rows_kernel(cplx* __restrict__ work, RowMask rows) {
+    constexpr int N = 8 * R1, Z = FusedCfg<R1>::Z;
+    constexpr size_t Ng = (size_t)N * N * N;
+    // one CTA per (box, pass-B tile): N rows of 8 Z elements
+    cplx* Wt = work + (size_t)blockIdx.y * Ng + (size_t)blockIdx.x * ((size_t)N * 8 * Z);
+    for (int e = threadIdx.x; e < N * 8 * Z; e += blockDim.x) {
+        const int x = e / (8 * Z);
+        if (rows.w[x >> 5] >> (x & 31) & 1u) Wt[e] = mk(EXX_RC(0.0), EXX_RC(0.0));
+    }
 }
 
 // inverse second half: work box p -> natural box p of out_base (second inverse y step, inverse z)
@@ -554,7 +590,32 @@ struct Launch {
         return EXX_OK;
     }
     // plain transforms of nbox boxes: forward natural in -> F layout in work; inverse F layout in work -> natural out
-    static int fft_forward(exx_ctx* c, const cplx* in_base, int nbox, cplx* work) {
+    static RowMask all_rows() {
+        RowMask m;
+        for (int i = 0; i < 4; i++) m.w[i] = 0u;
+        for (int x = 0; x < N; x++) m.w[x >> 5] |= 1u << (x & 31);  // exactly N bits: the kernel counts them for its transfer size
+        return m;
+    }
+    // F-layout x rows that hold frequencies |kx| <= gmax
+    static RowMask sphere_rows(int gmax) {
+        RowMask m;
+        for (int i = 0; i < 4; i++) m.w[i] = 0u;
+        for (int kx = 0; kx < N; kx++) {
+            const int g = 2 * kx < N ? kx : kx - N;
+            if (g >= -gmax && g <= gmax) {
+                const int xpos = 8 * (kx % R1) + kx / R1;
+                m.w[xpos >> 5] |= 1u << (xpos & 31);
+            }
+        }
+        return m;
+    }
+    static int zero_rows(exx_ctx* c, cplx* work, int nbox, const RowMask& rows) {
+        LaunchScope ls(c, KC_SCATTER, 0);
+        zero_rows_kernel<R1><<<dim3(R1 * (N / Z), nbox), 256, 0, c->stream>>>(work, rows);
+        EXX_CUDA(c, cudaGetLastError());
+        return EXX_OK;
+    }
+    static int fft_forward(exx_ctx* c, const cplx* in_base, int nbox, cplx* work, const RowMask& rows = all_rows()) {
         const unsigned tiles1 = N * (8 / U1), tiles2 = R1 * (N / Z);
         {
             LaunchScope ls(c, KC_FFT_FUSED, nbox);
@@ -562,16 +623,16 @@ struct Launch {
         }
         {
             LaunchScope ls(c, KC_FFT_FUSED, nbox);
-            fft_b_kernel<R1, -1><<<tiles2 * nbox, FusedCfg<R1>::NT2, smem_b, c->stream>>>(work, nbox);
+            fft_b_kernel<R1, -1><<<tiles2 * nbox, FusedCfg<R1>::NT2, smem_b, c->stream>>>(work, nbox, rows);
         }
         EXX_CUDA(c, cudaGetLastError());
         return EXX_OK;
     }
-    static int fft_inverse(exx_ctx* c, cplx* work, int nbox, cplx* out_base) {
+    static int fft_inverse(exx_ctx* c, cplx* work, int nbox, cplx* out_base, const RowMask& rows = all_rows()) {
         const unsigned tiles3 = N * (8 / U3), tiles2 = R1 * (N / Z);
         {
             LaunchScope ls(c, KC_FFT_FUSED, nbox);
-            fft_b_kernel<R1, +1><<<tiles2 * nbox, FusedCfg<R1>::NT2, smem_b, c->stream>>>(work, nbox);
+            fft_b_kernel<R1, +1><<<tiles2 * nbox, FusedCfg<R1>::NT2, smem_b, c->stream>>>(work, nbox, rows);
         }
         {
             LaunchScope ls(c, KC_FFT_FUSED, nbox);

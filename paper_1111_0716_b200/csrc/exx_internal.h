@@ -105,6 +105,7 @@ struct exx_ctx {
     bool u_valid = false;          // the u cache holds S1 of the psi of the previous call (fused path)
     int64_t opt_energy_route = 0;  // 0 auto (pair-density route E2 where the fused path runs), 1 always E1 from V_x psi
     int64_t energy_route_used = 0;
+    int64_t opt_prune_rows = 1;    // S1/S7 on the fused path: 1 = skip the F-layout x rows outside the spheres (see RowMask)
     int64_t opt_dual = 1;          // pair symmetry: 1 = one dual sweep of pass C per batch (default), 0 = two single sweeps
     int64_t opt_shard_count = 1, opt_shard_rank = 0;  // S8(f)-4: this context runs shard rank of count (exx_shard.h)
 
@@ -188,6 +189,10 @@ struct RJob {
     int tgt[TMAX];
     unsigned gmask[TMAX];
 };
+// F-layout x rows (bit xpos) of a box that a pruned plain transform reads (inverse, S1) or writes (forward, S7)
+struct RowMask {
+    uint32_t w[4];
+};
 // weights of one batch on the energy route: band (a,k) gets  wa[i] * sum_j wb[j] S_ij,  band (b,q) (pair symmetry) the mirror image
 struct EJob {
     double wa[TMAX], wb[TMAX];   // w_k f_a, w_q f_b
@@ -195,7 +200,7 @@ struct EJob {
     int sym, same_k;             // pair symmetry on; k == q (then the pair a == b is counted once)
 };
 int fft_generic_init(exx_ctx* c);
-int launch_scatter(exx_ctx* c, int ik, const double2* coef, int nbatch, double2* box, const int32_t* map = nullptr);  // map: override (F layout)
+int launch_scatter(exx_ctx* c, int ik, const double2* coef, int nbatch, double2* box, const int32_t* map = nullptr, bool clear = true);  // map: override (F layout); clear: zero the boxes first
 int launch_gather(exx_ctx* c, int ik, const double2* box, int nbatch, double2* coef, const int32_t* map = nullptr);
 int launch_fft3d_generic(exx_ctx* c, double2* box, int nbatch, int sign);
 int launch_codensity_tile(exx_ctx* c, const double2* un_base, int n0, int tn, const double2* uq_base, const MTile& mt, double2* work);

@@ -32,9 +32,9 @@ __global__ void gather_kernel(const double2* __restrict__ box, const int32_t* __
         coef[(int64_t)b * npw + ig] = box[(int64_t)b * Ng + map[ig]];
 }
 
-int launch_scatter(exx_ctx* c, int ik, const double2* coef, int nbatch, double2* box, const int32_t* map) {
+int launch_scatter(exx_ctx* c, int ik, const double2* coef, int nbatch, double2* box, const int32_t* map, bool clear) {
     if (!map) map = c->map_dev + c->map_off[ik];
-    EXX_CUDA(c, cudaMemsetAsync(box, 0, sizeof(double2) * (size_t)c->Ng * nbatch, c->stream));
+    if (clear) EXX_CUDA(c, cudaMemsetAsync(box, 0, sizeof(double2) * (size_t)c->Ng * nbatch, c->stream));
     int npw = c->npw[ik];
     for (int b0 = 0; b0 < nbatch; b0 += 32768) {
         int nb = nbatch - b0 < 32768 ? nbatch - b0 : 32768;

@@ -122,7 +122,7 @@ def test_plain_transforms_through_the_passes(emu, R1):
     assert np.linalg.norm(back - want) <= 1e-14 * np.linalg.norm(want)
 
 
-@pytest.mark.parametrize("R1,ta,tb", [(2, 5, 3), (4, 6, 4), (5, 3, 3), (6, 5, 2), (9, 5, 2)])
+@pytest.mark.parametrize("R1,ta,tb", [(2, 5, 3), (4, 6, 4), (5, 3, 3), (6, 5, 2), (9, 5, 2), (10, 3, 2)])
 def test_dual_sweep_equals_definition(emu, R1, ta, tb):
     """The dual sweep of pass C (pair symmetry) on a ragged ta x tb batch with holes: rows get
     acc_a -= sum_j coef_b[j] u_b[j] v_ij, columns get acc_b -= sum_i coef_a[i] u_a[i] conj(v_ij), v_ij = IFFT[K FFT[conj(u_b[j]) u_a[i]]],
@@ -157,6 +157,8 @@ def test_dual_sweep_equals_definition(emu, R1, ta, tb):
     up = C.POINTER(C.c_uint32)
     rc = emu.exx_emu_dual(R1, ta, tb, _p(ua), _p(ub), _p(K), _p(coef_a), _p(coef_b), ev.ctypes.data_as(up), bside.ctypes.data_as(up),
                           amask, _p(acc_a), _p(acc_b))
+    if rc == -2:
+        pytest.skip("no dual kernel for this grid (FusedCfg<R1>::RG = 0: two single sweeps)")
     assert rc == 0
     want_a, want_b = np.zeros_like(acc_a), np.zeros_like(acc_b)
     for i in range(ta):

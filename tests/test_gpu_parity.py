@@ -773,6 +773,46 @@ def test_fft3d_fused_refuses_unsupported_grids(B):
     g.close()
 
 
+@pytest.mark.parametrize("n", [72, 48])
+def test_fused_small_batches_dual_and_two_sweeps(B, n):
+    """The fused kernels of the benchmarked instantiation (N = 72: R1 = 9, dual sweep with 4 rows per CTA; N = 48: R1 = 6) on a
+    problem small enough for the full oracle and for compute-sanitizer (profiles/r2_sanitizer.md): 5 bands cut into 3 x 3 batches
+    (a diagonal batch, an off-diagonal one, a ragged last one), an empty band and a half-filled one, pair symmetry with the dual
+    sweep and with two sweeps, and no symmetry."""
+    w = W.custom("small%d" % n, 7200 + n, (n, n, n), W.cubic(10.0), [[0, 0, 0]], [1.0], 6.0, 5, [1.0, 1.0, 0.5, 0.0, 1.0])
+    o, g = _pair(B, w)
+    psi = w.coefficients(o.npw)
+    want = o.apply(psi, w.occ)
+    e_want, pb_want = o.energy(psi, w.occ, want)
+    pd = g.to_device(psi)
+    g.set_option(B.EXX_OPT_PRUNE, 0)
+    g.set_option(B.EXX_OPT_TILE_N, 3)
+    g.set_option(B.EXX_OPT_TILE_M, 3)
+    outs = []
+    import torch
+    pad = 4096
+    guard = torch.full((g.ncoef + 2 * pad,), float("nan"), dtype=torch.complex128, device="cuda")   # `out` between NaN canaries
+    for sym, dual in ((1, 1), (1, 0), (0, 1)):
+        g.set_option(B.EXX_OPT_SYMMETRY, sym)
+        g.set_option(B.EXX_OPT_DUAL_SWEEP, dual)
+        out = g.apply(pd, w.occ, guard[pad:pad + g.ncoef])
+        torch.cuda.synchronize()
+        assert bool(torch.isnan(guard[:pad].real).all()) and bool(torch.isnan(guard[pad + g.ncoef:].real).all())   # nothing written outside out
+        assert not bool(torch.isnan(out.real).any())
+        assert g.get_info(B.EXX_INFO_PATH_USED) == 2 and g.get_info(B.EXX_INFO_WORK_GRID) == n and g.get_info(B.EXX_INFO_SYMMETRY) == sym
+        assert g.get_info(B.EXX_INFO_PAIRS_ORDERED) == w.pair_evals
+        got = out.cpu().numpy()
+        for b in range(w.nbands):
+            assert _rel(o.band(got, 0, b), o.band(want, 0, b)) < TOL_VX, (n, sym, dual, b)
+        e, pb = g.energy(pd, w.occ, out)
+        assert abs(e - e_want) <= TOL_EX * abs(e_want) and np.abs(pb - pb_want).max() <= TOL_EX * abs(e_want)
+        outs.append(got)
+        out2 = g.apply(pd, w.occ)                       # fixed summation order: bit-identical from run to run
+        assert np.array_equal(out2.cpu().numpy(), got)
+    assert _rel(outs[0], outs[1]) < 1e-13 and _rel(outs[0], outs[2]) < 1e-13
+    g.close()
+
+
 def test_fused_degenerate_cases(B):
     """Fused path edge cases: a single band, all occupations zero, one occupied band among empties."""
     import torch

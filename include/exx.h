@@ -146,7 +146,8 @@ int exx_get_option(const exx_ctx* ctx, int option, int64_t* value);
 int exx_get_info(const exx_ctx* ctx, int what, int64_t* value);
 /* Per kernel class `kclass` (0 .. EXX_INFO_NUM_KERNEL_CLASSES-1), for the most recent exx_apply: launch count, work
  * units (generic kernels and fused_fft_pass: box passes, i.e. one read + one write of an FFT box; fused passes A/B: band pairs;
- * fused pass C: accumulation sweeps, one per pair and side), and — with
+ * fused pass C: accumulation sweeps, one per pair and side — or, for the dual sweep of EXX_OPT_DUAL_SWEEP, pair boxes, each serving
+ * both sides; fused pass R: partial boxes added to the accumulators), and — with
  * EXX_OPT_PROFILE = 1 — the device time from CUDA events on the context's stream (0 otherwise).  Synchronises.
  * exx_kernel_class_name gives the class name (static string, NULL if out of range). */
 int exx_get_kernel_time(exx_ctx* ctx, int kclass, double* ms_total, int64_t* launches, int64_t* units);
@@ -157,7 +158,10 @@ const char* exx_kernel_class_name(int kclass);
  * (tile = 0: the default, 32 for one shard and 16 for several; at most 32); batches are handed out longest first to the least loaded shard — deterministic, so every rank
  * computes the same plan.  occ_host: nk*nbands.  symmetry: as EXX_OPT_SYMMETRY (the caller says whether it applies).
  * Outputs (each nshards entries, either may be NULL): pairs_out = pair densities the shard transforms (passes A, B);
- * passes_out = fused pass executions (2 per pair + 1 per accumulation sweep), the load that is balanced. */
+ * passes_out = fused pass executions (2 per pair + 1 per accumulation sweep), the load that is balanced.
+ * The plan describes what a context runs only when `tile` is the tile that context uses: a context may shrink its tile below the
+ * default (pair workspace cap on grids of 128^3 and more, EXX_OPT_TILE_N/M), so pass the value EXX_INFO_TILE_N reports after an
+ * apply when the counts must match a particular context (totals over all shards do not depend on the tile). */
 int exx_shard_plan(int nk, int nbands, const double* occ_host, int symmetry, int tile, int nshards, int64_t* pairs_out, int64_t* passes_out);
 
 /* V_x applied to every band: out(k,n,:) = (V_x c)_nk.  psi_dev/out_dev: device, exx_psi_offset(nk) complex elements

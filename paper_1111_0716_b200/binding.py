@@ -159,6 +159,7 @@ class Exx:
         kw = np.ascontiguousarray(kweight, dtype=np.float64)
         kp = KernelParams(int(kind), float(mu), float(scale))
         self.stream = stream if stream is not None else torch.cuda.current_stream()
+        self.device = torch.cuda.current_device()   # libexx enqueues everything on this device's stream `self.stream`
         self._h = C.c_void_p()
         g = (C.c_int * 3)(*self.grid)
         rc = L.exx_create(C.byref(self._h), g, _dp(lat), self.nk, _dp(kf), _dp(kw), float(ecut), C.byref(kp), self.nbands,
@@ -232,6 +233,12 @@ class Exx:
     # ---- device helpers (torch = memory only)
     def _dev(self, t, nelem):
         torch = self._torch
+        # the library orders its work on the creation stream only: a call made under another torch stream (or device) would race
+        # with the producers/consumers of its tensors, so it is refused rather than silently unordered
+        if torch.cuda.current_device() != self.device or t.device.index != self.device:
+            raise RuntimeError("this Exx context lives on cuda:%d; call it with that device current and tensors on it" % self.device)
+        if torch.cuda.current_stream().cuda_stream != self.stream.cuda_stream:
+            raise RuntimeError("call Exx on its creation stream (torch.cuda.stream(ctx.stream)): libexx enqueues on that stream only")
         assert t.is_cuda and t.dtype == torch.complex128 and t.is_contiguous() and t.numel() == nelem, \
             "expected a contiguous complex128 CUDA tensor with %d elements" % nelem
         return C.c_void_p(t.data_ptr())

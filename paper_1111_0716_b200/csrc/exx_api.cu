@@ -381,9 +381,17 @@ static int create_impl(exx_ctx** out, const int grid[3], const double lattice[9]
 // the buffers that scale with nbands * Ng: real-space cache, pair workspace, accumulators, fused tables
 static int ensure_big(exx_ctx* c) {
     if (c->big_alloc) return EXX_OK;
+    // a failure part-way (out of memory) frees what this call allocated, so that a retry starts clean instead of leaking
+    auto undo = [&](int code) {
+        if (c->fused) fused_destroy(c);
+        cudaFree(c->u_dev), cudaFree(c->work_dev), cudaFree(c->acc_dev);
+        c->u_dev = c->work_dev = c->acc_dev = nullptr;
+        c->work_boxes = c->acc_boxes = 0;
+        return code;
+    };
     int rc;
     int nbt = c->nk * c->nb;
-    if ((rc = dev_alloc(c, &c->u_dev, (size_t)nbt * c->Ng))) return rc;
+    if ((rc = dev_alloc(c, &c->u_dev, (size_t)nbt * c->Ng))) return undo(rc);
     // generic pipeline: one n at a time, up to 16 m per tile, at most ~1 GiB of pair workspace;
     // fused pipeline: tn x tm pairs per batch (work) and tn accumulators
     size_t box_bytes = sizeof(double2) * (size_t)c->Ng;
@@ -396,10 +404,10 @@ static int ensure_big(exx_ctx* c) {
         c->acc_boxes = (size_t)c->nk * c->nb;  // the fused loop nest keeps one accumulator per (k, band)
         c->work_boxes = std::max<size_t>(wb, (size_t)tn * tm);
     }
-    if ((rc = dev_alloc(c, &c->work_dev, c->work_boxes * c->Ng))) return rc;
-    if ((rc = dev_alloc(c, &c->acc_dev, c->acc_boxes * c->Ng))) return rc;
+    if ((rc = dev_alloc(c, &c->work_dev, c->work_boxes * c->Ng))) return undo(rc);
+    if ((rc = dev_alloc(c, &c->acc_dev, c->acc_boxes * c->Ng))) return undo(rc);
     if (fused_supported(c))
-        if ((rc = fused_create(c))) return rc;
+        if ((rc = fused_create(c))) return undo(rc);
     c->big_alloc = true;
     return EXX_OK;
 }

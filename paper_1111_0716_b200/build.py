@@ -3,6 +3,14 @@
     python -m paper_1111_0716_b200.build [--force]
 
 nvcc cross-compiles without a GPU.  The built library sits next to this file so that it travels with the repo.
+
+Build knobs (supported, for tuning sweeps on a new GPU; libexx.so itself is always built without them): a variant library is
+built with `build(extra=["-D..."], out="/some/libexx_variant.so")` and loaded by setting EXX_LIB to its path.
+    -DEXX_TUNE_R1=<R1> with any of -DEXX_TUNE_{U1,NT1,U3,NT3,NT2,MINB1,MINB2,MINB3,TWREG,ACCREG,STAGE3}=<v>
+                          launch geometry of the fused passes for the grid N = 8 R1 (FusedCfg in csrc/exx_fused_phases.h)
+    -DEXX_STAGE3_ALL=<0|1|2>   cp.async staging level of pass C for every grid
+    -DEXX_DUAL_RG_ALL=<0|1|2|4>  rows per CTA of the dual sweep for every grid (0 = two single sweeps)
+    -DEXX_DEFAULT_TILE=<n>, -DEXX_SHARD_TILE=<n>, -DEXX_WORK_CAP_GIB=<n>   batch tiles and the pair-workspace cap (csrc/exx_internal.h)
 """
 import hashlib
 import os

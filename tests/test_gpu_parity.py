@@ -222,6 +222,9 @@ def _check_golden(B, name, live_rows=0, prune=1, symmetry=1, dual=1):
                 for n in range(w.nbands):
                     pr = gold["per_band_probe"][k * w.nbands + n]
                     assert abs(np.vdot(z, g.band(got, k, n)) - complex(pr[0], pr[1])) <= TOL_VX * gold["per_band_norm"][k * w.nbands + n], (name, k, n)
+    elif "E_x_E2" in gold:
+        # rows only plus the oracle's total energy by its second route (E2, forward transforms only: tests/golden/make_golden.py C5:e2)
+        assert abs(e - gold["E_x_E2"]) <= TOL_EX * abs(gold["E_x_E2"])
     # properties that hold at any size
     assert e < 0 and abs(pb.sum() - e) <= 1e-13 * abs(e) and np.all(pb <= 0)
     assert g.get_info(B.EXX_INFO_PAIRS_ORDERED) == w.pair_evals

@@ -60,3 +60,26 @@ def test_reference_arm_runs_on_rank0_only():
     line = json.loads(r.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["unit"] == "pair-evals/s" and line["value"] > 0
     assert line["cpu_baseline"]["kind"] == "oracle" and line["e2e"]["h2d_bytes_per_step"] == 0
+
+
+def test_ncu_counters_are_refused_for_another_build(tmp_path, monkeypatch):
+    """bench.py prints roofline.traffic / dram_frac / fp64_frac only from an ncu capture of the build it is running: a capture whose
+    recorded source hash differs from libexx.so's stamp (or of another work grid) is refused with the reason, never rescaled."""
+    sys.path.insert(0, ROOT)
+    import bench
+    cap = {"source": "test", "srchash": "abc", "work_grid": 72, "units_per_launch": {"fused_pass_a": 1},
+           "dram_bytes_per_launch": {"fused_pass_a": 1.0}, "fp64_flops_per_launch": {"fused_pass_a": 1.0}}
+    p = tmp_path / "cap.json"
+    p.write_text(json.dumps(cap))
+    monkeypatch.setattr(bench, "NCU_COUNTERS", str(p))
+    monkeypatch.setattr(bench, "lib_source_hash", lambda: "abc")
+    got, why = bench.ncu_counters(72 ** 3)
+    assert got is not None and got["srchash"] == "abc" and "ncu_counters" in why
+    got, why = bench.ncu_counters(96 ** 3)
+    assert got is None and "work grid" in why
+    monkeypatch.setattr(bench, "lib_source_hash", lambda: "other")
+    got, why = bench.ncu_counters(72 ** 3)
+    assert got is None and "another build" in why
+    monkeypatch.setattr(bench, "NCU_COUNTERS", str(tmp_path / "missing.json"))
+    got, why = bench.ncu_counters(72 ** 3)
+    assert got is None and "no capture" in why

@@ -816,6 +816,35 @@ def test_fused_small_batches_dual_and_two_sweeps(B, n):
     g.close()
 
 
+def test_sphere_pruned_transforms_are_bit_identical(B):
+    """EXX_OPT_PRUNE_SPHERE (S1 reads / S7 writes only the x rows of the frequency box that can hold sphere coefficients) changes
+    no bit of V_x psi or E_x, with k-points (spheres shifted per k: the row mask is the union) and on a compact work grid."""
+    for w in (W.custom("prune48", 4811, (48, 48, 48), W.rhombohedral(8.0, 64.0), [[0.25, 0.25, 0.25], [-0.25, 0.25, 0.0]], [0.5, 0.5], 6.0, 4,
+                       [1.0, 1.0, 0.5, 0.0]), W.make("C2")):
+        o, g = _pair(B, w)
+        psi = w.coefficients(o.npw)
+        pd = g.to_device(psi)
+        res = []
+        for val in (1, 0):
+            g.set_option(B.EXX_OPT_PRUNE_SPHERE, val)
+            assert g.get_option(B.EXX_OPT_PRUNE_SPHERE) == val
+            out = g.apply(pd, w.occ)
+            res.append((out.cpu().numpy(), g.energy(pd, w.occ, out)[0], g.energy(pd, w.occ, None)[0]))
+        assert np.array_equal(res[0][0], res[1][0]) and res[0][1] == res[1][1] and res[0][2] == res[1][2]
+        if w.name != "C2":
+            want = o.apply(psi, w.occ)
+            for k in range(w.nk):
+                for n in range(w.nbands):
+                    assert _rel(o.band(res[0][0], k, n), o.band(want, k, n)) < TOL_VX
+        g.close()
+
+
+def test_measured_fp64_peak_is_plausible(B):
+    """exx_measure_fp64_peak (bench.py's fp64 roofline denominator): a B200 delivers 25-40 TFLOP/s of fp64 FMA depending on its clocks."""
+    gf = B.measure_fp64_peak()
+    assert 1.0e4 < gf < 6.0e4, gf
+
+
 def test_fused_degenerate_cases(B):
     """Fused path edge cases: a single band, all occupations zero, one occupied band among empties."""
     import torch

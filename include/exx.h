@@ -59,7 +59,9 @@ enum {
     EXX_ERR_ALLOC = -7,       /* host or device allocation failed */
     EXX_ERR_CUDA = -8,        /* a CUDA call or kernel launch failed; see exx_last_error */
     EXX_ERR_BAD_ARG = -9,     /* index out of range, nk/nbands < 1, weights not finite, unknown option */
-    EXX_ERR_ALIAS = -10       /* out aliases psi */
+    EXX_ERR_ALIAS = -10,      /* out aliases psi */
+    EXX_ERR_LIMIT = -11       /* a size is beyond the fixed capacity of an entry point that allocates nothing (exx_subspace_static);
+                                 exx_last_error(NULL) names the limit */
 };
 
 /* Options (exx_set_option / exx_get_option).  All but EXX_OPT_PRECISION are tuning knobs: results differ only by rounding
@@ -199,6 +201,33 @@ int exx_subspace(exx_ctx* ctx, int ik, const double* psi_dev, const double* vxps
  * m_dev[i*nphi + j] = sum_g conj(phi_i(g)) vphi_j(g) within k-point ik, nphi x nphi complex128, row-major, device — the projected
  * operator <phi_i|V_x|phi_j> an iterative eigensolver builds from exx_apply_to's output.  Asynchronous. */
 int exx_subspace_block(exx_ctx* ctx, int ik, const double* phi_dev, const double* vphi_dev, int nphi, double* m_dev);
+
+/* The subspace matrix once more, for callers that must not allocate device memory:  m_dev[i*nvec + j] = sum_g conj(a_i(g)) b_j(g),
+ * nvec x nvec complex128, row-major.  Needs no context (exx_create allocates), and calls no cudaMalloc, cudaFree or any other
+ * allocating routine, on any call, successful or not.
+ *   Who needs this: a program whose GPU memory is wholly managed by someone else — a framework's caching pool that has reserved the
+ *   card, a job held to a fixed memory budget — where an allocation made behind the owner's back fails or steals what was promised
+ *   elsewhere; and a latency-critical loop that cannot take the device-wide synchronisation cudaMalloc and cudaFree bring.
+ *   Everyone else should call exx_subspace / exx_subspace_block, which have no size limit.
+ * a_dev, b_dev: nvec vectors of npw complex128 each, vector i at element i*npw (for one k-point of the packed psi / V_x psi arrays:
+ * the pointers psi_dev + 2*exx_psi_offset(ik) doubles, with npw = exx_npw(ik)); m_dev: nvec*nvec complex128; all three are device
+ * pointers on the CURRENT device, 16-byte aligned, owned by the caller; inputs are only read, m_dev may not overlap them.
+ * cuda_stream: a cudaStream_t of the current device cast to void* (NULL = default stream).  Asynchronous on that stream.
+ *   The split-K scratch of the ZGEMM lives in a fixed array inside the library image: EXX_STATIC_SCRATCH_BYTES of every GPU that
+ *   loads libexx stay occupied until the process exits, whether this call is used or not.  Hence the limits: 1 <= nvec <=
+ *   EXX_STATIC_MAX_NVEC and 1 <= npw <= EXX_STATIC_MAX_NPW; beyond them the call returns EXX_ERR_LIMIT, launches nothing and leaves
+ *   m_dev untouched (exx_last_error(NULL) then says which limit).
+ *   The first call a process makes with a given device current looks up that device's address of the array (and may make the CUDA
+ *   runtime load the library's kernels onto it): make that first call during set-up, outside any stream capture.
+ *   All calls on one device share the one array.  Nothing in it has to start at zero — each call overwrites every element it later
+ *   reads — so calls that follow one another on a stream, or are otherwise ordered, are independent.  Two calls whose kernels may
+ *   run at the same time on one GPU (different streams without an event between them, or two host threads) race on the array and
+ *   both results are garbage: order them.
+ * Deterministic (fixed slice order); agrees with exx_subspace to rounding order (the number of slices may differ). */
+#define EXX_STATIC_SCRATCH_BYTES (8 << 20) /* 8 MiB: 8 slices at nvec = 256, 20 at nvec = 160 */
+#define EXX_STATIC_MAX_NVEC 256
+#define EXX_STATIC_MAX_NPW (1 << 24)
+int exx_subspace_static(const double* a_dev, const double* b_dev, int nvec, int64_t npw, double* m_dev, void* cuda_stream);
 
 /* Same as exx_apply (+ exx_energy when ex_host_or_null != NULL) on HOST buffers: copies psi to the device, applies,
  * copies out back; synchronises.  Pinned host memory makes the copies asynchronous, pageable memory works too. */

@@ -28,7 +28,8 @@ EXX_INFO_ENERGY_ROUTE = 16
 SYMBOLS = ("exx_create", "exx_destroy", "exx_npw", "exx_index_map", "exx_psi_offset", "exx_set_option", "exx_get_option",
            "exx_get_info", "exx_get_kernel_time", "exx_kernel_class_name", "exx_apply", "exx_energy", "exx_apply_host",
            "exx_scatter", "exx_gather", "exx_fft3d", "exx_to_real", "exx_kernel_table", "exx_strerror", "exx_last_error",
-           "exx_version", "exx_subspace", "exx_fft3d_fused", "exx_findex", "exx_shard_plan", "exx_apply_to", "exx_subspace_block", "exx_measure_fp64_peak")
+           "exx_version", "exx_subspace", "exx_fft3d_fused", "exx_findex", "exx_shard_plan", "exx_apply_to", "exx_subspace_block", "exx_measure_fp64_peak",
+           "exx_subspace_static")
 
 
 class KernelParams(C.Structure):
@@ -100,6 +101,7 @@ def lib():
         L.exx_last_error.restype = C.c_char_p
         L.exx_version.restype = C.c_int
         L.exx_measure_fp64_peak.argtypes = [vp, dp]
+        L.exx_subspace_static.argtypes = [vp, vp, C.c_int, C.c_int64, vp, vp]
         _lib = L
     return _lib
 
@@ -130,6 +132,38 @@ def measure_fp64_peak(stream=None):
     if rc:
         raise ExxError(rc)
     return g.value
+
+
+EXX_ERR_LIMIT = -11
+STATIC_MAX_NVEC, STATIC_MAX_NPW, STATIC_SCRATCH_BYTES = 256, 1 << 24, 8 << 20
+
+
+def subspace_static(a_dev, b_dev, m_dev=None, stream=None):
+    """exx_subspace_static: M[i, j] = sum_g conj(a[i, g]) b[j, g] for two (nvec, npw) complex128 CUDA tensors, without any device
+    allocation inside the library (for processes whose GPU memory belongs to another allocator, or that cannot take cudaMalloc's
+    device-wide synchronisation).  Pass m_dev (nvec x nvec complex128) to keep this wrapper from allocating the result either.  The
+    scratch is one fixed 8 MiB array per GPU shared by all calls: nvec <= 256, npw <= 2^24 (ExxError code -11 beyond), and calls
+    that may overlap on the GPU race — keep them ordered.  Make the first call on a device before any stream capture."""
+    import torch
+    assert a_dev.is_cuda and b_dev.is_cuda and a_dev.dtype == b_dev.dtype == torch.complex128
+    assert a_dev.dim() == 2 and a_dev.shape == b_dev.shape and a_dev.is_contiguous() and b_dev.is_contiguous()
+    if a_dev.device.index != torch.cuda.current_device() or b_dev.device != a_dev.device:
+        raise RuntimeError("subspace_static works on the current device: make cuda:%d current" % a_dev.device.index)
+    nvec, npw = int(a_dev.shape[0]), int(a_dev.shape[1])
+    L = lib()
+    if (nvec > STATIC_MAX_NVEC or npw > STATIC_MAX_NPW) and m_dev is None:
+        # let the library refuse (same error as with a caller-provided m_dev) without allocating a result first
+        rc = L.exx_subspace_static(C.c_void_p(a_dev.data_ptr()), C.c_void_p(b_dev.data_ptr()), nvec, npw, C.c_void_p(a_dev.data_ptr()), None)
+        raise ExxError(rc, L.exx_last_error(None).decode())
+    if m_dev is None:
+        m_dev = torch.empty((nvec, nvec), dtype=torch.complex128, device=a_dev.device)
+    assert m_dev.is_cuda and m_dev.dtype == torch.complex128 and m_dev.is_contiguous() and m_dev.numel() == nvec * nvec
+    st = stream if stream is not None else torch.cuda.current_stream()
+    rc = L.exx_subspace_static(C.c_void_p(a_dev.data_ptr()), C.c_void_p(b_dev.data_ptr()), nvec, npw, C.c_void_p(m_dev.data_ptr()),
+                               C.c_void_p(st.cuda_stream))
+    if rc:
+        raise ExxError(rc, L.exx_last_error(None).decode())
+    return m_dev
 
 
 def all_reduce_sum(t, group=None):

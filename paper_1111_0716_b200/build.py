@@ -21,7 +21,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libexx.so")
 STAMP = LIB + ".srchash"   # hash of what LIB was built from (git-ignored like the library, travels with it)
-SOURCES = ["exx_api.cu", "exx_kernels.cu", "exx_fused.cu", "exx_subspace.cu"]
+SOURCES = ["exx_api.cu", "exx_kernels.cu", "exx_fused.cu", "exx_subspace.cu", "exx_static.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--fmad=true",
               "-Xcompiler", "-fPIC,-ffp-contract=off,-Wall,-Wno-unknown-pragmas", "-shared", "-cudart", "shared", "--threads", "4"]
 

@@ -169,6 +169,7 @@ const char* exx_strerror(int code) {
     case EXX_ERR_CUDA: return "CUDA error";
     case EXX_ERR_BAD_ARG: return "bad argument";
     case EXX_ERR_ALIAS: return "out aliases psi";
+    case EXX_ERR_LIMIT: return "size beyond the fixed capacity of a no-allocation entry point";
     default: return "unknown error";
     }
 }

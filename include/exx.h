@@ -23,8 +23,16 @@
  *       exx_psi_offset(k) + n*npw(k) + ig   (complex elements),  exx_psi_offset(k) = nbands * sum_{k'<k} npw(k').
  *   - pointers named *_dev are device (HBM) pointers, *_host are host pointers; both are owned by the caller.
  *     The context owns its index maps, kernel tables, the real-space cache u_nk(r) and all workspaces; they are
- *     allocated in exx_create and freed in exx_destroy.  exx_apply allocates nothing, except the first apply after
- *     EXX_OPT_PRUNE was switched off on a context that has a compact work grid (the full-grid buffers are made then).
+ *     allocated in exx_create and freed in exx_destroy, and the calls allocate nothing — with these exceptions, each made on
+ *     first use, kept until exx_destroy and counted in EXX_INFO_WORKSPACE_BYTES:
+ *       - exx_apply / exx_energy: the first call that runs the dual sweep (pair symmetry, EXX_OPT_DUAL_SWEEP = 1, a grid with a
+ *         dual kernel) makes its partial boxes (at most tile_n/RG x tile_m boxes; if the device refuses, two sweeps run instead);
+ *         the first call after EXX_OPT_PRUNE was switched off on a context with a compact work grid makes the full-grid buffers;
+ *         the first call with EXX_OPT_PRECISION = 1 makes the fp32 copies of u_nk(r) and of the kernel tables;
+ *       - exx_apply_to: boxes and accumulators of the trial vectors (again when nphi grows);
+ *       - exx_subspace / exx_subspace_block: the split-K partial matrices (again when they grow);
+ *       - exx_apply_host: one device copy of psi.
+ *     exx_subspace_static never allocates.
  *   - every call returns EXX_OK (0) or a negative error code; no exceptions, no abort, nothing printed.
  *     On error, output arguments are left untouched.  exx_last_error() gives detail for EXX_ERR_CUDA.
  *   - work is enqueued on the CUDA stream given to exx_create (a cudaStream_t cast to void*; NULL = default
@@ -95,7 +103,11 @@ enum {
                                accumulations (acc_a -= w_q f_b u_b v on chip, acc_b -= w_k f_a u_a conj(v) through one partial box per
                                (row group, column) that a small reduction kernel adds in a fixed order); 0: two sweeps of the last
                                pass, the second repeating the inverse y/z steps (grids without a dual kernel always do this).
-                               Results differ by rounding order only; both are deterministic */
+                               Results differ by rounding order only (fp64 mode); both are deterministic.  With EXX_OPT_PRECISION = 1
+                               the dual sweep adds the second side's products of one row group (at most 4 rows) in fp32 before they
+                               reach the fp64 accumulators, where two sweeps add each product in fp64: there the two differ at fp32
+                               rounding level, inside that mode's 1e-5 bar.  The partial boxes are allocated by the first apply
+                               that uses them; if the device refuses them, two sweeps run */
     EXX_OPT_PRUNE_SPHERE = 14, /* fused path, S1 and S7 ("the sphere is ~2 % of the box").  1 (default): the inverse
                                transform of the bands reads, and the forward transform of the accumulators writes, only the
                                x rows of the frequency box with |g_x| <= max |g_x| of the spheres (46 % of the rows at C4a); the
@@ -241,7 +253,7 @@ int exx_scatter(exx_ctx* ctx, int ik, const double* coef_dev, int nbatch, double
 int exx_gather(exx_ctx* ctx, int ik, const double* box_dev, int nbatch, double* coef_dev);
 int exx_fft3d(exx_ctx* ctx, double* box_dev, int nbatch, int sign);
 int exx_to_real(exx_ctx* ctx, int ik, const double* coef_dev, int nbatch, double* box_dev);
-/* Stand-alone batched 3-D transform through the fused passes (cubic N = 48, 64, 72, 96, 128; EXX_ERR_BAD_GRID otherwise): two
+/* Stand-alone batched 3-D transform through the fused passes (cubic N = 16, 32, 40, 48, 64, 72, 80, 96, 128; EXX_ERR_BAD_GRID otherwise): two
  * passes per transform instead of the three of exx_fft3d.  The frequency side lives in the library's "F layout":
  * exx_findex gives, for every natural C-order frequency index ((kx*N + ky)*N + kz), its position in an F-layout box.
  *   sign = -1: in_dev natural-order boxes (unchanged) -> out_dev F-layout boxes, unnormalised forward transform

@@ -193,11 +193,14 @@ class Exx:
         kw = np.ascontiguousarray(kweight, dtype=np.float64)
         kp = KernelParams(int(kind), float(mu), float(scale))
         self.stream = stream if stream is not None else torch.cuda.current_stream()
-        self.device = torch.cuda.current_device()   # libexx enqueues everything on this device's stream `self.stream`
+        # libexx enqueues everything on `self.stream`; the context lives on that stream's device (which need not be the current one
+        # when the caller hands in a stream), so it is created with that device current
+        self.device = self.stream.device.index if getattr(self.stream, "device", None) is not None else torch.cuda.current_device()
         self._h = C.c_void_p()
         g = (C.c_int * 3)(*self.grid)
-        rc = L.exx_create(C.byref(self._h), g, _dp(lat), self.nk, _dp(kf), _dp(kw), float(ecut), C.byref(kp), self.nbands,
-                          C.c_void_p(self.stream.cuda_stream))
+        with torch.cuda.device(self.device):
+            rc = L.exx_create(C.byref(self._h), g, _dp(lat), self.nk, _dp(kf), _dp(kw), float(ecut), C.byref(kp), self.nbands,
+                              C.c_void_p(self.stream.cuda_stream))
         if rc:
             raise ExxError(rc, L.exx_last_error(None).decode())
         self.npw = []

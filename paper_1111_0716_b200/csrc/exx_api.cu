@@ -2,6 +2,7 @@
 // workspaces), the loop nest over k, q, n-tiles, m-tiles, and the generic pipeline S1..S8.
 // Product code: shares nothing with oracle/.
 #include <math.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -15,6 +16,10 @@ namespace exx {
 
 static thread_local std::string g_thread_error;
 void set_thread_error(const std::string& s) { g_thread_error = s; }
+bool test_fail_alloc(const char* tag) {
+    const char* v = getenv("EXX_TEST_FAIL_ALLOC");
+    return v && !strcmp(v, tag);
+}
 
 int cuda_fail(exx_ctx* c, cudaError_t e, const char* what) {
     std::string s = std::string(what) + ": " + cudaGetErrorName(e) + " (" + cudaGetErrorString(e) + ")";
@@ -116,9 +121,9 @@ static void free_ctx(exx_ctx* c) {
 }
 
 template <typename T>
-static int dev_alloc(exx_ctx* c, T** p, size_t count) {
+static int dev_alloc(exx_ctx* c, T** p, size_t count, const char* test_tag = nullptr) {
     size_t bytes = sizeof(T) * (count ? count : 1);
-    cudaError_t e = cudaMalloc((void**)p, bytes);
+    cudaError_t e = (test_tag && test_fail_alloc(test_tag)) ? cudaErrorMemoryAllocation : cudaMalloc((void**)p, bytes);
     if (e != cudaSuccess) {
         cudaGetLastError();
         c->last_error = "cudaMalloc of " + std::to_string(bytes) + " bytes failed";
@@ -383,11 +388,13 @@ static int create_impl(exx_ctx** out, const int grid[3], const double lattice[9]
 static int ensure_big(exx_ctx* c) {
     if (c->big_alloc) return EXX_OK;
     // a failure part-way (out of memory) frees what this call allocated, so that a retry starts clean instead of leaking
+    const size_t bytes_before = c->dev_bytes;
     auto undo = [&](int code) {
         if (c->fused) fused_destroy(c);
         cudaFree(c->u_dev), cudaFree(c->work_dev), cudaFree(c->acc_dev);
         c->u_dev = c->work_dev = c->acc_dev = nullptr;
         c->work_boxes = c->acc_boxes = 0;
+        c->dev_bytes = bytes_before;  // EXX_INFO_WORKSPACE_BYTES counts what the context holds, not what it once tried to get
         return code;
     };
     int rc;
@@ -406,7 +413,7 @@ static int ensure_big(exx_ctx* c) {
         c->work_boxes = std::max<size_t>(wb, (size_t)tn * tm);
     }
     if ((rc = dev_alloc(c, &c->work_dev, c->work_boxes * c->Ng))) return undo(rc);
-    if ((rc = dev_alloc(c, &c->acc_dev, c->acc_boxes * c->Ng))) return undo(rc);
+    if ((rc = dev_alloc(c, &c->acc_dev, c->acc_boxes * c->Ng, "acc"))) return undo(rc);
     if (fused_supported(c))
         if ((rc = fused_create(c))) return undo(rc);
     c->big_alloc = true;

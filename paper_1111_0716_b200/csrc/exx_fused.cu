@@ -38,8 +38,10 @@ struct FusedState {
     cplx* uphi_dev = nullptr;
     size_t uphi_boxes = 0;
     // dual sweep of pass C (pair symmetry): partial boxes of the second side, one per (row group, column) of a batch
+    // (allocated by fused_ensure_part before the first dual sweep; an allocation that failed is remembered and not retried at that size)
     cplx* part_dev = nullptr;
     size_t part_boxes = 0;
+    size_t part_refused = 0;
 };
 
 #define EXX_DISPATCH_R1(R1v, EXPR)                  \
@@ -119,18 +121,6 @@ int fused_create(exx_ctx* c) {
             return EXX_ERR_ALLOC;
         }
         c->dev_bytes += sizeof(double) * (TMAX * TMAX * (tiles2 + 1) + (size_t)c->nk * c->nb);
-    }
-    int rg = 0;
-    EXX_DISPATCH_R1(st->R1, rg = L::RG);
-    if (rg > 0 && c->alias_free) {  // the pair symmetry (and with it the dual sweep) only ever runs on alias-free grids
-        int tn, tm;
-        fused_tiles(c, &tn, &tm);
-        st->part_boxes = (size_t)((tn + rg - 1) / rg) * tm;
-        if (cudaMalloc((void**)&st->part_dev, sizeof(cplx) * Ng * st->part_boxes) != cudaSuccess) {
-            cudaGetLastError();
-            return EXX_ERR_ALLOC;
-        }
-        c->dev_bytes += sizeof(cplx) * Ng * st->part_boxes;
     }
     int rc = EXX_OK;
     EXX_DISPATCH_R1(st->R1, rc = L::init(c));
@@ -460,6 +450,34 @@ static int fused_u_cache(exx_ctx* c, FusedState* st, const double2* psi, cplx* u
     return EXX_OK;
 }
 
+// The partial boxes of the dual sweep, one per (row group, column) of a ta_max x tb_max batch, are made here, right before the first
+// apply that can use them (pair symmetry on, EXX_OPT_DUAL_SWEEP on, a grid with a dual kernel) — never for contexts that run without
+// the symmetry or with two sweeps.  They come on top of the pair workspace EXX_WORK_CAP_GIB bounds (at most 1/RG of it: 0.25x at
+// 72^3, 0.5x at 96^3).  If the device cannot give them the apply is not refused: pair_loop sees no buffer and runs two sweeps.
+static int fused_ensure_part(exx_ctx* c, FusedState* st, bool sym, int ta_max, int tb_max) {
+    int rg = 0;
+    EXX_DISPATCH_R1(st->R1, rg = L::RG);
+    if (!sym || !c->opt_dual || rg <= 0) return EXX_OK;
+    const size_t Ng = (size_t)c->Ng;
+    const size_t need = (size_t)((ta_max + rg - 1) / rg) * tb_max;
+    if (need <= st->part_boxes || (st->part_refused && need >= st->part_refused)) return EXX_OK;
+    if (st->part_dev) {  // a larger batch than before (tile options changed)
+        cudaFree(st->part_dev);
+        c->dev_bytes -= sizeof(cplx) * Ng * st->part_boxes;
+        st->part_dev = nullptr;
+        st->part_boxes = 0;
+    }
+    if (test_fail_alloc("part") || cudaMalloc((void**)&st->part_dev, sizeof(cplx) * Ng * need) != cudaSuccess) {
+        cudaGetLastError();  // out of memory is not an error of this call: two sweeps need no partial boxes
+        st->part_dev = nullptr;
+        st->part_refused = need;
+        return EXX_OK;
+    }
+    st->part_boxes = need;
+    c->dev_bytes += sizeof(cplx) * Ng * need;
+    return EXX_OK;
+}
+
 // bands per side of a batch and whether the pair symmetry applies (options, workspace, shards); recorded in the counters
 static void fused_batch_shape(exx_ctx* c, int* ta, int* tb, bool* symmetry) {
     int ta_max = TMAX, tb_max = TMAX;
@@ -549,6 +567,7 @@ int fused_apply(exx_ctx* c, const double* occ, const double2* psi, double2* out,
     bool sym;
     fused_batch_shape(c, &ta_max, &tb_max, &sym);
     if (phi) sym = false, c->symmetry_used = 0;  // v_{b,a} = conj(v_{a,b}) pairs two bands of ONE set; here a and b come from different sets
+    if ((rc = fused_ensure_part(c, st, sym, ta_max, tb_max))) return rc;
     cplx* work = (cplx*)c->work_dev;
     // one accumulator box per (k, band), always fp64; exx_apply_to: per (k, trial vector), behind the trial vectors' boxes
     acc_c* acc = phi ? (acc_c*)(st->uphi_dev + Ng * st->uphi_boxes) : (acc_c*)c->acc_dev;

@@ -124,6 +124,10 @@ struct exx_ctx {
 namespace exx {
 
 void set_thread_error(const std::string& s);
+// Test hook for the out-of-memory branches, which a 180 GB device never takes by itself: while the environment variable
+// EXX_TEST_FAIL_ALLOC names `tag`, the device allocation carrying that tag reports failure without calling cudaMalloc.
+// Tags: "part" (partial boxes of the dual sweep), "acc" (accumulator boxes in ensure_big).  One getenv per tagged allocation.
+bool test_fail_alloc(const char* tag);
 int cuda_fail(exx_ctx* c, cudaError_t e, const char* what);
 
 #define EXX_CUDA(c, call)                                         \

@@ -5,8 +5,8 @@
 //
 // M = A^H B with A = psi (nb x npw, row-major, npw contiguous) and B = V_x psi (same layout):
 //   Re M_ij = sum_g (ar_ig br_jg + ai_ig bi_jg),   Im M_ij = sum_g (ar_ig bi_jg - ai_ig br_jg)
-// i.e. four real m8n8k4 products per 4 plane waves.  A warp owns one 8 x 8 tile of M over one slice of the plane waves
-// (split-K; 32 x 32 per warp, see the kernel); the slices are added in a fixed order by a second kernel, so the result is deterministic.
+// i.e. four real m8n8k4 products per 4 plane waves.  A warp owns one 32 x 32 tile of M (4 x 4 DMMA tiles of 8 x 8) over one slice of
+// the plane waves (split-K); the slices are added in a fixed order by a second kernel, so the result is deterministic.
 #include "exx_internal.h"
 
 namespace exx {

@@ -67,6 +67,14 @@ def test_create_rejects_bad_arguments_before_touching_the_gpu(L):
     assert L.exx_npw(None, 0, C.byref(n)) == -1 and n.value == 7
 
 
+def test_build_refuses_code_changing_flags_for_the_stamped_library():
+    """libexx.so carries the hash of the standard flags, so build() without out= accepts only ptxas verbosity as an extra."""
+    for extra in (["-Xptxas=-O0"], ["-Xptxas", "-O0"], ["-DEXX_DEFAULT_TILE=16"], ["-Xptxas", "-v", "-G"]):
+        with pytest.raises(ValueError):
+            build_mod.build(extra=extra)
+    assert build_mod.build(extra=["-Xptxas", "-v"]) == build_mod.LIB      # up to date: returns without compiling
+
+
 def test_workload_recipe():
     w = W.make("C4b")
     assert w.nk == 8 and w.nbands == 160 and w.nocc == 160 and w.pair_evals == 1638400

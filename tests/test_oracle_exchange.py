@@ -367,3 +367,22 @@ def test_apply_to_block_of_trial_vectors():
         lam = -sum(fj * 4 * np.pi / (Bm ** 2 * float((np.array(gv) - np.array(b)) @ (np.array(gv) - np.array(b)))) / o2.omega
                    for fj, b in zip(f, gm) if tuple(b) != tuple(gv))
         assert np.linalg.norm(out[i * o2.npw[0]:(i + 1) * o2.npw[0]] - lam * blk[i * o2.npw[0]:(i + 1) * o2.npw[0]]) <= 1e-13 * abs(lam)
+
+
+def test_stored_oracle_results_equal_the_survey_probe():
+    """tests/golden/exx_C{1,2,3}.json were written by make_golden.py from oracle/ alone.  SURVEY.md section 8(c)-PINS records the same
+    three configurations evaluated independently during the survey (numpy.fft, a different program): E_x, the norm of the first
+    output row and the checksum of the first index map.  A regenerated golden file that drifts from them fails here, without a GPU."""
+    import json
+    import os
+    gold_dir = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    survey = {"C1": (-0.0623251812923801, 0.01853725795907376, 1402128),
+              "C2": (-0.244336120072931, 0.028385606397239974, 77343110),
+              "C3": (-1.4051059069325562, 0.04419327891533337, 2015122368)}
+    for name, (ex, norm0, map0) in survey.items():
+        gold = json.load(open(os.path.join(gold_dir, "exx_%s.json" % name)))
+        assert gold["rows"][0] == [0, 0]
+        assert abs(gold["E_x_E1"] - ex) <= 1e-13 * abs(ex), name
+        assert abs(gold["E_x_E2"] - ex) <= 1e-13 * abs(ex), name
+        assert abs(gold["row_norm"][0] - norm0) <= 1e-13 * norm0, name
+        assert gold["map0_sum"] == map0, name

@@ -119,7 +119,9 @@ def run_reference(args, rank, world):
 # algorithmic bytes per work unit of each kernel class, in units of Ng bytes:
 # a generic box pass reads and writes one complex128 box (32 Ng); each fused pass moves 32 Ng per pair box (96 Ng for the
 # three passes = the B_model of the pair evaluation; the dual sweep of pass C serves both accumulations of a symmetric pair
-# and is still booked at 32 Ng per box: work box 16 + one u read 16); pass R reads one partial box (16 Ng) per unit.
+# and is still booked at 32 Ng per box: work box 16 + one u read 16); pass R is booked at the partial box it reads (16 Ng per unit);
+# its read-modify-write of the accumulator (32 Ng per COLUMN, shared by the up to tile_n/RG partial boxes of that column: 4 Ng per
+# unit at C4a, 19.9 B/pt measured) is not a per-unit quantity and is left out: a lower bound, used only if pass R ever dominates.
 BYTES_PER_UNIT_NG = {"fft_axis_generic": 32, "codensity": 32, "kernel_multiply": 32, "accumulate": 32,
                      "fused_pass_a": 32, "fused_pass_b": 32, "fused_pass_c": 32, "fused_fft_pass": 32, "fused_pass_r": 16,
                      "scatter": 16, "gather": 16}
@@ -392,7 +394,23 @@ def run_ours(args, rank, world, local):
         sync_all()
         ms_s = s0.elapsed_time(s1) / reps
         fl = 8.0 * w.nbands * w.nbands * g.npw[0]
+        # yardstick only, never on the product path: the same contraction as a library ZGEMM (torch.matmul -> cuBLAS)
+        a_m = pd[g.offsets[0]:g.offsets[0] + w.nbands * g.npw[0]].view(w.nbands, g.npw[0])
+        b_m = out[g.offsets[0]:g.offsets[0] + w.nbands * g.npw[0]].view(w.nbands, g.npw[0])
+        bt = b_m.t().contiguous()
+        ref_m = torch.matmul(a_m.conj(), bt)
+        sync_all()
+        y0, y1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        y0.record()
+        for _ in range(reps):
+            torch.matmul(a_m.conj(), bt, out=ref_m)
+        y1.record()
+        sync_all()
+        ms_y = y0.elapsed_time(y1) / reps
         subspace = {"shape": [w.nbands, w.nbands, g.npw[0]], "ms_per_call": ms_s, "gflops": fl / (ms_s * 1e-3) / 1e9,
+                    "yardstick_cublas_zgemm": {"ms_per_call": ms_y, "gflops": fl / (ms_y * 1e-3) / 1e9,
+                                               "max_abs_diff": float((ref_m - m).abs().max().item()),
+                                               "note": "torch.matmul(conj(A), B^T) on the same operands (conj materialised inside the timed call); a yardstick, not on the product path"},
                     "fp64_peak_gflops_measured": fp64_peak, "frac_of_fp64_peak": fl / (ms_s * 1e-3) / 1e9 / fp64_peak,
                     "kernel": "mma.sync.m8n8k4.f64 (DMMA), 32 x 32 tile per warp, split-K with fixed-order reduction",
                     "hermiticity_defect": float((m - m.conj().T).abs().max().item()) if w.nocc == w.nbands else None}
@@ -423,7 +441,10 @@ def run_ours(args, rank, world, local):
                        "path": {1: "generic", 2: "fused"}.get(g.get_info(B.EXX_INFO_PATH_USED)),
                        "tile_n": g.get_info(B.EXX_INFO_TILE_N), "tile_m": g.get_info(B.EXX_INFO_TILE_M),
                        "pruned": g.get_info(B.EXX_INFO_PRUNED), "pair_symmetry": g.get_info(B.EXX_INFO_SYMMETRY), "work_grid": pipeline["work_grid"],
-                       "pairs_executed_per_step": pairs_exec, "dual_sweep": g.get_option(B.EXX_OPT_DUAL_SWEEP),
+                       "pairs_executed_per_step": pairs_exec,
+                       # whether the dual-sweep kernel RAN in the timed applies (pass R launches > 0), not the option's value: grids
+                       # without a dual kernel (40^3, 64^3, 128^3) run two sweeps whatever EXX_OPT_DUAL_SWEEP says
+                       "dual_sweep": int(acc.get("fused_pass_r", (0.0, 0, 0))[1] > 0), "dual_sweep_option": g.get_option(B.EXX_OPT_DUAL_SWEEP),
                        "l2": "inputs larger than L2: the real-space cache u_nk(r) is %.2f GB, streamed every step" % (w.nk * w.nbands * ngw * 16 / 1e9)},
             "E_x": ex, "vx_apply_ms": ms, "clocks": sampler.summary(), "roofline": roofline, "pipeline_roofline": pipeline,
             "e2e": {"value": job_pairs / (ms_e2e * 1e-3), "unit": UNIT, "ms_per_step": ms_e2e,

@@ -125,7 +125,7 @@ def run_reference(args, rank, world):
 BYTES_PER_UNIT_NG = {"fft_axis_generic": 32, "codensity": 32, "kernel_multiply": 32, "accumulate": 32,
                      "fused_pass_a": 32, "fused_pass_b": 32, "fused_pass_c": 32, "fused_fft_pass": 32, "fused_pass_r": 16,
                      "scatter": 16, "gather": 16}
-NCU_COUNTERS = os.path.join(ROOT, "profiles", "ncu_counters_r2.json")
+NCU_COUNTERS = os.path.join(ROOT, "profiles", "ncu_counters_r3.json")
 
 
 def lib_source_hash():
@@ -139,7 +139,7 @@ def lib_source_hash():
 
 def ncu_counters(ngw):
     """Per-unit DRAM bytes and fp64 instruction counts of the fused kernels from the committed `ncu --set full` capture
-    (profiles/ncu_counters_r2.json), or (None, why) when that capture was taken from other sources or another work grid:
+    (profiles/ncu_counters_r3.json), or (None, why) when that capture was taken from other sources or another work grid:
     a stale capture is never printed."""
     try:
         tj = json.load(open(NCU_COUNTERS))
@@ -149,7 +149,7 @@ def ncu_counters(ngw):
         return None, "capture is of another build (source hash differs)"
     if tj.get("work_grid", 0) ** 3 != ngw:
         return None, "capture is of another work grid"
-    return tj, "profiles/ncu_counters_r2.json (%s)" % tj.get("source", "")
+    return tj, "profiles/ncu_counters_r3.json (%s)" % tj.get("source", "")
 
 
 def run_ours(args, rank, world, local):
@@ -412,7 +412,7 @@ def run_ours(args, rank, world, local):
                                                "max_abs_diff": float((ref_m - m).abs().max().item()),
                                                "note": "torch.matmul(conj(A), B^T) on the same operands (conj materialised inside the timed call); a yardstick, not on the product path"},
                     "fp64_peak_gflops_measured": fp64_peak, "frac_of_fp64_peak": fl / (ms_s * 1e-3) / 1e9 / fp64_peak,
-                    "kernel": "mma.sync.m8n8k4.f64 (DMMA), 32 x 32 tile per warp, split-K with fixed-order reduction",
+                    "kernel": "mma.sync.m8n8k4.f64 (DMMA), 32 x 32 tile per warp, register-pipelined fragment loads, split-K with fixed-order reduction",
                     "hermiticity_defect": float((m - m.conj().T).abs().max().item()) if w.nocc == w.nbands else None}
 
     # ---- timed region 3: end to end through exx_apply_host, pinned host buffers, copies inside the timed region
